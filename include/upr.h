@@ -1,0 +1,180 @@
+/*
+ * upr.h -- C ABI of libupr: B200 (sm_100a) ranking cross-attention over a shared user-history
+ * KV cache, the serving hot path of UniPinRec (arxiv/paper_2606_00422; citations below are
+ * lines of /root/reference/PAPER.md).
+ *
+ * What the path computes: for every user b, each of that
+ * user's C_b candidate items attends -- softmax scaled-dot-product attention -- over the
+ * user's L_b cached, candidate-independent history keys/values, never over other
+ * candidates; optionally a candidate also attends to its own key/value (the identity block
+ * of the paper's M-FALCON mask).  The history K/V live in a pool written by
+ * the retrieval stage, shape [layers, slots, heads, n, D], and each ranking
+ * request copies its slot into a decode cache -- here a packed ragged cache.
+ *
+ * Conventions (all entry points):
+ *  - Plain C. No exceptions cross the boundary; every function returns a upr_status and
+ *    upr_last_error() returns a thread-local message for the last failure.
+ *  - The caller owns all memory. The library never allocates or frees device memory.
+ *    "device" pointers must be accessible from the current CUDA device; "host" pointers
+ *    are ordinary host memory.
+ *  - Device work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy
+ *    default stream) and the calls never synchronise: they are asynchronous and CUDA-graph
+ *    capturable.  No host read of any device table happens.
+ *  - Only NVIDIA B200 / sm_100a is supported. There is no CPU fallback and no alternative
+ *    backend: unsupported arguments return UPR_ERR_UNSUPPORTED, never a slow path.
+ *  - Head dim d must be 64 or 128.
+ *
+ * Packed cache layout ("decode cache"; upr_kv_cache_layout describes it):
+ *    element (layer l, head h, user b, key j, t) of K (or V) is at element index
+ *        ((l*H + h) * R + row_off[b] + j) * d + t
+ *    row_off[0] = 0, row_off[b+1] = row_off[b] + round_up(L_b, UPR_ROW_ALIGN), R = row_off[B].
+ *    The rows [L_b, round_up(L_b,16)) of each user must hold finite values (upr_kv_pack
+ *    writes zeros).  After the last (layer, head) block the buffer extends by
+ *    UPR_TAIL_ROWS rows (any content; they are read by the last tile's TMA box, never
+ *    used).  A cache buffer must therefore be at least layout.bytes_cache bytes and
+ *    128-byte aligned (torch allocations are).
+ */
+#ifndef UPR_H_
+#define UPR_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  UPR_OK = 0,
+  UPR_ERR_INVALID_ARG = 1, /* NULL where not allowed, negative size, bad enum */
+  UPR_ERR_UNSUPPORTED = 2, /* d not in {64,128}, dtype combination not implemented */
+  UPR_ERR_WORKSPACE = 3,   /* workspace missing or too small */
+  UPR_ERR_CUDA = 4         /* a CUDA runtime/driver call failed (message in upr_last_error) */
+} upr_status;
+
+typedef enum { UPR_F32 = 0, UPR_BF16 = 1, UPR_FP8_E4M3 = 2 } upr_dtype;
+
+#define UPR_ROW_ALIGN 16  /* rows; every user's block starts on a multiple of this */
+#define UPR_TAIL_ROWS 128 /* rows of slack after the last block (one TMA box) */
+
+/* Integer description of a packed cache. All sizes in bytes unless named *_rows / R. */
+typedef struct upr_kv_layout {
+  int32_t B, H, d, n_layers;
+  int32_t dtype;      /* upr_dtype of the cache elements */
+  int32_t row_align;  /* = UPR_ROW_ALIGN */
+  int32_t tail_rows;  /* = UPR_TAIL_ROWS */
+  int32_t elem_bytes; /* 4, 2 or 1 */
+  int64_t R;          /* rows per (layer, head) block = sum_b round_up(L_b, row_align) */
+  int64_t row_bytes;
+  int64_t head_stride_bytes;
+  int64_t layer_stride_bytes;
+  int64_t bytes_cache;  /* bytes of ONE cache (K or V), tail rows included */
+  int64_t bytes_scales; /* bytes of ONE scale table: n_layers*H*4 for FP8, else 0 */
+} upr_kv_layout;
+
+/*
+ * a0 -- layout / offsets (integer only, host only, deterministic; the CPU oracle mirrors it
+ * bit for bit).  PAPER.md:202-204 fixes the pool; the ragged packed form is this library's.
+ *   seq_lens  host  [B] history lengths L_b >= 0
+ *   out       host  receives the layout
+ *   row_off   host  [B+1] receives the row offsets, or NULL
+ * Errors: INVALID_ARG for NULL out / negative sizes or lengths; UNSUPPORTED for d or dtype.
+ * B == 0 is valid (R = 0).
+ */
+upr_status upr_kv_cache_layout(const int32_t* seq_lens, int B, int H, int d, int n_layers,
+                               upr_dtype dtype, upr_kv_layout* out, int64_t* row_off);
+
+/*
+ * a1 -- pack: the slot -> decode-cache copy of PAPER.md:204 ("each ranking consumer copies
+ * each request's past KV from its slot in the mapped pool into its own decode cache").
+ *   k_pool, v_pool  device  bf16 [n_layers, S, H, n_max, d]  (PAPER.md:202 [L,S,H,n,D]);
+ *                           user b's valid rows are [0, L_b) of slot slot_ids[b]
+ *   slot_ids        device  int32 [B], each in [0, S)
+ *   seq_lens        device  int32 [B], each in [0, n_max]
+ *   layout          host    from upr_kv_cache_layout for the same lengths
+ *   k_cache,v_cache device  layout->bytes_cache bytes each; fully written (valid rows,
+ *                           zeroed alignment padding and tail)
+ *   k_scale,v_scale device  fp32 [n_layers*H]; written when layout->dtype is FP8, else
+ *                           ignored (may be NULL)
+ * dtype BF16: bit-exact 16-bit copy.  dtype F32: exact widening.  dtype FP8_E4M3 (format
+ * "fn": max finite 448, no infinities): per (layer, head) amax over all users' valid
+ * rows; scale = amax / 448.0f (fp32 divide; amax == 0 -> 1.0f); stored byte =
+ * cvt.rn.satfinite.e4m3( x * (448.0f / amax) ) with the product rounded once in fp32.
+ * Either pool/cache pair may be NULL to pack only the other.
+ */
+upr_status upr_kv_pack(const void* k_pool, const void* v_pool, int S, int n_max,
+                       const int32_t* slot_ids, const int32_t* seq_lens,
+                       const upr_kv_layout* layout, void* k_cache, void* v_cache, float* k_scale,
+                       float* v_scale, void* stream);
+
+/*
+ * a2-a7 -- the named entry point: one layer, softmax scale 1/sqrt(d), no self term,
+ * no split-K.  For every user b and candidate c in [cand_offsets[b], cand_offsets[b+1]):
+ *     out[c,h,:] = softmax_j( q[c,h,:] . K[b,h,j,:] / sqrt(d) ) @ V[b,h,:,:],  j < L_b
+ * (PAPER.md:138, 198, 255).  A candidate with no key at all gets zeros.
+ *   q            device  [total_q, H, d] row-major; bf16, or fp32 when dtype == UPR_F32
+ *   k_cache,v_cache device packed cache of `dtype` for ONE layer (layout above, n_layers=1);
+ *                   FP8 caches are read with unit scales here (use _ex for scales)
+ *   seq_lens     device  int32 [B]
+ *   cand_offsets device  int32 [B+1], non-decreasing, [0] = 0, [B] = total_q
+ *   out          device  fp32 [total_q, H, d]
+ * B == 0 returns UPR_OK without a launch.
+ */
+upr_status upr_cross_attn_fwd(const void* q, const void* k_cache, const void* v_cache,
+                              const int32_t* seq_lens, const int32_t* cand_offsets, float* out,
+                              int B, int H, int d, upr_dtype dtype, void* stream);
+
+/* Extended call: layers, self term, FP8 scales, split-K. Zero-initialise, then fill. */
+typedef struct upr_attn_params {
+  const void* q;               /* device [n_layers, total_q, H, d], q_dtype */
+  const void* k_cache;         /* device packed cache, kv_dtype */
+  const void* v_cache;
+  const int32_t* seq_lens;     /* device [B] */
+  const int32_t* cand_offsets; /* device [B+1] */
+  float* out;                  /* device fp32 [n_layers, total_q, H, d] */
+  const void* k_self;          /* device, same shape/dtype as q, or NULL: the candidate's own */
+  const void* v_self;          /*   key/value joins its softmax (PAPER.md:198 identity mask) */
+  const float* k_scale;        /* device fp32 [n_layers*H] or NULL (=1): FP8 dequant scales */
+  const float* v_scale;
+  int32_t B, H, d, n_layers;
+  int32_t kv_dtype;            /* upr_dtype of the caches */
+  int32_t q_dtype;             /* UPR_BF16 or UPR_F32 (q, k_self, v_self) */
+  int64_t total_q;             /* host copy of cand_offsets[B] */
+  float sm_scale;              /* softmax scale; 0 -> 1/sqrt(d) */
+  int32_t num_splits;          /* split-K factor along the history; 0 -> heuristic, 1 -> off */
+  int32_t max_seq_len;         /* hint for the heuristic (0 = unknown) */
+  void* workspace;             /* device, >= upr_cross_attn_workspace_bytes(), 256-B aligned */
+  size_t workspace_bytes;
+} upr_attn_params;
+
+/* Bytes of workspace upr_cross_attn_fwd_ex needs for these params (dynamic-scheduler
+ * counter + split-K partial states (m, l, O~), a8). Returns 0 on invalid params. */
+size_t upr_cross_attn_workspace_bytes(const upr_attn_params* p);
+
+/* Number of history splits the heuristic picks for these params (>= 1). */
+int upr_cross_attn_num_splits(const upr_attn_params* p);
+
+/*
+ * a2-a8 -- extended forward. As upr_cross_attn_fwd, per layer, plus:
+ *  - self term (k_self/v_self non-NULL): logit scale*<q_c, k_self_c> joins candidate c's
+ *    softmax and v_self_c its weighted sum; with L_b == 0 the output is v_self_c.
+ *  - FP8: K = e4m3(byte) * k_scale[l*H+h], V likewise; dequantised in registers, MMA in bf16.
+ *  - split-K: the history is cut into num_splits ranges of whole 128-key tiles, each CTA
+ *    writes its partial (m, l, O~) to the workspace and a combine kernel merges them.
+ * Errors: WORKSPACE if workspace is NULL/too small; others as above.
+ */
+upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream);
+
+/* Kernel launches the last successful call on this thread enqueued (for accounting). */
+int upr_last_launch_count(void);
+
+/* Thread-local description of the last error on this thread ("" if none). */
+const char* upr_last_error(void);
+
+/* Library version string, e.g. "upr 0.1 sm_100a". */
+const char* upr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UPR_H_ */

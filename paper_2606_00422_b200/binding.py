@@ -1,0 +1,173 @@
+"""ctypes binding of libupr.so: same names as include/upr.h, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+UPR_F32, UPR_BF16, UPR_FP8_E4M3 = 0, 1, 2
+UPR_ROW_ALIGN, UPR_TAIL_ROWS = 16, 128
+EXPORTED_SYMBOLS = [
+    "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
+    "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
+    "upr_last_error", "upr_version",
+]
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libupr.so")
+
+
+class UprError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libupr status {status}: {msg}")
+        self.status = status
+
+
+class KvLayout(ctypes.Structure):
+    _fields_ = [
+        ("B", ctypes.c_int32), ("H", ctypes.c_int32), ("d", ctypes.c_int32), ("n_layers", ctypes.c_int32),
+        ("dtype", ctypes.c_int32), ("row_align", ctypes.c_int32), ("tail_rows", ctypes.c_int32),
+        ("elem_bytes", ctypes.c_int32), ("R", ctypes.c_int64), ("row_bytes", ctypes.c_int64),
+        ("head_stride_bytes", ctypes.c_int64), ("layer_stride_bytes", ctypes.c_int64),
+        ("bytes_cache", ctypes.c_int64), ("bytes_scales", ctypes.c_int64),
+    ]
+
+
+class _AttnParams(ctypes.Structure):
+    _fields_ = [
+        ("q", ctypes.c_void_p), ("k_cache", ctypes.c_void_p), ("v_cache", ctypes.c_void_p),
+        ("seq_lens", ctypes.c_void_p), ("cand_offsets", ctypes.c_void_p), ("out", ctypes.c_void_p),
+        ("k_self", ctypes.c_void_p), ("v_self", ctypes.c_void_p),
+        ("k_scale", ctypes.c_void_p), ("v_scale", ctypes.c_void_p),
+        ("B", ctypes.c_int32), ("H", ctypes.c_int32), ("d", ctypes.c_int32), ("n_layers", ctypes.c_int32),
+        ("kv_dtype", ctypes.c_int32), ("q_dtype", ctypes.c_int32),
+        ("total_q", ctypes.c_int64), ("sm_scale", ctypes.c_float), ("num_splits", ctypes.c_int32),
+        ("max_seq_len", ctypes.c_int32), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
+    ]
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def _load() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        path = lib_path()
+        if not os.path.exists(path):
+            raise ImportError(
+                f"{path} is missing: build it with `python -m paper_2606_00422_b200.build` "
+                "(nvcc, sm_100a). There is no CPU fallback.")
+        lib = ctypes.CDLL(path)
+        lib.upr_last_error.restype = ctypes.c_char_p
+        lib.upr_version.restype = ctypes.c_char_p
+        lib.upr_last_launch_count.restype = ctypes.c_int
+        lib.upr_cross_attn_workspace_bytes.restype = ctypes.c_size_t
+        lib.upr_cross_attn_workspace_bytes.argtypes = [ctypes.POINTER(_AttnParams)]
+        lib.upr_cross_attn_num_splits.restype = ctypes.c_int
+        lib.upr_cross_attn_num_splits.argtypes = [ctypes.POINTER(_AttnParams)]
+        lib.upr_kv_cache_layout.restype = ctypes.c_int
+        lib.upr_kv_cache_layout.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                            ctypes.c_int, ctypes.POINTER(KvLayout), ctypes.c_void_p]
+        lib.upr_kv_pack.restype = ctypes.c_int
+        lib.upr_kv_pack.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
+                                    ctypes.c_void_p, ctypes.POINTER(KvLayout), ctypes.c_void_p, ctypes.c_void_p,
+                                    ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.upr_cross_attn_fwd.restype = ctypes.c_int
+        lib.upr_cross_attn_fwd.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_int] * 4 + [ctypes.c_void_p]
+        lib.upr_cross_attn_fwd_ex.restype = ctypes.c_int
+        lib.upr_cross_attn_fwd_ex.argtypes = [ctypes.POINTER(_AttnParams), ctypes.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _check(status: int) -> None:
+    if status != 0:
+        raise UprError(status, _load().upr_last_error().decode())
+
+
+def _ptr(t: Optional[torch.Tensor]) -> Optional[int]:
+    if t is None:
+        return None
+    assert t.is_contiguous(), "libupr takes contiguous tensors"
+    return t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream or None
+
+
+def upr_version() -> str:
+    return _load().upr_version().decode()
+
+
+def upr_last_launch_count() -> int:
+    return int(_load().upr_last_launch_count())
+
+
+def upr_kv_cache_layout(seq_lens, H: int, d: int, n_layers: int, dtype: int):
+    """Host-only. seq_lens: host int32 array-like [B]. Returns (KvLayout, row_off int64 [B+1])."""
+    sl = np.ascontiguousarray(np.asarray(seq_lens, dtype=np.int32))
+    B = int(sl.shape[0])
+    lay = KvLayout()
+    row_off = np.zeros(B + 1, dtype=np.int64)
+    _check(_load().upr_kv_cache_layout(sl.ctypes.data, B, H, d, n_layers, dtype, ctypes.byref(lay),
+                                       row_off.ctypes.data))
+    return lay, row_off
+
+
+def upr_kv_pack(k_pool, v_pool, slot_ids, seq_lens, layout: KvLayout, k_cache, v_cache,
+                k_scale=None, v_scale=None, stream=None) -> None:
+    """Pools: device bf16 [n_layers, S, H, n_max, d]; slot_ids/seq_lens: device int32 [B]."""
+    ref = k_pool if k_pool is not None else v_pool
+    S, n_max = int(ref.shape[1]), int(ref.shape[3])
+    _check(_load().upr_kv_pack(_ptr(k_pool), _ptr(v_pool), S, n_max, _ptr(slot_ids), _ptr(seq_lens),
+                               ctypes.byref(layout), _ptr(k_cache), _ptr(v_cache), _ptr(k_scale), _ptr(v_scale),
+                               _stream(stream)))
+
+
+def upr_cross_attn_fwd(q, k_cache, v_cache, seq_lens, cand_offsets, out, B: int, H: int, d: int, dtype: int,
+                       stream=None) -> None:
+    _check(_load().upr_cross_attn_fwd(_ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(seq_lens), _ptr(cand_offsets),
+                                      _ptr(out), B, H, d, dtype, _stream(stream)))
+
+
+def _params(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers, kv_dtype, q_dtype, total_q,
+            k_self=None, v_self=None, k_scale=None, v_scale=None, sm_scale=0.0, num_splits=0, max_seq_len=0,
+            workspace=None) -> _AttnParams:
+    p = _AttnParams()
+    p.q, p.k_cache, p.v_cache = _ptr(q), _ptr(k_cache), _ptr(v_cache)
+    p.seq_lens, p.cand_offsets, p.out = _ptr(seq_lens), _ptr(cand_offsets), _ptr(out)
+    p.k_self, p.v_self, p.k_scale, p.v_scale = _ptr(k_self), _ptr(v_self), _ptr(k_scale), _ptr(v_scale)
+    p.B, p.H, p.d, p.n_layers, p.kv_dtype, p.q_dtype = B, H, d, n_layers, kv_dtype, q_dtype
+    p.total_q, p.sm_scale, p.num_splits, p.max_seq_len = total_q, sm_scale, num_splits, max_seq_len
+    p.workspace = _ptr(workspace)
+    p.workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    return p
+
+
+def upr_cross_attn_workspace_bytes(B, H, d, n_layers, total_q, num_splits=0, max_seq_len=0) -> int:
+    p = _params(None, None, None, None, None, None, B, H, d, n_layers, UPR_BF16, UPR_BF16, total_q,
+                num_splits=num_splits, max_seq_len=max_seq_len)
+    return int(_load().upr_cross_attn_workspace_bytes(ctypes.byref(p)))
+
+
+def upr_cross_attn_num_splits(B, H, d, n_layers, total_q, num_splits=0, max_seq_len=0) -> int:
+    p = _params(None, None, None, None, None, None, B, H, d, n_layers, UPR_BF16, UPR_BF16, total_q,
+                num_splits=num_splits, max_seq_len=max_seq_len)
+    return int(_load().upr_cross_attn_num_splits(ctypes.byref(p)))
+
+
+def upr_cross_attn_fwd_ex(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers, kv_dtype, q_dtype,
+                          total_q, workspace, k_self=None, v_self=None, k_scale=None, v_scale=None, sm_scale=0.0,
+                          num_splits=0, max_seq_len=0, stream=None) -> None:
+    p = _params(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers, kv_dtype, q_dtype, total_q,
+                k_self, v_self, k_scale, v_scale, sm_scale, num_splits, max_seq_len, workspace)
+    _check(_load().upr_cross_attn_fwd_ex(ctypes.byref(p), _stream(stream)))

@@ -1,0 +1,639 @@
+// attn_kernel.cuh -- ranking-head cross-attention forward (steps a2-a7 of SURVEY.md 8(a)).
+//
+// For each user b, candidate rows q[c] (cand_offsets[b] <= c < cand_offsets[b+1]) attend over
+// that user's cached history K/V rows [0, L_b) -- never over other candidates (PAPER.md:138,
+// 198); optionally each candidate also sees its own key/value (identity block of the
+// M-FALCON mask).  out = softmax(scale * q K^T) V, fp32.
+//
+// Persistent, warp-specialised CTA (one per SM), work item = (layer, user, head, history
+// split, block of <= 256 candidates):
+//   warps 0-3 : softmax group for candidate tile 0 (rows   0..127), one thread per row
+//   warps 4-7 : softmax group for candidate tile 1 (rows 128..255)
+//   warp  8   : scheduler + TMA producer (decodes work items from the device offset tables,
+//               streams the user's K/V tiles HBM -> swizzled smem ring, once per item)
+//   warp  9   : tcgen05.mma issuer: S_t = Q_t K^T (SS), O_t += P_t V (A = P from TMEM)
+// TMEM (512 cols): S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [256+D,256+2D); P_t (bf16)
+// overwrites the first 64 columns of S_t once S_t has been read into registers.
+// Online softmax in fp32 with lazy rescaling of O (only when the running max grows by more
+// than 2^8); row reductions are thread-local because the 32x32b TMEM load gives each thread
+// a whole row.
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "ptx.cuh"
+
+namespace upr {
+
+constexpr int kTileM = 128;     // candidate rows per MMA tile == TMEM lanes
+constexpr int kTileN = 128;     // keys per K/V tile
+constexpr int kQBlock = 256;    // candidate rows per work item (two tiles)
+constexpr int kRowAlign = 16;   // UPR_ROW_ALIGN
+constexpr int kAttnThreads = 320;
+constexpr int kProducerWarp = 8;
+constexpr int kMmaWarp = 9;
+constexpr int kTmemCols = 512;
+constexpr float kRescaleTau = 8.0f;  // lazy-rescale threshold, log2 units
+
+struct AttnArgs {
+  const void* q;
+  const void* k_self;
+  const void* v_self;
+  float* out;
+  const int32_t* seq_lens;
+  const int32_t* cand_offsets;
+  const float* k_scale;
+  const float* v_scale;
+  float* part_o;          // split-K partial O~  [n_layers][total_q][H][ns][D]
+  float* part_ml;         // split-K partial (m, l) [n_layers][total_q][H][ns][2]
+  unsigned int* counter;  // dynamic work counter (zeroed before launch) or nullptr = static
+  int B, H, n_layers, num_splits;
+  int q_is_f32;
+  float scale_log2;       // sm_scale * log2(e)
+};
+
+struct WorkItem {
+  int valid;     // 0 = no more work
+  int layer, h, split;
+  int q_row0;    // first candidate row (global index into [total_q]) of this block
+  int n_rows;    // valid rows in this block (1..256)
+  int kv_row0;   // row into the 2-D [n_layers*H*R, d] cache view of the first key of the split
+  int key0;      // first key index (within the user) of this split
+  int n_keys;    // valid keys in this split's range (>= 0)
+  int total_q;   // cand_offsets[B]
+};
+
+template <int D>
+struct AttnCfg {
+  static constexpr int kBoxBytes = kTileN * 128;            // one [128 rows x 64 bf16] TMA box
+  static constexpr int kBoxes = D / 64;                     // boxes per tile
+  static constexpr int kTileBytes = kBoxBytes * kBoxes;     // Q tile, K tile or V tile
+  static constexpr int kStages = (D == 128) ? 5 : 8;        // K/V ring slots
+  static constexpr int kSmemQ = 2 * kTileBytes;
+  static constexpr int kSmemKV = kStages * kTileBytes;
+  static constexpr int kSmemCtrl = 1024;
+  static constexpr int kSmemTotal = kSmemQ + kSmemKV + kSmemCtrl + 1024;  // + alignment slack
+  static constexpr uint32_t kIdescQK = make_idesc_bf16(kTileM, kTileN, 0, 0);
+  static constexpr uint32_t kIdescPV = make_idesc_bf16(kTileM, D, 0, 1);
+};
+
+struct __align__(8) AttnCtrl {
+  uint64_t kv_full[8];
+  uint64_t kv_empty[8];
+  uint64_t q_full[2];
+  uint64_t s_full[2];
+  uint64_t p_full[2];
+  uint64_t o_full[2];
+  uint64_t item_full[2];
+  uint64_t item_empty[2];
+  WorkItem items[2];
+  uint32_t tmem_base;
+};
+static_assert(sizeof(AttnCtrl) <= 1024, "control block too large");
+
+// ---------------------------------------------------------------------------------------
+// Scheduler state: a forward-only cursor over users, 32 at a time (one per lane).
+// ---------------------------------------------------------------------------------------
+struct UserCursor {
+  int b0;           // first user of the current 32-user window
+  int w_before;     // work items of users < b0 (within one layer)
+  int rows_before;  // aligned cache rows of users < b0
+};
+
+__device__ __forceinline__ int warp_incl_scan(int v, int lane) {
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    int t = __shfl_up_sync(0xffffffffu, v, o);
+    if (lane >= o) v += t;
+  }
+  return v;
+}
+
+// items and aligned rows of user u (0 if u >= B)
+__device__ __forceinline__ void user_sizes(const AttnArgs& a, int u, int& w, int& rows, int& C,
+                                           int& L) {
+  w = 0; rows = 0; C = 0; L = 0;
+  if (u < a.B) {
+    int c0 = __ldg(a.cand_offsets + u), c1 = __ldg(a.cand_offsets + u + 1);
+    C = c1 - c0;
+    L = __ldg(a.seq_lens + u);
+    int nq = (C + kQBlock - 1) / kQBlock;
+    w = nq * a.H * a.num_splits;
+    rows = (L + kRowAlign - 1) / kRowAlign * kRowAlign;
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// Q tile: global [rows, H*D] (bf16 or fp32) -> bf16 smem in the 128B-swizzled K-major layout
+// the UMMA descriptor expects (identical to what a SWIZZLE_128B TMA box would write).
+// ---------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void load_q_tile(uint32_t tile_smem, const void* q, bool q_is_f32,
+                                            size_t elem_base, size_t row_stride, int rows_valid,
+                                            int tid128) {
+  constexpr int CPR = D / 8;  // 16-byte bf16 chunks per row
+#pragma unroll 4
+  for (int i = 0; i < CPR; ++i) {
+    int id = i * 128 + tid128;
+    int row = id / CPR, c = id % CPR;
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (row < rows_valid) {
+      size_t e = elem_base + static_cast<size_t>(row) * row_stride + static_cast<size_t>(c) * 8;
+      if (!q_is_f32) {
+        v = __ldg(reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(q) + e));
+      } else {
+        const float4* p = reinterpret_cast<const float4*>(static_cast<const float*>(q) + e);
+        float4 a = __ldg(p), b = __ldg(p + 1);
+        v.x = pack_bf16x2(a.x, a.y);
+        v.y = pack_bf16x2(a.z, a.w);
+        v.z = pack_bf16x2(b.x, b.y);
+        v.w = pack_bf16x2(b.z, b.w);
+      }
+    }
+    int box = c >> 3, cc = c & 7;
+    uint32_t addr = tile_smem + box * (kTileM * 128) + row * 128 + ((cc ^ (row & 7)) << 4);
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y),
+                 "r"(v.z), "r"(v.w)
+                 : "memory");
+  }
+}
+
+// dot(q_row, kself_row) for the self logit; both rows in global, bf16 or fp32
+template <int D>
+__device__ __forceinline__ float row_dot(const void* a, const void* b, bool is_f32, size_t e) {
+  float acc = 0.f;
+  if (!is_f32) {
+    const uint4* pa = reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(a) + e);
+    const uint4* pb = reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(b) + e);
+#pragma unroll 4
+    for (int i = 0; i < D / 8; ++i) {
+      uint4 x = __ldg(pa + i), y = __ldg(pb + i);
+      const __nv_bfloat162* xs = reinterpret_cast<const __nv_bfloat162*>(&x);
+      const __nv_bfloat162* ys = reinterpret_cast<const __nv_bfloat162*>(&y);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        float2 fx = __bfloat1622float2(xs[k]), fy = __bfloat1622float2(ys[k]);
+        acc = fmaf(fx.x, fy.x, acc);
+        acc = fmaf(fx.y, fy.y, acc);
+      }
+    }
+  } else {
+    const float4* pa = reinterpret_cast<const float4*>(static_cast<const float*>(a) + e);
+    const float4* pb = reinterpret_cast<const float4*>(static_cast<const float*>(b) + e);
+#pragma unroll 4
+    for (int i = 0; i < D / 4; ++i) {
+      float4 x = __ldg(pa + i), y = __ldg(pb + i);
+      acc = fmaf(x.x, y.x, acc);
+      acc = fmaf(x.y, y.y, acc);
+      acc = fmaf(x.z, y.z, acc);
+      acc = fmaf(x.w, y.w, acc);
+    }
+  }
+  return acc;
+}
+
+__device__ __forceinline__ float load_elem_f(const void* p, bool is_f32, size_t e) {
+  return is_f32 ? __ldg(static_cast<const float*>(p) + e)
+                : __bfloat162float(static_cast<const __nv_bfloat16*>(p)[e]);
+}
+
+// ---------------------------------------------------------------------------------------
+// The kernel
+// ---------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(kAttnThreads, 1)
+upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
+                    const __grid_constant__ CUtensorMap tmap_v, const AttnArgs args) {
+  using Cfg = AttnCfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem_aligned = smem_raw + (smem_base - smem_u32(smem_raw));
+  const uint32_t q_smem = smem_base;
+  const uint32_t kv_smem = smem_base + Cfg::kSmemQ;
+  AttnCtrl* ctrl = reinterpret_cast<AttnCtrl*>(smem_aligned + Cfg::kSmemQ + Cfg::kSmemKV);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  // ------------------------------------------------------------------ one-time setup
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < Cfg::kStages; ++i) {
+      mbar_init(smem_u32(&ctrl->kv_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->kv_empty[i]), 1);
+    }
+    for (int t = 0; t < 2; ++t) {
+      mbar_init(smem_u32(&ctrl->q_full[t]), 128);
+      mbar_init(smem_u32(&ctrl->s_full[t]), 1);
+      mbar_init(smem_u32(&ctrl->p_full[t]), 128);
+      mbar_init(smem_u32(&ctrl->o_full[t]), 1);
+      mbar_init(smem_u32(&ctrl->item_full[t]), 1);
+      mbar_init(smem_u32(&ctrl->item_empty[t]), 257);  // 256 softmax threads + MMA lane 0
+    }
+    fence_mbar_init();
+  }
+  if (warp == kProducerWarp) {
+    if (lane == 0) {
+      tma_prefetch_desc(&tmap_k);
+      tma_prefetch_desc(&tmap_v);
+    }
+  }
+  if (warp == kMmaWarp) {
+    tmem_alloc(smem_u32(&ctrl->tmem_base), kTmemCols);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = ctrl->tmem_base;
+
+  if (warp == kProducerWarp) {
+    // ================================================================= scheduler + TMA
+    // one pass over the users: items per layer (W) and aligned rows per (layer, head) (R)
+    int W = 0, R = 0;
+    for (int u0 = 0; u0 < args.B; u0 += 32) {
+      int w, rows, C, L;
+      user_sizes(args, u0 + lane, w, rows, C, L);
+      W += w;
+      R += rows;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      W += __shfl_xor_sync(0xffffffffu, W, o);
+      R += __shfl_xor_sync(0xffffffffu, R, o);
+    }
+    const int total_items = W * args.n_layers;
+    const int total_q = (args.B > 0) ? __ldg(args.cand_offsets + args.B) : 0;
+
+    UserCursor cur{0, 0, 0};
+    uint32_t kv_it = 0;
+    for (uint32_t n = 0;; ++n) {
+      const int islot = n & 1;
+      mbar_wait(smem_u32(&ctrl->item_empty[islot]), ((n >> 1) & 1) ^ 1);
+      int idx;
+      if (args.counter != nullptr) {
+        idx = 0;
+        if (lane == 0) idx = static_cast<int>(atomicAdd(args.counter, 1u));
+        idx = __shfl_sync(0xffffffffu, idx, 0);
+      } else {
+        idx = static_cast<int>(blockIdx.x + n * gridDim.x);
+      }
+      if (idx >= total_items) {
+        if (lane == 0) {
+          ctrl->items[islot].valid = 0;
+          mbar_arrive(smem_u32(&ctrl->item_full[islot]));
+        }
+        break;
+      }
+      const int layer = idx / W;
+      const int r = idx - layer * W;
+      if (r < cur.w_before) cur = UserCursor{0, 0, 0};
+      // advance the window until it contains item r
+      int w, rows, C, L, w_incl, rows_incl;
+      for (;;) {
+        user_sizes(args, cur.b0 + lane, w, rows, C, L);
+        w_incl = warp_incl_scan(w, lane);
+        rows_incl = warp_incl_scan(rows, lane);
+        int w_tot = __shfl_sync(0xffffffffu, w_incl, 31);
+        if (r < cur.w_before + w_tot) break;
+        cur.w_before += w_tot;
+        cur.rows_before += __shfl_sync(0xffffffffu, rows_incl, 31);
+        cur.b0 += 32;
+      }
+      const unsigned hit = __ballot_sync(0xffffffffu, cur.w_before + w_incl > r);
+      const int src = __ffs(hit) - 1;
+      const int local = r - (cur.w_before + __shfl_sync(0xffffffffu, w_incl - w, src));
+      const int row_off_b = cur.rows_before + __shfl_sync(0xffffffffu, rows_incl - rows, src);
+      const int Cb = __shfl_sync(0xffffffffu, C, src);
+      const int Lb = __shfl_sync(0xffffffffu, L, src);
+      const int b = cur.b0 + src;
+      const int nq = (Cb + kQBlock - 1) / kQBlock;
+      const int per_h = nq * args.num_splits;
+      const int h = local / per_h;
+      const int rem = local - h * per_h;
+      const int split = rem / nq;
+      const int qblk = rem - split * nq;
+      const int nt_user = (Lb + kTileN - 1) / kTileN;
+      const int t0 = static_cast<int>((static_cast<long long>(split) * nt_user) / args.num_splits);
+      const int t1 =
+          static_cast<int>((static_cast<long long>(split + 1) * nt_user) / args.num_splits);
+      const int key0 = t0 * kTileN;
+      const int n_keys = (t1 > t0) ? (min(Lb, t1 * kTileN) - key0) : 0;
+      const int kv_row0 = (layer * args.H + h) * R + row_off_b + key0;
+      if (lane == 0) {
+        WorkItem& it = ctrl->items[islot];
+        it.valid = 1;
+        it.layer = layer;
+        it.h = h;
+        it.split = split;
+        it.q_row0 = __ldg(args.cand_offsets + b) + qblk * kQBlock;
+        it.n_rows = min(kQBlock, Cb - qblk * kQBlock);
+        it.kv_row0 = kv_row0;
+        it.key0 = key0;
+        it.n_keys = n_keys;
+        it.total_q = total_q;
+        mbar_arrive(smem_u32(&ctrl->item_full[islot]));
+        // stream this item's K/V tiles: K0 V0 K1 V1 ...
+        const int nt = (n_keys + kTileN - 1) / kTileN;
+        for (int j = 0; j < nt; ++j) {
+#pragma unroll
+          for (int kv = 0; kv < 2; ++kv) {
+            const uint32_t slot = kv_it % Cfg::kStages;
+            const uint32_t ph = (kv_it / Cfg::kStages) & 1;
+            mbar_wait(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
+            const uint32_t full = smem_u32(&ctrl->kv_full[slot]);
+            mbar_arrive_expect_tx(full, Cfg::kTileBytes);
+            const uint32_t dst = kv_smem + slot * Cfg::kTileBytes;
+#pragma unroll
+            for (int bx = 0; bx < Cfg::kBoxes; ++bx)
+              tma_load_2d(dst + bx * Cfg::kBoxBytes, kv == 0 ? &tmap_k : &tmap_v, bx * 64,
+                          kv_row0 + j * kTileN, full);
+            ++kv_it;
+          }
+        }
+      }
+      __syncwarp();
+    }
+  } else if (warp == kMmaWarp) {
+    // ================================================================= MMA issuer
+    uint32_t kv_it = 0, q_it[2] = {0, 0}, sp_it[2] = {0, 0};
+    const uint32_t tm_s[2] = {tmem_base, tmem_base + 128};
+    const uint32_t tm_o[2] = {tmem_base + 256, tmem_base + 256 + D};
+    for (uint32_t n = 0;; ++n) {
+      const int islot = n & 1;
+      mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+      const WorkItem it = ctrl->items[islot];
+      if (!it.valid) break;
+      const int nt = (it.n_keys + kTileN - 1) / kTileN;
+      const int ntile = (it.n_rows > kTileM) ? 2 : 1;
+      if (nt > 0) {
+        for (int t = 0; t < ntile; ++t) {
+          mbar_wait(smem_u32(&ctrl->q_full[t]), q_it[t] & 1);
+          ++q_it[t];
+        }
+        tc_fence_after();
+        // S_t(0) = Q_t K(0)^T
+        {
+          const uint32_t slot = kv_it % Cfg::kStages, ph = (kv_it / Cfg::kStages) & 1;
+          mbar_wait(smem_u32(&ctrl->kv_full[slot]), ph);
+          tc_fence_after();
+          if (lane == 0) {
+            const uint32_t kb = kv_smem + slot * Cfg::kTileBytes;
+            for (int t = 0; t < ntile; ++t) {
+              const uint32_t qb = q_smem + t * Cfg::kTileBytes;
+#pragma unroll
+              for (int k = 0; k < D / 16; ++k) {
+                const uint32_t off = (k >> 2) * Cfg::kBoxBytes + (k & 3) * 32;
+                umma_ss(tm_s[t], make_smem_desc_sw128(qb + off, 16, 1024),
+                        make_smem_desc_sw128(kb + off, 16, 1024), Cfg::kIdescQK, k > 0);
+              }
+              umma_commit(smem_u32(&ctrl->s_full[t]));
+            }
+            umma_commit(smem_u32(&ctrl->kv_empty[slot]));
+          }
+          __syncwarp();
+          ++kv_it;
+        }
+        for (int j = 0; j < nt; ++j) {
+          const uint32_t vslot = kv_it % Cfg::kStages, vph = (kv_it / Cfg::kStages) & 1;
+          ++kv_it;
+          const bool has_next = (j + 1 < nt);
+          const uint32_t kslot = kv_it % Cfg::kStages, kph = (kv_it / Cfg::kStages) & 1;
+          mbar_wait(smem_u32(&ctrl->kv_full[vslot]), vph);
+          const int keys_here = min(kTileN, it.n_keys - j * kTileN);
+          const int ksteps = (keys_here + 15) >> 4;
+          for (int t = 0; t < ntile; ++t) {
+            mbar_wait(smem_u32(&ctrl->p_full[t]), sp_it[t] & 1);
+            ++sp_it[t];
+            tc_fence_after();
+            if (lane == 0) {
+              const uint32_t vb = kv_smem + vslot * Cfg::kTileBytes;
+              for (int k = 0; k < ksteps; ++k) {
+                // A = P_t[:, 16k..16k+16) : 8 TMEM columns of packed bf16 pairs
+                // B = V rows [16k, 16k+16) : MN-major, 8-row groups 1024 B apart, the two
+                //     64-column halves (D = 128) one box apart
+                umma_ts(tm_o[t], tm_s[t] + k * 8,
+                        make_smem_desc_sw128(vb + k * 2048, Cfg::kBoxBytes, 1024), Cfg::kIdescPV,
+                        (j > 0 || k > 0) ? 1u : 0u);
+              }
+            }
+            __syncwarp();
+            if (has_next && t == 0) {
+              mbar_wait(smem_u32(&ctrl->kv_full[kslot]), kph);
+              tc_fence_after();
+            }
+            if (lane == 0) {
+              if (has_next) {
+                const uint32_t kb = kv_smem + kslot * Cfg::kTileBytes;
+                const uint32_t qb = q_smem + t * Cfg::kTileBytes;
+#pragma unroll
+                for (int k = 0; k < D / 16; ++k) {
+                  const uint32_t off = (k >> 2) * Cfg::kBoxBytes + (k & 3) * 32;
+                  umma_ss(tm_s[t], make_smem_desc_sw128(qb + off, 16, 1024),
+                          make_smem_desc_sw128(kb + off, 16, 1024), Cfg::kIdescQK, k > 0);
+                }
+                umma_commit(smem_u32(&ctrl->s_full[t]));
+              } else {
+                umma_commit(smem_u32(&ctrl->o_full[t]));
+              }
+            }
+            __syncwarp();
+          }
+          if (lane == 0) {
+            umma_commit(smem_u32(&ctrl->kv_empty[vslot]));
+            if (has_next) umma_commit(smem_u32(&ctrl->kv_empty[kslot]));
+          }
+          __syncwarp();
+          if (has_next) ++kv_it;
+        }
+      }
+      if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+      __syncwarp();
+    }
+  } else {
+    // ================================================================= softmax groups
+    const int t = warp >> 2;                 // candidate tile of this group
+    const int tid128 = threadIdx.x & 127;    // row within the tile == TMEM lane
+    const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
+    const uint32_t tm_s = tmem_base + lane_base + t * 128;
+    const uint32_t tm_o = tmem_base + lane_base + 256 + t * D;
+    uint32_t sp_it = 0, o_it = 0;
+    const bool has_self = (args.k_self != nullptr);
+    const bool q32 = args.q_is_f32 != 0;
+
+    for (uint32_t n = 0;; ++n) {
+      const int islot = n & 1;
+      mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+      const WorkItem it = ctrl->items[islot];
+      if (!it.valid) break;
+      const int rows_here = min(kTileM, it.n_rows - t * kTileM);  // <= 0: tile inactive
+      if (rows_here > 0) {
+        const int nt = (it.n_keys + kTileN - 1) / kTileN;
+        const bool row_valid = tid128 < rows_here;
+        const size_t row_stride = static_cast<size_t>(args.H) * D;
+        const size_t tile_elem0 =
+            ((static_cast<size_t>(it.layer) * it.total_q + it.q_row0 + t * kTileM) * args.H +
+             it.h) * D;
+        const size_t my_elem0 = tile_elem0 + static_cast<size_t>(tid128) * row_stride;
+        if (nt > 0) {
+          load_q_tile<D>(q_smem + t * Cfg::kTileBytes, args.q, q32, tile_elem0, row_stride,
+                         rows_here, tid128);
+          fence_proxy_async_smem();
+          mbar_arrive(smem_u32(&ctrl->q_full[t]));
+        }
+        const int sidx = it.layer * args.H + it.h;
+        const float ks = args.k_scale ? __ldg(args.k_scale + sidx) : 1.0f;
+        const float vs = args.v_scale ? __ldg(args.v_scale + sidx) : 1.0f;
+        const float c_log2 = args.scale_log2 * ks;  // multiplies raw S
+
+        // running state, log2 units. The self key (first split only) seeds it.
+        const bool self_here = has_self && it.split == 0;
+        float m_used = -INFINITY, l = 0.f, s_self = 0.f;
+        if (self_here) {
+          s_self = row_valid ? row_dot<D>(args.q, args.k_self, q32, my_elem0) * args.scale_log2
+                             : 0.f;
+          m_used = s_self;
+          l = 1.f;
+        }
+
+        for (int j = 0; j < nt; ++j) {
+          mbar_wait(smem_u32(&ctrl->s_full[t]), sp_it & 1);
+          tc_fence_after();
+          uint32_t sr[128];
+          {
+            uint32_t(&a0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[0]);
+            uint32_t(&a1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[32]);
+            uint32_t(&a2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[64]);
+            uint32_t(&a3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[96]);
+            tmem_ld32(tm_s + 0, a0);
+            tmem_ld32(tm_s + 32, a1);
+            tmem_ld32(tm_s + 64, a2);
+            tmem_ld32(tm_s + 96, a3);
+          }
+          tmem_wait_ld_regs(sr);
+          const int keys_here = it.n_keys - j * kTileN;  // may exceed 128
+          if (keys_here < kTileN) {
+#pragma unroll
+            for (int c = 0; c < kTileN; ++c)
+              if (c >= keys_here) sr[c] = 0xff800000u;  // -inf
+          }
+          float mx = __uint_as_float(sr[0]);
+#pragma unroll
+          for (int c = 1; c < kTileN; ++c) mx = fmaxf(mx, __uint_as_float(sr[c]));
+          const float m_new = fmaxf(m_used, mx * c_log2);
+          const bool need = m_new > m_used + kRescaleTau;
+          if (j == 0) {
+            // nothing accumulated in O yet (first PV overwrites); only l may hold the self weight
+            if (need) {
+              l *= ex2_approx(m_used - m_new);
+              m_used = m_new;
+            }
+          } else if (__any_sync(0xffffffffu, need)) {
+            const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
+#pragma unroll
+            for (int c0 = 0; c0 < D; c0 += 32) {
+              uint32_t orr[32];
+              tmem_ld32(tm_o + c0, orr);
+              tmem_wait_ld_regs(orr);
+#pragma unroll
+              for (int c = 0; c < 32; ++c)
+                orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
+              tmem_st32(tm_o + c0, orr);
+            }
+            l *= alpha;
+            if (need) m_used = m_new;
+          }
+          // P = exp2(S*c - m), row sum, pack to bf16 pairs
+          float sum = 0.f;
+          uint32_t pr[64];
+#pragma unroll
+          for (int c = 0; c < kTileN; c += 2) {
+            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[c]), c_log2, -m_used));
+            const float p1 = ex2_approx(fmaf(__uint_as_float(sr[c + 1]), c_log2, -m_used));
+            sum += p0 + p1;
+            pr[c >> 1] = pack_bf16x2(p0, p1);
+          }
+          l += sum;
+          {
+            uint32_t(&b0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&pr[0]);
+            uint32_t(&b1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&pr[32]);
+            tmem_st32(tm_s + 0, b0);
+            tmem_st32(tm_s + 32, b1);
+          }
+          tmem_wait_st();
+          tc_fence_before();
+          mbar_arrive(smem_u32(&ctrl->p_full[t]));
+          ++sp_it;
+        }
+
+        // ------------------------------------------------------------ epilogue (a7 / a8)
+        if (nt > 0) {
+          mbar_wait(smem_u32(&ctrl->o_full[t]), o_it & 1);
+          ++o_it;
+          tc_fence_after();
+        }
+        const bool partial = args.num_splits > 1;
+        float w_self = 0.f;
+        if (self_here) w_self = ex2_approx(s_self - m_used);
+        const float inv = (!partial && l > 0.f) ? (1.0f / l) : (partial ? 1.0f : 0.f);
+        float* dst;
+        if (!partial) {
+          dst = args.out + my_elem0;
+        } else {
+          const size_t prow =
+              ((static_cast<size_t>(it.layer) * it.total_q + it.q_row0 + t * kTileM + tid128) *
+                   args.H + it.h) * args.num_splits + it.split;
+          dst = args.part_o + prow * D;
+          if (row_valid) {
+            args.part_ml[prow * 2 + 0] = m_used;
+            args.part_ml[prow * 2 + 1] = l;
+          }
+        }
+#pragma unroll
+        for (int c0 = 0; c0 < D; c0 += 32) {
+          uint32_t orr[32];
+          if (nt > 0) {
+            tmem_ld32(tm_o + c0, orr);
+            tmem_wait_ld_regs(orr);
+          } else {
+#pragma unroll
+            for (int c = 0; c < 32; ++c) orr[c] = 0u;
+          }
+          if (row_valid) {
+#pragma unroll
+            for (int c = 0; c < 32; c += 4) {
+              float4 o;
+              o.x = __uint_as_float(orr[c + 0]) * vs;
+              o.y = __uint_as_float(orr[c + 1]) * vs;
+              o.z = __uint_as_float(orr[c + 2]) * vs;
+              o.w = __uint_as_float(orr[c + 3]) * vs;
+              if (self_here) {
+                const size_t e = my_elem0 + c0 + c;
+                o.x = fmaf(w_self, load_elem_f(args.v_self, q32, e + 0), o.x);
+                o.y = fmaf(w_self, load_elem_f(args.v_self, q32, e + 1), o.y);
+                o.z = fmaf(w_self, load_elem_f(args.v_self, q32, e + 2), o.z);
+                o.w = fmaf(w_self, load_elem_f(args.v_self, q32, e + 3), o.w);
+              }
+              o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
+              *reinterpret_cast<float4*>(dst + c0 + c) = o;
+            }
+          }
+        }
+        tc_fence_before();
+      }
+      mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+    }
+  }
+
+  // ------------------------------------------------------------------ teardown
+  tc_fence_before();
+  __syncthreads();
+  if (warp == kMmaWarp) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base, kTmemCols);
+  }
+}
+
+}  // namespace upr

@@ -1,0 +1,76 @@
+"""Shared helpers for the GPU parity tests: build seeded inputs, run the CUDA path through the
+C-ABI binding, run the oracle on the SAME stored input values (never on CUDA outputs)."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+import oracle
+import upr_synth as S
+
+ORACLE_DT = {"f32": oracle.F32, "bf16": oracle.BF16, "fp8": oracle.FP8_E4M3}
+
+
+def bits(t: torch.Tensor) -> np.ndarray:
+    """bf16 tensor -> uint16 bit patterns on the host; fp32 tensor -> float32 array."""
+    t = t.detach().cpu().contiguous()
+    if t.dtype == torch.bfloat16:
+        return t.view(torch.int16).numpy().view(np.uint16)
+    return t.numpy()
+
+
+def to_f64(t: torch.Tensor) -> np.ndarray:
+    return t.detach().cpu().to(torch.float64).numpy()
+
+
+class Inputs:
+    def __init__(self, w: S.Workload, device, q_scale: float = 1.0):
+        self.w = w
+        self.device = device
+        self.q = S.gen_queries(w, "q", device, q_scale)
+        self.k_self = S.gen_queries(w, "k_self", device) if w.self_term else None
+        self.v_self = S.gen_queries(w, "v_self", device) if w.self_term else None
+        self.k_pool = S.gen_pool(w, "k_pool", device)
+        self.v_pool = S.gen_pool(w, "v_pool", device)
+        self.slot_ids_host = S.slot_ids(w)
+        self.slot_ids = torch.as_tensor(self.slot_ids_host, device=device)
+
+    def block_kv_f64(self, l: int, b: int, h: int):
+        """History K/V rows of one (layer, user, head) block, straight from the generated pool
+        (bf16 values widened exactly) -- for bf16/f32 caches this IS what the cache stores."""
+        Lb = int(self.w.seq_lens[b])
+        s = int(self.slot_ids_host[b])
+        return to_f64(self.k_pool[l, s, h, :Lb]), to_f64(self.v_pool[l, s, h, :Lb])
+
+    def block_q_f64(self, l: int, b: int, h: int):
+        co = self.w.cand_offsets
+        sl = slice(int(co[b]), int(co[b + 1]))
+        q = to_f64(self.q[l, sl, h])
+        if self.k_self is None:
+            return q, None, None
+        return q, to_f64(self.k_self[l, sl, h]), to_f64(self.v_self[l, sl, h])
+
+
+def oracle_block(inp: Inputs, l: int, b: int, h: int, sm_scale=None) -> np.ndarray:
+    K, V = inp.block_kv_f64(l, b, h)
+    q, ks, vs = inp.block_q_f64(l, b, h)
+    return oracle.attn_block(q, K, V, ks, vs, scale=sm_scale)
+
+
+def oracle_all(inp: Inputs, sm_scale=None) -> np.ndarray:
+    w = inp.w
+    out = np.zeros((w.n_layers, w.total_q, w.H, w.d))
+    co = w.cand_offsets
+    for l in range(w.n_layers):
+        for b in range(w.B):
+            if co[b + 1] == co[b]:
+                continue
+            for h in range(w.H):
+                out[l, co[b]:co[b + 1], h] = oracle_block(inp, l, b, h, sm_scale)
+    return out
+
+
+def error_stats(got: np.ndarray, want: np.ndarray):
+    diff = np.abs(got.astype(np.float64) - want)
+    rms = float(np.sqrt(np.mean(want ** 2))) or 1.0
+    return float(diff.max()) if diff.size else 0.0, float(np.sqrt(np.mean(diff ** 2)) / rms) if diff.size else 0.0

@@ -225,3 +225,13 @@ def gen_queries(w: Workload, tag: str = "q", device="cpu", scale: float = 1.0) -
 def gen_pool(w: Workload, tag: str, device="cpu") -> torch.Tensor:
     """The paper's KV pool [n_layers, S=B, H, n_max, d] in bf16."""
     return normal_bf16(w.seed, tag, (w.n_layers, w.B, w.H, w.n_max, w.d), device)
+
+
+def custom_workload(name: str, seed: int, seq_lens, cand_counts, H: int, d: int, n_layers: int = 1,
+                    kv_dtype: str = "bf16", q_dtype: str = "bf16", self_term: bool = False,
+                    n_max: Optional[int] = None) -> Workload:
+    """Arbitrary ragged shape for edge-case parity tests."""
+    L = np.asarray(seq_lens, dtype=np.int32)
+    n_max = n_max or max(1, int(L.max()) if L.size else 1)
+    return Workload(name, seed, int(L.shape[0]), H, d, n_layers, L, _offsets(cand_counts), kv_dtype, q_dtype,
+                    self_term, n_max)
