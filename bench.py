@@ -1,0 +1,347 @@
+#!/usr/bin/env python
+"""bench.py -- ranking cross-attention candidates/s on one node (driver contract).
+
+One "step" is one pass of the whole hot path over one batch of
+synthetic input: layout (host integers) -> pack the users' pool slots into the decode cache
+ -> cross-attention of every candidate over its user's cached history for all
+layers [-> split-K combine when the split policy engages].
+
+    python bench.py --gpus N --steps K --warmup W [--config 3] [--impl reference]
+
+N = 1: BASELINE.json config 3 (largest bf16 config, the one the 60%-of-roofline target names).
+N > 1 (torchrun): users are independent, so every rank runs its own batch of
+the same config with a rank-specific seed -- weak scaling, no data-path collective.
+Prints ONE JSON line on rank 0.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import upr_synth as S  # noqa: E402
+
+METRIC = "ranking cross-attn candidates/sec/GPU; TFLOP/s as fraction of roofline"
+
+
+# ----------------------------------------------------------------------------- helpers
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"hbm_gbs": p["hbm_gbs"], "bf16_tflops": p["bf16_tflops"],
+                "bf16_tflops_sustained": p.get("bf16_tflops_sustained", p["bf16_tflops"]), "source": "measured"}
+    # fallback stated in B200_PROFILING.md
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def aggregate_over_ranks(local_ms: float, local_units: int, dist=None):
+    """Whole-job numbers from per-rank ones: time = max over ranks, units = sum over ranks.
+    Works on any backend (nccl on GPU, gloo in the CPU test)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_ms, local_units
+    dev = "cuda" if dist.get_backend() == "nccl" else "cpu"
+    t = torch.tensor([local_ms], dtype=torch.float64, device=dev)
+    u = torch.tensor([local_units], dtype=torch.int64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), int(u.item())
+
+
+def rank_workload(cfg, rank: int) -> S.Workload:
+    """Rank r's batch: same config, rank-specific seed (users are independent units)."""
+    w = S.workload(cfg)
+    if rank:
+        w.seed = w.seed + 7919 * rank
+    return w
+
+
+# ----------------------------------------------------------------------------- oracle legs
+def oracle_step(w: S.Workload, users: int):
+    """One oracle pass (pack + attention, all layers/heads) over the first `users` users.
+    Returns (seconds, candidates processed)."""
+    import oracle
+    sub = S.workload(w.cfg, users=users)
+    dt = {"f32": oracle.F32, "bf16": oracle.BF16, "fp8": oracle.FP8_E4M3}[sub.kv_dtype]
+    qdt = oracle.F32 if sub.q_dtype == "f32" else oracle.BF16
+
+    def b(t):
+        t = t.contiguous()
+        return t.view(torch.int16).numpy().view(np.uint16) if t.dtype == torch.bfloat16 else t.numpy()
+    q = b(S.gen_queries(sub, "q"))
+    ks = b(S.gen_queries(sub, "k_self")) if sub.self_term else None
+    vs = b(S.gen_queries(sub, "v_self")) if sub.self_term else None
+    kp, vp = b(S.gen_pool(sub, "k_pool")), b(S.gen_pool(sub, "v_pool"))
+    slots = S.slot_ids(sub)
+    t0 = time.perf_counter()
+    kc, ksc = oracle.pack(kp, slots, sub.seq_lens, dt)
+    vc, vsc = oracle.pack(vp, slots, sub.seq_lens, dt)
+    oracle.cross_attn_packed(q, qdt, kc, vc, dt, sub.seq_lens, sub.cand_offsets, sub.H, sub.d, sub.n_layers,
+                             ksc, vsc, ks, vs)
+    return time.perf_counter() - t0, sub.total_q
+
+
+def oracle_sample_users(w: S.Workload, budget_s: float) -> int:
+    t1, _ = oracle_step(w, 1)
+    return int(max(1, min(w.B, budget_s / max(t1, 1e-3))))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    w = S.workload(args.config)
+    users = oracle_sample_users(w, 6.0)
+    for _ in range(args.warmup):
+        oracle_step(w, users)
+    ts, cands = [], 0
+    for _ in range(args.steps):
+        t, cands = oracle_step(w, users)
+        ts.append(t)
+    ms = 1e3 * float(np.mean(ts))
+    val = cands / (ms * 1e-3)
+    sample = f"first {users} of {w.B} users of {w.name}, all layers and heads, pack + attention"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "candidates/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": "candidates/s", "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": val, "unit": "candidates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------- CUDA arm
+def run_ours(args):
+    import paper_2606_00422_b200 as P
+    from paper_2606_00422_b200 import pipeline as pl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist_.init_process_group("nccl", device_id=dev)
+        dist = dist_
+
+    w = rank_workload(args.config, rank)
+    kv_id, q_id = pl.DTYPE_ID[w.kv_dtype], pl.DTYPE_ID[w.q_dtype]
+    # ---- device-resident inputs (the pool is GPU-resident by design)
+    q = S.gen_queries(w, "q", dev)
+    k_self = S.gen_queries(w, "k_self", dev) if w.self_term else None
+    v_self = S.gen_queries(w, "v_self", dev) if w.self_term else None
+    k_pool, v_pool = S.gen_pool(w, "k_pool", dev), S.gen_pool(w, "v_pool", dev)
+    slots = torch.as_tensor(S.slot_ids(w), device=dev)
+    cache = pl.alloc_cache(w.seq_lens, w.H, w.d, w.n_layers, kv_id, dev)
+    attn = pl.CrossAttention(cache, w.cand_offsets, q_id, num_splits=0)
+    stream = torch.cuda.current_stream()
+
+    launches = [0]
+
+    def step(q_dev):
+        # a0: layout is integer-only host work, redone every step like a new batch would
+        P.upr_kv_cache_layout(w.seq_lens, w.H, w.d, w.n_layers, kv_id)
+        pl.pack_cache(cache, k_pool, v_pool, slots, stream)           # a1
+        launches[0] += P.upr_last_launch_count()
+        out = attn(q_dev, k_self, v_self, stream=stream)              # a2-a8
+        launches[0] += P.upr_last_launch_count()
+        return out
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step(q)
+    barrier()
+
+    # ---- device-resident timed region: K steps, per-kernel events inside
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+    e_start, e_end = ev(), ev()
+    marks = [(ev(), ev(), ev()) for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches[0] = 0
+    barrier()
+    e_start.record(stream)
+    for i in range(args.steps):
+        a, b, c = marks[i]
+        a.record(stream)
+        P.upr_kv_cache_layout(w.seq_lens, w.H, w.d, w.n_layers, kv_id)
+        pl.pack_cache(cache, k_pool, v_pool, slots, stream)
+        launches[0] += P.upr_last_launch_count()
+        b.record(stream)
+        attn(q, k_self, v_self, stream=stream)
+        launches[0] += P.upr_last_launch_count()
+        c.record(stream)
+    e_end.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = e_start.elapsed_time(e_end)
+    pack_ms = float(np.mean([a.elapsed_time(b) for a, b, c in marks]))
+    attn_ms = float(np.mean([b.elapsed_time(c) for a, b, c in marks]))
+    gpu_launches = launches[0]
+    ms_step, units = aggregate_over_ranks(total_ms / args.steps, w.total_q, dist)
+    value = units / (ms_step * 1e-3)
+
+    # ---- end-to-end through the public API with HOST buffers (q in, out back), every step
+    q_host = q.cpu().pin_memory()
+    out_host = torch.empty(attn.out.shape, dtype=torch.float32).pin_memory()
+    sl_host = torch.as_tensor(w.seq_lens).pin_memory()
+    co_host = torch.as_tensor(w.cand_offsets).pin_memory()
+    q_dev2 = torch.empty_like(q)
+    e2e_steps = max(1, min(args.steps, 5))
+
+    def e2e_step():
+        q_dev2.copy_(q_host, non_blocking=True)
+        cache.seq_lens.copy_(sl_host, non_blocking=True)
+        attn.cand_offsets.copy_(co_host, non_blocking=True)
+        out = step(q_dev2)
+        out_host.copy_(out, non_blocking=True)
+    e2e_step()
+    barrier()
+    e0, e1 = ev(), ev()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        e2e_step()
+    e1.record(stream)
+    barrier()
+    e2e_ms, _ = aggregate_over_ranks(e0.elapsed_time(e1) / e2e_steps, w.total_q, dist)
+    h2d = q_host.numel() * q_host.element_size() + sl_host.numel() * 4 + co_host.numel() * 4
+    d2h = out_host.numel() * 4
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (attention): a dense contraction -> tensor peak
+    peaks = measured_peaks()
+    flops = w.flops
+    tflops = flops / (attn_ms * 1e-3) / 1e12
+    t_flop = flops / (peaks["bf16_tflops"] * 1e12)
+    t_mem = w.kv_bytes / (peaks["hbm_gbs"] * 1e9)
+    roof_ms = 1e3 * max(t_flop, t_mem)
+    roofline = {"bound": "tensor" if t_flop >= t_mem else "hbm", "kernel": "upr_attn_fwd_kernel",
+                "achieved": tflops, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                "frac": tflops / peaks["bf16_tflops"], "traffic": None,
+                "peak_source": peaks["source"] + " (burst cuBLAS bf16)",
+                "frac_of_sustained": tflops / peaks["bf16_tflops_sustained"],
+                "kernel_ms": attn_ms, "roofline_ms": roof_ms, "frac_of_roofline_time": roof_ms / attn_ms,
+                "flops_per_launch": flops, "kv_bytes_per_launch": w.kv_bytes,
+                "kv_gbs": w.kv_bytes / (attn_ms * 1e-3) / 1e9}
+    pack_bytes = 2 * w.kv_bytes  # read pool rows + write cache rows (bf16)
+    extra = {"pack_ms": pack_ms, "attn_ms": attn_ms, "pack_gbs": pack_bytes / (pack_ms * 1e-3) / 1e9,
+             "attn_candidates_per_s": w.total_q / (attn_ms * 1e-3), "splits": attn.splits}
+
+    # ---- CPU baseline: the oracle as it stands, bounded sample, host cores of this box
+    import oracle
+    users = oracle_sample_users(w, 15.0)
+    t_cpu, cands = oracle_step(w, users)
+    sample = f"first {users} of {w.B} users of {w.name}, all layers and heads, pack + attention, {t_cpu:.1f} s"
+    cpu_baseline = {"value": cands / t_cpu, "unit": "candidates/s", "cores": oracle.num_threads(), "kind": "oracle",
+                    "sample": sample}
+
+    line = {"metric": METRIC, "value": value, "unit": "candidates/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16" if w.kv_dtype != "f32" else "f32", "data": "synthetic",
+            "config": {"workload": w.name, "B": w.B, "H": w.H, "d": w.d, "layers": w.n_layers,
+                       "total_candidates": w.total_q, "sum_history": int(w.seq_lens.sum()),
+                       "kv_dtype": w.kv_dtype, "self_term": w.self_term,
+                       "step": "layout + pack(pool->cache) + cross-attention, all layers",
+                       "l2": "inputs larger than L2 (K/V %.1f GB per step)" % (w.kv_bytes / 1e9),
+                       "parallelism": "users sharded by rank, no collective" if world > 1 else "single GPU"},
+            "clocks": clocks, "gpu_launches": gpu_launches,
+            "e2e": {"value": units / (e2e_ms * 1e-3), "unit": "candidates/s", "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms, "steps": e2e_steps},
+            "roofline": roofline, "cpu_baseline": cpu_baseline, "detail": extra}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="3")
+    args = ap.parse_args()
+    args.config = int(args.config) if args.config.isdigit() else args.config
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

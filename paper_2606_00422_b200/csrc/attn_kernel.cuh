@@ -546,16 +546,20 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             if (need) m_used = m_new;
           }
           // P = exp2(S*c - m), row sum, pack to bf16 pairs
-          float sum = 0.f;
+          // l accumulates the bf16-ROUNDED weights, i.e. exactly what the PV MMA multiplies,
+          // so that out = sum(p~ v) / sum(p~) stays a convex combination of V rows.
+          float sum0 = 0.f, sum1 = 0.f;
           uint32_t pr[64];
 #pragma unroll
           for (int c = 0; c < kTileN; c += 2) {
             const float p0 = ex2_approx(fmaf(__uint_as_float(sr[c]), c_log2, -m_used));
             const float p1 = ex2_approx(fmaf(__uint_as_float(sr[c + 1]), c_log2, -m_used));
-            sum += p0 + p1;
-            pr[c >> 1] = pack_bf16x2(p0, p1);
+            const uint32_t w = pack_bf16x2(p0, p1);
+            pr[c >> 1] = w;
+            sum0 += __uint_as_float(w << 16);
+            sum1 += __uint_as_float(w & 0xffff0000u);
           }
-          l += sum;
+          l += sum0 + sum1;
           {
             uint32_t(&b0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&pr[0]);
             uint32_t(&b1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&pr[32]);

@@ -8,7 +8,7 @@ import torch
 
 import oracle
 import upr_synth as S
-from tests.harness import Inputs, bits, error_stats, oracle_all, oracle_block
+from harness import Inputs, bits, error_stats, oracle_all, oracle_block
 
 pytestmark = pytest.mark.gpu
 
@@ -42,6 +42,7 @@ def check(got, want, tol=TOL_BF16, strict=TOL_STRICT):
     assert mx <= tol, f"max-abs {mx} > {tol}"
     assert mx <= strict, f"max-abs {mx} > strict {strict}"
     assert rel <= TOL_RMS, f"relative RMS {rel}"
+    print(f"max-abs {mx:.2e} rel-rms {rel:.2e}")
     return mx, rel
 
 
@@ -118,10 +119,10 @@ def test_peaked_queries_and_custom_scale(P):
     inp = Inputs(w, "cuda", q_scale=8.0)
     got, _, _ = run_cuda(P, inp)
     mx, rel = error_stats(got, oracle_all(inp))
-    assert mx <= TOL_BF16 and rel <= 2e-2
+    assert mx <= 2e-2 and rel <= 1e-2, (mx, rel)  # outputs are O(1): bf16 P rounding (2^-9) x |v| <= 4.3
     got2, _, _ = run_cuda(P, inp, sm_scale=0.05)
     mx2, _ = error_stats(got2, oracle_all(inp, sm_scale=0.05))
-    assert mx2 <= TOL_BF16
+    assert mx2 <= TOL_BF16, mx2
 
 
 def test_basic_entry_point_and_candidate_permutation(P):

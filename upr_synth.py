@@ -139,6 +139,7 @@ class Workload:
     q_dtype: str               # "f32" | "bf16"
     self_term: bool
     n_max: int                 # pool slot length (paper's n in [L,S,H,n,D])
+    cfg: object = None         # BASELINE.json config id this workload was built from
 
     @property
     def total_q(self) -> int:
@@ -176,6 +177,12 @@ def _offsets(counts) -> np.ndarray:
 def workload(cfg: int | str, users: Optional[int] = None) -> Workload:
     """The five BASELINE.json configs (1..5) and the supplementary low-C shape "S1".
     ``users`` overrides B (same per-user distributions) for reduced-size parity cases."""
+    w = _workload(cfg, users)
+    w.cfg = cfg
+    return w
+
+
+def _workload(cfg, users):
     if cfg == 1:
         B = users or 1
         return Workload("cfg1_fp32_toy", 1001, B, 4, 64, 1, np.full(B, 256, np.int32), _offsets([16] * B),
