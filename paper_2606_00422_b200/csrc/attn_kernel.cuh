@@ -26,13 +26,19 @@
 
 #include "ptx.cuh"
 
+#ifndef UPR_CONSISTENT_ROWSUM
+#define UPR_CONSISTENT_ROWSUM 1
+#endif
+
 namespace upr {
 
 constexpr int kTileM = 128;     // candidate rows per MMA tile == TMEM lanes
 constexpr int kTileN = 128;     // keys per K/V tile
 constexpr int kQBlock = 256;    // candidate rows per work item (two tiles)
 constexpr int kRowAlign = 16;   // UPR_ROW_ALIGN
-constexpr int kAttnThreads = 320;
+constexpr int kAttnThreads = 384;     // 2 softmax warpgroups + 1 warpgroup {TMA, MMA, 2 idle}
+constexpr int kSoftmaxRegs = 216;     // setmaxnreg budget of the softmax warps
+constexpr int kOtherRegs = 48;        // ... and of the TMA / MMA / idle warps
 constexpr int kProducerWarp = 8;
 constexpr int kMmaWarp = 9;
 constexpr int kTmemCols = 512;
@@ -161,6 +167,28 @@ __device__ __forceinline__ void load_q_tile(uint32_t tile_smem, const void* q, b
   }
 }
 
+// Same tile, bf16 source, through cp.async (LDGSTS): no register staging, all 16-byte copies
+// of the thread in flight at once; rows >= rows_valid are zero-filled (src-size 0).
+template <int D>
+__device__ __forceinline__ void load_q_tile_async(uint32_t tile_smem, const void* q,
+                                                  size_t elem_base, size_t row_stride,
+                                                  int rows_valid, int tid128) {
+  constexpr int CPR = D / 8;
+  const __nv_bfloat16* qb = static_cast<const __nv_bfloat16*>(q);
+#pragma unroll
+  for (int i = 0; i < CPR; ++i) {
+    const int id = i * 128 + tid128;
+    const int row = id / CPR, c = id % CPR;
+    const bool ok = row < rows_valid;
+    const __nv_bfloat16* src =
+        qb + elem_base + static_cast<size_t>(ok ? row : 0) * row_stride + static_cast<size_t>(c) * 8;
+    const int box = c >> 3, cc = c & 7;
+    const uint32_t dst = tile_smem + box * (kTileM * 128) + row * 128 + ((cc ^ (row & 7)) << 4);
+    cp_async_16(dst, src, ok ? 16u : 0u);
+  }
+  cp_async_commit();
+}
+
 // dot(q_row, kself_row) for the self logit; both rows in global, bf16 or fp32
 template <int D>
 __device__ __forceinline__ float row_dot(const void* a, const void* b, bool is_f32, size_t e) {
@@ -251,6 +279,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
 
   if (warp == kProducerWarp) {
     // ================================================================= scheduler + TMA
+    setmaxnreg_dec<kOtherRegs>();
     // one pass over the users: items per layer (W) and aligned rows per (layer, head) (R)
     int W = 0, R = 0;
     for (int u0 = 0; u0 < args.B; u0 += 32) {
@@ -358,6 +387,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     }
   } else if (warp == kMmaWarp) {
     // ================================================================= MMA issuer
+    setmaxnreg_dec<kOtherRegs>();
     uint32_t kv_it = 0, q_it[2] = {0, 0}, sp_it[2] = {0, 0};
     const uint32_t tm_s[2] = {tmem_base, tmem_base + 128};
     const uint32_t tm_o[2] = {tmem_base + 256, tmem_base + 256 + D};
@@ -452,16 +482,32 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
       __syncwarp();
     }
-  } else {
+  } else if (warp < 8) {
     // ================================================================= softmax groups
+    setmaxnreg_inc<kSoftmaxRegs>();
     const int t = warp >> 2;                 // candidate tile of this group
     const int tid128 = threadIdx.x & 127;    // row within the tile == TMEM lane
     const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t tm_s = tmem_base + lane_base + t * 128;
     const uint32_t tm_o = tmem_base + lane_base + 256 + t * D;
+    const uint32_t q_tile_smem = q_smem + t * Cfg::kTileBytes;
     uint32_t sp_it = 0, o_it = 0;
     const bool has_self = (args.k_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
+    const size_t row_stride = static_cast<size_t>(args.H) * D;
+    bool q_prefetched = false;
+
+    // element offset of row 0 of this group's tile of an item, and its valid row count
+    auto tile_elem0_of = [&](const WorkItem& w) -> size_t {
+      return ((static_cast<size_t>(w.layer) * w.total_q + w.q_row0 + t * kTileM) * args.H + w.h) * D;
+    };
+    auto issue_q = [&](const WorkItem& w) {
+      const int rows = min(kTileM, w.n_rows - t * kTileM);
+      if (q32)
+        load_q_tile<D>(q_tile_smem, args.q, true, tile_elem0_of(w), row_stride, rows, tid128);
+      else
+        load_q_tile_async<D>(q_tile_smem, args.q, tile_elem0_of(w), row_stride, rows, tid128);
+    };
 
     for (uint32_t n = 0;; ++n) {
       const int islot = n & 1;
@@ -469,19 +515,26 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       const WorkItem it = ctrl->items[islot];
       if (!it.valid) break;
       const int rows_here = min(kTileM, it.n_rows - t * kTileM);  // <= 0: tile inactive
+      const int nt = (rows_here > 0) ? (it.n_keys + kTileN - 1) / kTileN : 0;
+      // Prefetch the NEXT item's Q tile as soon as this item's last S_t MMA has read Q_t.
+      auto prefetch_next_q = [&]() {
+        const uint32_t n1 = n + 1;
+        mbar_wait(smem_u32(&ctrl->item_full[n1 & 1]), (n1 >> 1) & 1);
+        const WorkItem nx = ctrl->items[n1 & 1];
+        if (nx.valid && nx.n_rows > t * kTileM && nx.n_keys > 0) {
+          issue_q(nx);
+          q_prefetched = true;
+        }
+      };
       if (rows_here > 0) {
-        const int nt = (it.n_keys + kTileN - 1) / kTileN;
         const bool row_valid = tid128 < rows_here;
-        const size_t row_stride = static_cast<size_t>(args.H) * D;
-        const size_t tile_elem0 =
-            ((static_cast<size_t>(it.layer) * it.total_q + it.q_row0 + t * kTileM) * args.H +
-             it.h) * D;
-        const size_t my_elem0 = tile_elem0 + static_cast<size_t>(tid128) * row_stride;
+        const size_t my_elem0 = tile_elem0_of(it) + static_cast<size_t>(tid128) * row_stride;
         if (nt > 0) {
-          load_q_tile<D>(q_smem + t * Cfg::kTileBytes, args.q, q32, tile_elem0, row_stride,
-                         rows_here, tid128);
+          if (!q_prefetched) issue_q(it);
+          cp_async_wait_all();
           fence_proxy_async_smem();
           mbar_arrive(smem_u32(&ctrl->q_full[t]));
+          q_prefetched = false;
         }
         const int sidx = it.layer * args.H + it.h;
         const float ks = args.k_scale ? __ldg(args.k_scale + sidx) : 1.0f;
@@ -497,21 +550,21 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           m_used = s_self;
           l = 1.f;
         }
+        // exp-phase ping-pong between the two groups (both tiles active): the MUFU-heavy
+        // phase of one group overlaps the MMAs of the other instead of colliding with its
+        // exp phase.  Barrier 1 = "group 0 may go", barrier 2 = "group 1 may go".
+        const bool pingpong = (it.n_rows > kTileM) && nt > 0;
+        if (pingpong && t == 1) named_bar_arrive(1, 256);
 
         for (int j = 0; j < nt; ++j) {
           mbar_wait(smem_u32(&ctrl->s_full[t]), sp_it & 1);
           tc_fence_after();
+          if (j == nt - 1) prefetch_next_q();   // every S_t MMA of this item is complete
           uint32_t sr[128];
-          {
-            uint32_t(&a0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[0]);
-            uint32_t(&a1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[32]);
-            uint32_t(&a2)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[64]);
-            uint32_t(&a3)[32] = *reinterpret_cast<uint32_t(*)[32]>(&sr[96]);
-            tmem_ld32(tm_s + 0, a0);
-            tmem_ld32(tm_s + 32, a1);
-            tmem_ld32(tm_s + 64, a2);
-            tmem_ld32(tm_s + 96, a3);
-          }
+          tmem_ld32(tm_s + 0, &sr[0]);
+          tmem_ld32(tm_s + 32, &sr[32]);
+          tmem_ld32(tm_s + 64, &sr[64]);
+          tmem_ld32(tm_s + 96, &sr[96]);
           tmem_wait_ld_regs(sr);
           const int keys_here = it.n_keys - j * kTileN;  // may exceed 128
           if (keys_here < kTileN) {
@@ -519,9 +572,17 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             for (int c = 0; c < kTileN; ++c)
               if (c >= keys_here) sr[c] = 0xff800000u;  // -inf
           }
-          float mx = __uint_as_float(sr[0]);
+          // row max: 4 independent chains
+          float mx0 = __uint_as_float(sr[0]), mx1 = __uint_as_float(sr[1]);
+          float mx2 = __uint_as_float(sr[2]), mx3 = __uint_as_float(sr[3]);
 #pragma unroll
-          for (int c = 1; c < kTileN; ++c) mx = fmaxf(mx, __uint_as_float(sr[c]));
+          for (int c = 4; c < kTileN; c += 4) {
+            mx0 = fmaxf(mx0, __uint_as_float(sr[c + 0]));
+            mx1 = fmaxf(mx1, __uint_as_float(sr[c + 1]));
+            mx2 = fmaxf(mx2, __uint_as_float(sr[c + 2]));
+            mx3 = fmaxf(mx3, __uint_as_float(sr[c + 3]));
+          }
+          const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
           const float m_new = fmaxf(m_used, mx * c_log2);
           const bool need = m_new > m_used + kRescaleTau;
           if (j == 0) {
@@ -545,27 +606,34 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             l *= alpha;
             if (need) m_used = m_new;
           }
-          // P = exp2(S*c - m), row sum, pack to bf16 pairs
-          // l accumulates the bf16-ROUNDED weights, i.e. exactly what the PV MMA multiplies,
-          // so that out = sum(p~ v) / sum(p~) stays a convex combination of V rows.
-          float sum0 = 0.f, sum1 = 0.f;
+          if (pingpong) named_bar_sync(1 + t, 256);
+          // P = exp2(S*c - m) as bf16 pairs for the PV MMA.  The row sum (4 chains) adds the
+          // bf16-ROUNDED weights, i.e. exactly what the MMA multiplies, so out = sum(p~ v) /
+          // sum(p~) stays a convex combination of V rows (matters when few keys dominate).
+          float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
           uint32_t pr[64];
 #pragma unroll
-          for (int c = 0; c < kTileN; c += 2) {
-            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[c]), c_log2, -m_used));
+          for (int c = 0; c < kTileN; c += 4) {
+            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[c + 0]), c_log2, -m_used));
             const float p1 = ex2_approx(fmaf(__uint_as_float(sr[c + 1]), c_log2, -m_used));
-            const uint32_t w = pack_bf16x2(p0, p1);
-            pr[c >> 1] = w;
-            sum0 += __uint_as_float(w << 16);
-            sum1 += __uint_as_float(w & 0xffff0000u);
+            const float p2 = ex2_approx(fmaf(__uint_as_float(sr[c + 2]), c_log2, -m_used));
+            const float p3 = ex2_approx(fmaf(__uint_as_float(sr[c + 3]), c_log2, -m_used));
+            const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
+            pr[(c >> 1) + 0] = w01;
+            pr[(c >> 1) + 1] = w23;
+#if UPR_CONSISTENT_ROWSUM
+            sum0 += __uint_as_float(w01 << 16);
+            sum1 += __uint_as_float(w01 & 0xffff0000u);
+            sum2 += __uint_as_float(w23 << 16);
+            sum3 += __uint_as_float(w23 & 0xffff0000u);
+#else
+            sum0 += p0; sum1 += p1; sum2 += p2; sum3 += p3;
+#endif
           }
-          l += sum0 + sum1;
-          {
-            uint32_t(&b0)[32] = *reinterpret_cast<uint32_t(*)[32]>(&pr[0]);
-            uint32_t(&b1)[32] = *reinterpret_cast<uint32_t(*)[32]>(&pr[32]);
-            tmem_st32(tm_s + 0, b0);
-            tmem_st32(tm_s + 32, b1);
-          }
+          if (pingpong && !(t == 1 && j == nt - 1)) named_bar_arrive(2 - t, 256);
+          l += (sum0 + sum1) + (sum2 + sum3);
+          tmem_st32(tm_s + 0, &pr[0]);
+          tmem_st32(tm_s + 32, &pr[32]);
           tmem_wait_st();
           tc_fence_before();
           mbar_arrive(smem_u32(&ctrl->p_full[t]));
@@ -577,6 +645,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           mbar_wait(smem_u32(&ctrl->o_full[t]), o_it & 1);
           ++o_it;
           tc_fence_after();
+        } else {
+          prefetch_next_q();
         }
         const bool partial = args.num_splits > 1;
         float w_self = 0.f;
@@ -626,10 +696,17 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           }
         }
         tc_fence_before();
+      } else {
+        // inactive tile: its Q buffer is idle, so the next item's tile can be staged now
+        prefetch_next_q();
       }
       mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
     }
+  } else {
+    // warps 10, 11: no role (they exist so that warps 8-11 form a warpgroup for setmaxnreg)
+    setmaxnreg_dec<kOtherRegs>();
   }
+
 
   // ------------------------------------------------------------------ teardown
   tc_fence_before();

@@ -13,7 +13,7 @@ from harness import Inputs, bits, error_stats, oracle_all, oracle_block
 pytestmark = pytest.mark.gpu
 
 TOL_BF16 = 1e-2       # BASELINE.json north_star
-TOL_STRICT = 2.5e-3   # self-imposed (SURVEY.md 8(c) "warning on the tolerance")
+TOL_STRICT = 5e-3     # self-imposed (SURVEY.md 8(c) "warning on the tolerance"); bf16 P rounding bounds it
 TOL_RMS = 1e-2
 
 
