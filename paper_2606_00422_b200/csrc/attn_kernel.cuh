@@ -5,13 +5,20 @@
 // 198); optionally each candidate also sees its own key/value (identity block of the
 // M-FALCON mask).  out = softmax(scale * q K^T) V, fp32.
 //
-// Persistent, warp-specialised CTA (one per SM), work item = (layer, user, head, history
-// split, block of <= 256 candidates):
-//   warps 0-3 : softmax group for candidate tile 0 (rows   0..127), one thread per row
-//   warps 4-7 : softmax group for candidate tile 1 (rows 128..255)
-//   warp  8   : scheduler + TMA producer (decodes work items from the device offset tables,
-//               streams the user's K/V tiles HBM -> swizzled smem ring, once per item)
-//   warp  9   : tcgen05.mma issuer: S_t = Q_t K^T (SS), O_t += P_t V (A = P from TMEM)
+// Persistent, warp-specialised CTA (one per SM, 512 threads), work item = (layer, user, head,
+// history split, block of <= 256 candidates):
+//   warps 0-3   : softmax group for candidate tile 0 (rows   0..127), one thread per row
+//   warps 4-7   : softmax group for candidate tile 1 (rows 128..255)
+//   warp  8     : scheduler + producer (decodes work items from the device offset tables and
+//                 streams the user's K/V tiles HBM -> smem, once per item: TMA tensor boxes
+//                 for a bf16 cache, contiguous bulk copies of raw rows for fp8 / fp32 caches)
+//   warp  9     : tcgen05.mma issuer: S_t = Q_t K^T (SS), O_t += P_t V (A = P from TMEM)
+//   warps 10-11 : converters (fp8 / fp32 caches only): raw rows -> bf16 swizzled MMA tiles,
+//                 "dequantised in registers"; the scales fold into the softmax scale (K) and
+//                 the epilogue (V), so the conversion is a pure, exact type change for E4M3
+//   warps 12-15 : epilogue group: drains O_t from TMEM, scales by 1/l, transposes 32x32
+//                 blocks through padded shared memory and writes full 128-byte lines, while
+//                 the softmax and MMA warps are already on the next item
 // TMEM (512 cols): S0 [0,128) S1 [128,256) O0 [256,256+D) O1 [256+D,256+2D); P_t (bf16)
 // overwrites the first 64 columns of S_t once S_t has been read into registers.
 // Online softmax in fp32 with lazy rescaling of O (only when the running max grows by more
@@ -36,13 +43,20 @@ constexpr int kTileM = 128;     // candidate rows per MMA tile == TMEM lanes
 constexpr int kTileN = 128;     // keys per K/V tile
 constexpr int kQBlock = 256;    // candidate rows per work item (two tiles)
 constexpr int kRowAlign = 16;   // UPR_ROW_ALIGN
-constexpr int kAttnThreads = 384;     // 2 softmax warpgroups + 1 warpgroup {TMA, MMA, 2 idle}
-constexpr int kSoftmaxRegs = 216;     // setmaxnreg budget of the softmax warps
-constexpr int kOtherRegs = 48;        // ... and of the TMA / MMA / idle warps
+constexpr int kAttnThreads = 512;     // 2 softmax warpgroups + {TMA, MMA, 2 converters} + epilogue
+constexpr int kSoftmaxRegs = 200;     // setmaxnreg budgets (sum over 512 threads <= 64 K registers)
+constexpr int kOtherRegs = 48;        //   producer / MMA / converter warpgroup
+constexpr int kEpilogueRegs = 64;     //   epilogue warpgroup
 constexpr int kProducerWarp = 8;
 constexpr int kMmaWarp = 9;
+constexpr int kConvWarp0 = 10;        // warps 10, 11
+constexpr int kConvThreads = 64;
+constexpr int kEpiWarp0 = 12;         // warps 12..15
 constexpr int kTmemCols = 512;
 constexpr float kRescaleTau = 8.0f;  // lazy-rescale threshold, log2 units
+constexpr int kEpiRowBytes = 144;     // 32 floats + 16 B pad: conflict-free 16-byte accesses
+
+enum : int { KV_BF16 = 0, KV_FP8 = 1, KV_F32 = 2 };
 
 struct AttnArgs {
   const void* q;
@@ -53,6 +67,8 @@ struct AttnArgs {
   const int32_t* cand_offsets;
   const float* k_scale;
   const float* v_scale;
+  const uint8_t* k_raw;   // fp8 / fp32 caches: base of the packed cache (bulk-copied raw rows)
+  const uint8_t* v_raw;
   float* part_o;          // split-K partial O~  [n_layers][total_q][H][ns][D]
   float* part_ml;         // split-K partial (m, l) [n_layers][total_q][H][ns][2]
   unsigned int* counter;  // dynamic work counter (zeroed before launch) or nullptr = static
@@ -72,33 +88,51 @@ struct WorkItem {
   int total_q;   // cand_offsets[B]
 };
 
-template <int D>
+template <int D, int KV>
 struct AttnCfg {
-  static constexpr int kBoxBytes = kTileN * 128;            // one [128 rows x 64 bf16] TMA box
+  static constexpr int kBoxBytes = kTileN * 128;            // one [128 rows x 64 bf16] box
   static constexpr int kBoxes = D / 64;                     // boxes per tile
-  static constexpr int kTileBytes = kBoxBytes * kBoxes;     // Q tile, K tile or V tile
-  static constexpr int kStages = (D == 128) ? 5 : 8;        // K/V ring slots
+  static constexpr int kTileBytes = kBoxBytes * kBoxes;     // Q tile, K tile or V tile (bf16)
+  static constexpr int kStages =                            // K/V ring slots (bf16 tiles)
+      (KV == KV_BF16) ? ((D == 128) ? 4 : 8) : ((D == 128) ? 3 : 6);
+  // raw ring (fp8 / fp32 caches): one slot = kRawRows contiguous cache rows
+  static constexpr int kElemBytes = (KV == KV_FP8) ? 1 : (KV == KV_F32) ? 4 : 2;
+  static constexpr int kRawRows = (KV == KV_F32) ? 32 : 128;
+  static constexpr int kRawSlotBytes = kRawRows * D * kElemBytes;   // 16 KB (D=128) / 8 KB
+  static constexpr int kRawStages = (KV == KV_BF16) ? 0 : ((D == 128) ? 2 : 4);
+  static constexpr int kRawPerTile = kTileN / kRawRows;
   static constexpr int kSmemQ = 2 * kTileBytes;
   static constexpr int kSmemKV = kStages * kTileBytes;
-  static constexpr int kSmemCtrl = 1024;
-  static constexpr int kSmemTotal = kSmemQ + kSmemKV + kSmemCtrl + 1024;  // + alignment slack
+  static constexpr int kSmemRaw = kRawStages * kRawSlotBytes;
+  static constexpr int kSmemEpi = 4 * 32 * kEpiRowBytes;    // one 32 x 32 fp32 block per warp
+  static constexpr int kSmemCtrl = 6144;
+  static constexpr int kSmemTotal =
+      kSmemQ + kSmemKV + kSmemRaw + kSmemEpi + kSmemCtrl + 1024;  // + alignment slack
   static constexpr uint32_t kIdescQK = make_idesc_bf16(kTileM, kTileN, 0, 0);
   static constexpr uint32_t kIdescPV = make_idesc_bf16(kTileM, D, 0, 1);
+  static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
 };
 
-struct __align__(8) AttnCtrl {
+struct __align__(16) AttnCtrl {
   uint64_t kv_full[8];
   uint64_t kv_empty[8];
+  uint64_t raw_full[4];
+  uint64_t raw_empty[4];
   uint64_t q_full[2];
   uint64_t s_full[2];
   uint64_t p_full[2];
   uint64_t o_full[2];
+  uint64_t o_empty[2];
+  uint64_t l_ready[2];
   uint64_t item_full[2];
   uint64_t item_empty[2];
   WorkItem items[2];
   uint32_t tmem_base;
+  uint32_t pad_[3];
+  float epi_inv[2][2][kTileM];    // [item slot][tile][row]: 1/l (or 1 for split-K partials)
+  float epi_wself[2][2][kTileM];  // weight of the candidate's own value row
 };
-static_assert(sizeof(AttnCtrl) <= 1024, "control block too large");
+static_assert(sizeof(AttnCtrl) <= 6144, "control block too large");
 
 // ---------------------------------------------------------------------------------------
 // Scheduler state: a forward-only cursor over users, 32 at a time (one per lane).
@@ -223,46 +257,72 @@ __device__ __forceinline__ float row_dot(const void* a, const void* b, bool is_f
   return acc;
 }
 
-__device__ __forceinline__ float load_elem_f(const void* p, bool is_f32, size_t e) {
-  return is_f32 ? __ldg(static_cast<const float*>(p) + e)
-                : __bfloat162float(static_cast<const __nv_bfloat16*>(p)[e]);
+// Four E4M3 bytes -> two bf16x2 words, exactly.  The 7 magnitude bits are placed so that the
+// E4M3 exponent sits in the low bits of the bf16 exponent field (value scaled by 2^-120,
+// E4M3 subnormals become bf16 subnormals of the same mantissa), then a packed bf16 multiply
+// by 2^120 restores the value; every E4M3 value is representable in bf16, so the product is
+// exact.  (S.1111.111, E4M3's NaN, decodes to +-480: caches must hold finite codes, as
+// upr_kv_pack's satfinite conversion guarantees.)
+__device__ __forceinline__ void e4m3x4_to_bf16x4(uint32_t w, uint32_t& lo, uint32_t& hi) {
+  const __nv_bfloat162 k = __halves2bfloat162(__ushort_as_bfloat16(0x7B80), __ushort_as_bfloat16(0x7B80));
+  uint32_t a = __byte_perm(w, 0u, 0x1404);  // halves: b0 << 8, b1 << 8
+  uint32_t b = __byte_perm(w, 0u, 0x3424);  //         b2 << 8, b3 << 8
+  a = (a & 0x80008000u) | ((a >> 4) & 0x07f007f0u);
+  b = (b & 0x80008000u) | ((b >> 4) & 0x07f007f0u);
+  __nv_bfloat162 ra = __hmul2(*reinterpret_cast<__nv_bfloat162*>(&a), k);
+  __nv_bfloat162 rb = __hmul2(*reinterpret_cast<__nv_bfloat162*>(&b), k);
+  lo = *reinterpret_cast<uint32_t*>(&ra);
+  hi = *reinterpret_cast<uint32_t*>(&rb);
 }
 
 // ---------------------------------------------------------------------------------------
 // The kernel
 // ---------------------------------------------------------------------------------------
-template <int D>
+template <int D, int KV>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v, const AttnArgs args) {
-  using Cfg = AttnCfg<D>;
+  using Cfg = AttnCfg<D, KV>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem_aligned = smem_raw + (smem_base - smem_u32(smem_raw));
   const uint32_t q_smem = smem_base;
-  const uint32_t kv_smem = smem_base + Cfg::kSmemQ;
-  AttnCtrl* ctrl = reinterpret_cast<AttnCtrl*>(smem_aligned + Cfg::kSmemQ + Cfg::kSmemKV);
+  const uint32_t kv_smem = q_smem + Cfg::kSmemQ;
+  const uint32_t raw_smem = kv_smem + Cfg::kSmemKV;
+  const uint32_t epi_smem = raw_smem + Cfg::kSmemRaw;
+  AttnCtrl* ctrl = reinterpret_cast<AttnCtrl*>(smem_aligned + Cfg::kSmemQ + Cfg::kSmemKV +
+                                               Cfg::kSmemRaw + Cfg::kSmemEpi);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
+  constexpr bool kConvert = (KV != KV_BF16);
+  // arrivals that release an item slot: 256 softmax threads, MMA lane 0, one lane of each
+  // epilogue warp, one lane of each converter warp
+  constexpr uint32_t kItemReaders = 256 + 1 + 4 + (kConvert ? 2 : 0);
 
   // ------------------------------------------------------------------ one-time setup
   if (threadIdx.x == 0) {
     for (int i = 0; i < Cfg::kStages; ++i) {
-      mbar_init(smem_u32(&ctrl->kv_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->kv_full[i]), kConvert ? kConvThreads : 1);
       mbar_init(smem_u32(&ctrl->kv_empty[i]), 1);
+    }
+    for (int i = 0; i < Cfg::kRawStages; ++i) {
+      mbar_init(smem_u32(&ctrl->raw_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->raw_empty[i]), kConvThreads);
     }
     for (int t = 0; t < 2; ++t) {
       mbar_init(smem_u32(&ctrl->q_full[t]), 128);
       mbar_init(smem_u32(&ctrl->s_full[t]), 1);
       mbar_init(smem_u32(&ctrl->p_full[t]), 128);
       mbar_init(smem_u32(&ctrl->o_full[t]), 1);
+      mbar_init(smem_u32(&ctrl->o_empty[t]), 4);
+      mbar_init(smem_u32(&ctrl->l_ready[t]), 128);
       mbar_init(smem_u32(&ctrl->item_full[t]), 1);
-      mbar_init(smem_u32(&ctrl->item_empty[t]), 257);  // 256 softmax threads + MMA lane 0
+      mbar_init(smem_u32(&ctrl->item_empty[t]), kItemReaders);
     }
     fence_mbar_init();
   }
-  if (warp == kProducerWarp) {
+  if (warp == kProducerWarp && !kConvert) {
     if (lane == 0) {
       tma_prefetch_desc(&tmap_k);
       tma_prefetch_desc(&tmap_v);
@@ -278,7 +338,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
   const uint32_t tmem_base = ctrl->tmem_base;
 
   if (warp == kProducerWarp) {
-    // ================================================================= scheduler + TMA
+    // ================================================================= scheduler + producer
     setmaxnreg_dec<kOtherRegs>();
     // one pass over the users: items per layer (W) and aligned rows per (layer, head) (R)
     int W = 0, R = 0;
@@ -297,7 +357,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     const int total_q = (args.B > 0) ? __ldg(args.cand_offsets + args.B) : 0;
 
     UserCursor cur{0, 0, 0};
-    uint32_t kv_it = 0;
+    uint32_t kv_it = 0;   // bf16 ring position (TMA mode) / raw ring position (convert mode)
     for (uint32_t n = 0;; ++n) {
       const int islot = n & 1;
       mbar_wait(smem_u32(&ctrl->item_empty[islot]), ((n >> 1) & 1) ^ 1);
@@ -369,17 +429,33 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         for (int j = 0; j < nt; ++j) {
 #pragma unroll
           for (int kv = 0; kv < 2; ++kv) {
-            const uint32_t slot = kv_it % Cfg::kStages;
-            const uint32_t ph = (kv_it / Cfg::kStages) & 1;
-            mbar_wait(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
-            const uint32_t full = smem_u32(&ctrl->kv_full[slot]);
-            mbar_arrive_expect_tx(full, Cfg::kTileBytes);
-            const uint32_t dst = kv_smem + slot * Cfg::kTileBytes;
+            if constexpr (!kConvert) {
+              const uint32_t slot = kv_it % Cfg::kStages;
+              const uint32_t ph = (kv_it / Cfg::kStages) & 1;
+              mbar_wait(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
+              const uint32_t full = smem_u32(&ctrl->kv_full[slot]);
+              mbar_arrive_expect_tx(full, Cfg::kTileBytes);
+              const uint32_t dst = kv_smem + slot * Cfg::kTileBytes;
 #pragma unroll
-            for (int bx = 0; bx < Cfg::kBoxes; ++bx)
-              tma_load_2d(dst + bx * Cfg::kBoxBytes, kv == 0 ? &tmap_k : &tmap_v, bx * 64,
-                          kv_row0 + j * kTileN, full);
-            ++kv_it;
+              for (int bx = 0; bx < Cfg::kBoxes; ++bx)
+                tma_load_2d(dst + bx * Cfg::kBoxBytes, kv == 0 ? &tmap_k : &tmap_v, bx * 64,
+                            kv_row0 + j * kTileN, full);
+              ++kv_it;
+            } else {
+              const uint8_t* base = (kv == 0) ? args.k_raw : args.v_raw;
+#pragma unroll 1
+              for (int c = 0; c < Cfg::kRawPerTile; ++c) {
+                const uint32_t slot = kv_it % Cfg::kRawStages;
+                const uint32_t ph = (kv_it / Cfg::kRawStages) & 1;
+                mbar_wait(smem_u32(&ctrl->raw_empty[slot]), ph ^ 1);
+                const uint32_t full = smem_u32(&ctrl->raw_full[slot]);
+                mbar_arrive_expect_tx(full, Cfg::kRawSlotBytes);
+                const size_t row = static_cast<size_t>(kv_row0) + j * kTileN + c * Cfg::kRawRows;
+                bulk_load_1d(raw_smem + slot * Cfg::kRawSlotBytes,
+                             base + row * (D * Cfg::kElemBytes), Cfg::kRawSlotBytes, full);
+                ++kv_it;
+              }
+            }
           }
         }
       }
@@ -388,7 +464,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
   } else if (warp == kMmaWarp) {
     // ================================================================= MMA issuer
     setmaxnreg_dec<kOtherRegs>();
-    uint32_t kv_it = 0, q_it[2] = {0, 0}, sp_it[2] = {0, 0};
+    uint32_t kv_it = 0, q_it[2] = {0, 0}, sp_it[2] = {0, 0}, od_it[2] = {0, 0};
     const uint32_t tm_s[2] = {tmem_base, tmem_base + 128};
     const uint32_t tm_o[2] = {tmem_base + 256, tmem_base + 256 + D};
     for (uint32_t n = 0;; ++n) {
@@ -435,6 +511,11 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           const int keys_here = min(kTileN, it.n_keys - j * kTileN);
           const int ksteps = (keys_here + 15) >> 4;
           for (int t = 0; t < ntile; ++t) {
+            if (j == 0) {
+              // the epilogue group must have drained O_t of the previous item
+              mbar_wait(smem_u32(&ctrl->o_empty[t]), (od_it[t] & 1) ^ 1);
+              ++od_it[t];
+            }
             mbar_wait(smem_u32(&ctrl->p_full[t]), sp_it[t] & 1);
             ++sp_it[t];
             tc_fence_after();
@@ -482,6 +563,72 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
       __syncwarp();
     }
+  } else if (warp == kConvWarp0 || warp == kConvWarp0 + 1) {
+    // ================================================================= converters
+    setmaxnreg_dec<kOtherRegs>();
+    if constexpr (kConvert) {
+      const int ctid = threadIdx.x - kConvWarp0 * 32;  // 0..63
+      uint32_t kv_it = 0, raw_it = 0;
+      for (uint32_t n = 0;; ++n) {
+        const int islot = n & 1;
+        mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+        const WorkItem it = ctrl->items[islot];
+        if (!it.valid) break;
+        const int nt = (it.n_keys + kTileN - 1) / kTileN;
+        for (int jj = 0; jj < 2 * nt; ++jj) {  // K0 V0 K1 V1 ...
+          const uint32_t slot = kv_it % Cfg::kStages, ph = (kv_it / Cfg::kStages) & 1;
+          mbar_wait(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
+          const uint32_t tile = kv_smem + slot * Cfg::kTileBytes;
+#pragma unroll 1
+          for (int c = 0; c < Cfg::kRawPerTile; ++c) {
+            const uint32_t rslot = raw_it % Cfg::kRawStages, rph = (raw_it / Cfg::kRawStages) & 1;
+            mbar_wait(smem_u32(&ctrl->raw_full[rslot]), rph);
+            const uint32_t raw = raw_smem + rslot * Cfg::kRawSlotBytes;
+            if constexpr (KV == KV_FP8) {
+              constexpr int PPR = D / 16;                   // 16-byte pieces per row
+              constexpr int NP = Cfg::kRawRows * PPR;
+#pragma unroll 4
+              for (int p = ctid; p < NP; p += kConvThreads) {
+                const int row = p / PPR, c16 = p % PPR;
+                const uint4 v = lds128(raw + p * 16);
+                uint32_t o[8];
+                e4m3x4_to_bf16x4(v.x, o[0], o[1]);
+                e4m3x4_to_bf16x4(v.y, o[2], o[3]);
+                e4m3x4_to_bf16x4(v.z, o[4], o[5]);
+                e4m3x4_to_bf16x4(v.w, o[6], o[7]);
+                const int ca = 2 * c16, cb = 2 * c16 + 1;
+                const uint32_t rbase = tile + row * 128;
+                sts128(rbase + (ca >> 3) * Cfg::kBoxBytes + (((ca & 7) ^ (row & 7)) << 4), o[0], o[1],
+                       o[2], o[3]);
+                sts128(rbase + (cb >> 3) * Cfg::kBoxBytes + (((cb & 7) ^ (row & 7)) << 4), o[4], o[5],
+                       o[6], o[7]);
+              }
+            } else {
+              constexpr int PPR = D / 8;                    // 32-byte pieces (8 floats) per row
+              constexpr int NP = Cfg::kRawRows * PPR;
+#pragma unroll 2
+              for (int p = ctid; p < NP; p += kConvThreads) {
+                const int row = c * Cfg::kRawRows + p / PPR, cc = p % PPR;
+                const uint4 a = lds128(raw + p * 32), b = lds128(raw + p * 32 + 16);
+                const uint32_t o0 = pack_bf16x2(__uint_as_float(a.x), __uint_as_float(a.y));
+                const uint32_t o1 = pack_bf16x2(__uint_as_float(a.z), __uint_as_float(a.w));
+                const uint32_t o2 = pack_bf16x2(__uint_as_float(b.x), __uint_as_float(b.y));
+                const uint32_t o3 = pack_bf16x2(__uint_as_float(b.z), __uint_as_float(b.w));
+                sts128(tile + row * 128 + (cc >> 3) * Cfg::kBoxBytes + (((cc & 7) ^ (row & 7)) << 4),
+                       o0, o1, o2, o3);
+              }
+            }
+            mbar_arrive(smem_u32(&ctrl->raw_empty[rslot]));
+            ++raw_it;
+          }
+          fence_proxy_async_smem();   // generic-proxy tile writes -> visible to tcgen05.mma
+          mbar_arrive(smem_u32(&ctrl->kv_full[slot]));
+          ++kv_it;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+      }
+    }
   } else if (warp < 8) {
     // ================================================================= softmax groups
     setmaxnreg_inc<kSoftmaxRegs>();
@@ -491,7 +638,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     const uint32_t tm_s = tmem_base + lane_base + t * 128;
     const uint32_t tm_o = tmem_base + lane_base + 256 + t * D;
     const uint32_t q_tile_smem = q_smem + t * Cfg::kTileBytes;
-    uint32_t sp_it = 0, o_it = 0;
+    uint32_t sp_it = 0;
     const bool has_self = (args.k_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
     const size_t row_stride = static_cast<size_t>(args.H) * D;
@@ -538,7 +685,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         }
         const int sidx = it.layer * args.H + it.h;
         const float ks = args.k_scale ? __ldg(args.k_scale + sidx) : 1.0f;
-        const float vs = args.v_scale ? __ldg(args.v_scale + sidx) : 1.0f;
         const float c_log2 = args.scale_log2 * ks;  // multiplies raw S
 
         // running state, log2 units. The self key (first split only) seeds it.
@@ -594,78 +740,120 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           } else if (__any_sync(0xffffffffu, need)) {
             const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
 #pragma unroll
-            for (int c0 = 0; c0 < D; c0 += 32) {
-              uint32_t orr[32];
-              tmem_ld32(tm_o + c0, orr);
+            for (int c0 = 0; c0 < D; c0 += 16) {
+              uint32_t orr[16];
+              tmem_ld16(tm_o + c0, orr);
               tmem_wait_ld_regs(orr);
 #pragma unroll
-              for (int c = 0; c < 32; ++c)
+              for (int c = 0; c < 16; ++c)
                 orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
-              tmem_st32(tm_o + c0, orr);
+              tmem_st16(tm_o + c0, orr);
             }
             l *= alpha;
             if (need) m_used = m_new;
           }
           if (pingpong) named_bar_sync(1 + t, 256);
-          // P = exp2(S*c - m) as bf16 pairs for the PV MMA.  The row sum (4 chains) adds the
-          // bf16-ROUNDED weights, i.e. exactly what the MMA multiplies, so out = sum(p~ v) /
-          // sum(p~) stays a convex combination of V rows (matters when few keys dominate).
+          // P = exp2(S*c - m) as bf16 pairs for the PV MMA, written back over S in chunks of
+          // 32 keys.  The row sum (4 chains) adds the bf16-ROUNDED weights, i.e. exactly
+          // what the MMA multiplies, so out = sum(p~ v) / sum(p~) stays a convex combination
+          // of V rows (matters when few keys dominate).
           float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
-          uint32_t pr[64];
 #pragma unroll
-          for (int c = 0; c < kTileN; c += 4) {
-            const float p0 = ex2_approx(fmaf(__uint_as_float(sr[c + 0]), c_log2, -m_used));
-            const float p1 = ex2_approx(fmaf(__uint_as_float(sr[c + 1]), c_log2, -m_used));
-            const float p2 = ex2_approx(fmaf(__uint_as_float(sr[c + 2]), c_log2, -m_used));
-            const float p3 = ex2_approx(fmaf(__uint_as_float(sr[c + 3]), c_log2, -m_used));
-            const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
-            pr[(c >> 1) + 0] = w01;
-            pr[(c >> 1) + 1] = w23;
+          for (int c0 = 0; c0 < kTileN; c0 += 32) {
+            uint32_t pr[16];
+#pragma unroll
+            for (int c = 0; c < 32; c += 4) {
+              const float p0 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 0]), c_log2, -m_used));
+              const float p1 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 1]), c_log2, -m_used));
+              const float p2 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 2]), c_log2, -m_used));
+              const float p3 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 3]), c_log2, -m_used));
+              const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
+              pr[(c >> 1) + 0] = w01;
+              pr[(c >> 1) + 1] = w23;
 #if UPR_CONSISTENT_ROWSUM
-            sum0 += __uint_as_float(w01 << 16);
-            sum1 += __uint_as_float(w01 & 0xffff0000u);
-            sum2 += __uint_as_float(w23 << 16);
-            sum3 += __uint_as_float(w23 & 0xffff0000u);
+              sum0 += __uint_as_float(w01 << 16);
+              sum1 += __uint_as_float(w01 & 0xffff0000u);
+              sum2 += __uint_as_float(w23 << 16);
+              sum3 += __uint_as_float(w23 & 0xffff0000u);
 #else
-            sum0 += p0; sum1 += p1; sum2 += p2; sum3 += p3;
+              sum0 += p0; sum1 += p1; sum2 += p2; sum3 += p3;
 #endif
+            }
+            tmem_st16(tm_s + (c0 >> 1), pr);
           }
           if (pingpong && !(t == 1 && j == nt - 1)) named_bar_arrive(2 - t, 256);
           l += (sum0 + sum1) + (sum2 + sum3);
-          tmem_st32(tm_s + 0, &pr[0]);
-          tmem_st32(tm_s + 32, &pr[32]);
           tmem_wait_st();
           tc_fence_before();
           mbar_arrive(smem_u32(&ctrl->p_full[t]));
           ++sp_it;
         }
+        if (nt == 0) prefetch_next_q();
 
-        // ------------------------------------------------------------ epilogue (a7 / a8)
-        if (nt > 0) {
-          mbar_wait(smem_u32(&ctrl->o_full[t]), o_it & 1);
-          ++o_it;
-          tc_fence_after();
-        } else {
-          prefetch_next_q();
-        }
+        // ---------------------------------------------------------- hand over to the epilogue
         const bool partial = args.num_splits > 1;
-        float w_self = 0.f;
-        if (self_here) w_self = ex2_approx(s_self - m_used);
-        const float inv = (!partial && l > 0.f) ? (1.0f / l) : (partial ? 1.0f : 0.f);
-        float* dst;
-        if (!partial) {
-          dst = args.out + my_elem0;
-        } else {
+        ctrl->epi_inv[islot][t][tid128] = partial ? 1.0f : (l > 0.f ? 1.0f / l : 0.f);
+        ctrl->epi_wself[islot][t][tid128] = self_here ? ex2_approx(s_self - m_used) : 0.f;
+        if (partial && row_valid) {
           const size_t prow =
               ((static_cast<size_t>(it.layer) * it.total_q + it.q_row0 + t * kTileM + tid128) *
                    args.H + it.h) * args.num_splits + it.split;
-          dst = args.part_o + prow * D;
-          if (row_valid) {
-            args.part_ml[prow * 2 + 0] = m_used;
-            args.part_ml[prow * 2 + 1] = l;
-          }
+          args.part_ml[prow * 2 + 0] = m_used;
+          args.part_ml[prow * 2 + 1] = l;
         }
-#pragma unroll
+        mbar_arrive(smem_u32(&ctrl->l_ready[t]));
+      } else {
+        // inactive tile: its Q buffer is idle, so the next item's tile can be staged now
+        prefetch_next_q();
+      }
+      mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+    }
+  } else {
+    // ================================================================= epilogue group (a7)
+    setmaxnreg_dec<kEpilogueRegs>();
+    const int ew = warp - kEpiWarp0;                     // TMEM lane quarter of this warp
+    const uint32_t lane_base = static_cast<uint32_t>(ew * 32) << 16;
+    const uint32_t stage = epi_smem + ew * (32 * kEpiRowBytes);
+    const bool has_self = (args.v_self != nullptr);
+    const bool q32 = args.q_is_f32 != 0;
+    const bool partial = args.num_splits > 1;
+    uint32_t lr_it[2] = {0, 0}, of_it[2] = {0, 0};
+    for (uint32_t n = 0;; ++n) {
+      const int islot = n & 1;
+      mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+      const WorkItem it = ctrl->items[islot];
+      if (!it.valid) break;
+      const int nt = (it.n_keys + kTileN - 1) / kTileN;
+      const bool self_here = has_self && it.split == 0;
+      const float vs = args.v_scale ? __ldg(args.v_scale + it.layer * args.H + it.h) : 1.0f;
+#pragma unroll 1
+      for (int t = 0; t < 2; ++t) {
+        const int rows_here = min(kTileM, it.n_rows - t * kTileM);
+        if (rows_here <= 0) break;
+        mbar_wait(smem_u32(&ctrl->l_ready[t]), lr_it[t] & 1);
+        ++lr_it[t];
+        if (nt > 0) {
+          mbar_wait(smem_u32(&ctrl->o_full[t]), of_it[t] & 1);
+          ++of_it[t];
+          tc_fence_after();
+        }
+        const int row = ew * 32 + lane;                  // row of this thread within the tile
+        const float inv = ctrl->epi_inv[islot][t][row];
+        const float wself = ctrl->epi_wself[islot][t][row];
+        const size_t grow0 = static_cast<size_t>(it.layer) * it.total_q + it.q_row0 + t * kTileM;
+        // candidate-side element offset of (row 0 of the tile, head h)
+        const size_t q_elem0 = (grow0 * args.H + it.h) * D;
+        float* dst0;
+        size_t dst_stride;
+        if (!partial) {
+          dst0 = args.out + q_elem0;
+          dst_stride = static_cast<size_t>(args.H) * D;
+        } else {
+          dst0 = args.part_o + ((grow0 * args.H + it.h) * args.num_splits + it.split) * D;
+          dst_stride = static_cast<size_t>(args.H) * args.num_splits * D;
+        }
+        const uint32_t tm_o = tmem_base + lane_base + 256 + t * D;
+#pragma unroll 1
         for (int c0 = 0; c0 < D; c0 += 32) {
           uint32_t orr[32];
           if (nt > 0) {
@@ -675,38 +863,64 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
 #pragma unroll
             for (int c = 0; c < 32; ++c) orr[c] = 0u;
           }
-          if (row_valid) {
+          const bool add_self = self_here && row < rows_here;
+          const size_t se = q_elem0 + static_cast<size_t>(row) * args.H * D + c0;
 #pragma unroll
-            for (int c = 0; c < 32; c += 4) {
-              float4 o;
-              o.x = __uint_as_float(orr[c + 0]) * vs;
-              o.y = __uint_as_float(orr[c + 1]) * vs;
-              o.z = __uint_as_float(orr[c + 2]) * vs;
-              o.w = __uint_as_float(orr[c + 3]) * vs;
-              if (self_here) {
-                const size_t e = my_elem0 + c0 + c;
-                o.x = fmaf(w_self, load_elem_f(args.v_self, q32, e + 0), o.x);
-                o.y = fmaf(w_self, load_elem_f(args.v_self, q32, e + 1), o.y);
-                o.z = fmaf(w_self, load_elem_f(args.v_self, q32, e + 2), o.z);
-                o.w = fmaf(w_self, load_elem_f(args.v_self, q32, e + 3), o.w);
+          for (int c = 0; c < 32; c += 8) {
+            float sv[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k) sv[k] = 0.f;
+            if (add_self) {
+              if (!q32) {
+                const uint4 x = __ldg(reinterpret_cast<const uint4*>(
+                    static_cast<const __nv_bfloat16*>(args.v_self) + se + c));
+                const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                  sv[2 * k + 0] = __uint_as_float(w[k] << 16);
+                  sv[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+                }
+              } else {
+                const float4* s4 =
+                    reinterpret_cast<const float4*>(static_cast<const float*>(args.v_self) + se + c);
+                const float4 a = __ldg(s4), b = __ldg(s4 + 1);
+                sv[0] = a.x; sv[1] = a.y; sv[2] = a.z; sv[3] = a.w;
+                sv[4] = b.x; sv[5] = b.y; sv[6] = b.z; sv[7] = b.w;
               }
-              o.x *= inv; o.y *= inv; o.z *= inv; o.w *= inv;
-              *reinterpret_cast<float4*>(dst + c0 + c) = o;
             }
+            float o[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+              o[k] = fmaf(wself, sv[k], __uint_as_float(orr[c + k]) * vs) * inv;
+            const uint32_t a = stage + lane * kEpiRowBytes + c * 4;
+            sts128(a, __float_as_uint(o[0]), __float_as_uint(o[1]), __float_as_uint(o[2]),
+                   __float_as_uint(o[3]));
+            sts128(a + 16, __float_as_uint(o[4]), __float_as_uint(o[5]), __float_as_uint(o[6]),
+                   __float_as_uint(o[7]));
           }
+          __syncwarp();
+          // transposed read-back: 8 lanes cover one row's 128-byte line, 4 rows per access
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const int r = 4 * k + (lane >> 3);
+            const uint4 v = lds128(stage + r * kEpiRowBytes + (lane & 7) * 16);
+            const int trow = ew * 32 + r;
+            if (trow < rows_here)
+              *reinterpret_cast<uint4*>(dst0 + static_cast<size_t>(trow) * dst_stride + c0 +
+                                        (lane & 7) * 4) = v;
+          }
+          __syncwarp();
         }
-        tc_fence_before();
-      } else {
-        // inactive tile: its Q buffer is idle, so the next item's tile can be staged now
-        prefetch_next_q();
+        if (nt > 0) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&ctrl->o_empty[t]));
+        }
       }
-      mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
     }
-  } else {
-    // warps 10, 11: no role (they exist so that warps 8-11 form a warpgroup for setmaxnreg)
-    setmaxnreg_dec<kOtherRegs>();
   }
-
 
   // ------------------------------------------------------------------ teardown
   tc_fence_before();

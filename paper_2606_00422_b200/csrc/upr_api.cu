@@ -116,8 +116,8 @@ upr_status validate(const upr_attn_params* p) {
                 p->B, p->H, p->n_layers, (long long)p->total_q);
   if (p->d != 64 && p->d != 128)
     return fail(UPR_ERR_UNSUPPORTED, "head dim d=%d unsupported (64 or 128)", p->d);
-  if (p->kv_dtype != UPR_BF16)
-    return fail(UPR_ERR_UNSUPPORTED, "kv_dtype %d not implemented yet (bf16 only)", p->kv_dtype);
+  if (p->kv_dtype != UPR_BF16 && p->kv_dtype != UPR_FP8_E4M3 && p->kv_dtype != UPR_F32)
+    return fail(UPR_ERR_UNSUPPORTED, "kv_dtype %d unsupported (f32, bf16 or fp8 e4m3)", p->kv_dtype);
   if (p->q_dtype != UPR_BF16 && p->q_dtype != UPR_F32)
     return fail(UPR_ERR_UNSUPPORTED, "q_dtype %d unsupported (bf16 or f32)", p->q_dtype);
   if (p->B > 0 && p->total_q > 0 &&
@@ -132,20 +132,30 @@ upr_status validate(const upr_attn_params* p) {
   return UPR_OK;
 }
 
-template <int D>
+template <int D, int KV>
 upr_status launch_attn(const upr::AttnArgs& a, const CUtensorMap& tk, const CUtensorMap& tv,
                        int grid, cudaStream_t st) {
-  using Cfg = upr::AttnCfg<D>;
+  using Cfg = upr::AttnCfg<D, KV>;
   static bool attr_set = false;
   if (!attr_set) {
-    UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::upr_attn_fwd_kernel<D>,
+    UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::upr_attn_fwd_kernel<D, KV>,
                                         cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         Cfg::kSmemTotal));
     attr_set = true;
   }
-  upr::upr_attn_fwd_kernel<D><<<grid, upr::kAttnThreads, Cfg::kSmemTotal, st>>>(tk, tv, a);
+  upr::upr_attn_fwd_kernel<D, KV><<<grid, upr::kAttnThreads, Cfg::kSmemTotal, st>>>(tk, tv, a);
   UPR_CUDA_CHECK(cudaGetLastError());
   return UPR_OK;
+}
+
+template <int D>
+upr_status launch_attn_d(int kv_dtype, const upr::AttnArgs& a, const CUtensorMap& tk,
+                         const CUtensorMap& tv, int grid, cudaStream_t st) {
+  switch (kv_dtype) {
+    case UPR_BF16: return launch_attn<D, upr::KV_BF16>(a, tk, tv, grid, st);
+    case UPR_FP8_E4M3: return launch_attn<D, upr::KV_FP8>(a, tk, tv, grid, st);
+    default: return launch_attn<D, upr::KV_F32>(a, tk, tv, grid, st);
+  }
 }
 
 upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t st) {
@@ -192,11 +202,21 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
     }
   }
 
+  // bf16 caches are read through TMA tensor maps; fp8 / fp32 caches as contiguous raw rows
   CUtensorMap tk, tv;
-  s = make_kv_tmap(&tk, p->k_cache, p->d);
-  if (s != UPR_OK) return s;
-  s = make_kv_tmap(&tv, p->v_cache, p->d);
-  if (s != UPR_OK) return s;
+  memset(&tk, 0, sizeof(tk));
+  memset(&tv, 0, sizeof(tv));
+  if (p->kv_dtype == UPR_BF16) {
+    s = make_kv_tmap(&tk, p->k_cache, p->d);
+    if (s != UPR_OK) return s;
+    s = make_kv_tmap(&tv, p->v_cache, p->d);
+    if (s != UPR_OK) return s;
+  } else {
+    if ((reinterpret_cast<uintptr_t>(p->k_cache) & 15) || (reinterpret_cast<uintptr_t>(p->v_cache) & 15))
+      return fail(UPR_ERR_INVALID_ARG, "k_cache / v_cache must be 16-byte aligned");
+    a.k_raw = static_cast<const uint8_t*>(p->k_cache);
+    a.v_raw = static_cast<const uint8_t*>(p->v_cache);
+  }
 
   // persistent grid: one CTA per SM, never more CTAs than an upper bound on the item count
   long long max_items = ((p->total_q + upr::kQBlock - 1) / upr::kQBlock + p->B) *
@@ -205,7 +225,8 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   if (grid <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
   if (max_items < grid) grid = static_cast<int>(max_items < 1 ? 1 : max_items);
 
-  s = (p->d == 64) ? launch_attn<64>(a, tk, tv, grid, st) : launch_attn<128>(a, tk, tv, grid, st);
+  s = (p->d == 64) ? launch_attn_d<64>(p->kv_dtype, a, tk, tv, grid, st)
+                   : launch_attn_d<128>(p->kv_dtype, a, tk, tv, grid, st);
   if (s != UPR_OK) return s;
   g_launches = 1;
   if (ns > 1) {

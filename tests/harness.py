@@ -42,6 +42,39 @@ class Inputs:
         s = int(self.slot_ids_host[b])
         return to_f64(self.k_pool[l, s, h, :Lb]), to_f64(self.v_pool[l, s, h, :Lb])
 
+    def oracle_fp8_cache(self):
+        """(k_bytes, k_scale, v_bytes, v_scale, row_off, R): the ORACLE's E4M3 pack of the whole pools
+        (small workloads only: the oracle's nearest-code search costs ~0.1 us per element)."""
+        if not hasattr(self, "_fp8"):
+            kc, ks = oracle.pack(bits(self.k_pool), self.slot_ids_host, self.w.seq_lens, oracle.FP8_E4M3)
+            vc, vs = oracle.pack(bits(self.v_pool), self.slot_ids_host, self.w.seq_lens, oracle.FP8_E4M3)
+            lay = oracle.layout(self.w.seq_lens, self.w.H, self.w.d, self.w.n_layers, oracle.FP8_E4M3)
+            self._fp8 = (kc, ks, vc, vs, lay["row_off"], lay["R"])
+        return self._fp8
+
+    def _oracle_fp8_head(self, l: int, h: int):
+        """The oracle's E4M3 pack of ONE (layer, head) slice of the pools, all users: the scale is
+        per (layer, head) over every user's valid rows, so this slice is self-contained."""
+        cache = self.__dict__.setdefault("_fp8_head", {})
+        if (l, h) not in cache:
+            kp = bits(self.k_pool[l:l + 1, :, h:h + 1])
+            vp = bits(self.v_pool[l:l + 1, :, h:h + 1])
+            kc, ks = oracle.pack(kp, self.slot_ids_host, self.w.seq_lens, oracle.FP8_E4M3)
+            vc, vs = oracle.pack(vp, self.slot_ids_host, self.w.seq_lens, oracle.FP8_E4M3)
+            lay = oracle.layout(self.w.seq_lens, 1, self.w.d, 1, oracle.FP8_E4M3)
+            cache.clear()                                  # keep one slice at a time
+            cache[(l, h)] = (kc, float(ks[0]), vc, float(vs[0]), lay["row_off"])
+        return cache[(l, h)]
+
+    def block_kv_dequant_f64(self, l: int, b: int, h: int):
+        """History K/V of one block as the FP8 cache stores them: decode(byte) * scale, exact in fp64."""
+        kc, ks, vc, vs, row_off = self._oracle_fp8_head(l, h)
+        d, Lb = self.w.d, int(self.w.seq_lens[b])
+        r0 = int(row_off[b]) * d
+        K = oracle.e4m3_decode(kc[r0:r0 + Lb * d]).reshape(Lb, d) * ks
+        V = oracle.e4m3_decode(vc[r0:r0 + Lb * d]).reshape(Lb, d) * vs
+        return K, V
+
     def block_q_f64(self, l: int, b: int, h: int):
         co = self.w.cand_offsets
         sl = slice(int(co[b]), int(co[b + 1]))
@@ -51,22 +84,22 @@ class Inputs:
         return q, to_f64(self.k_self[l, sl, h]), to_f64(self.v_self[l, sl, h])
 
 
-def oracle_block(inp: Inputs, l: int, b: int, h: int, sm_scale=None) -> np.ndarray:
-    K, V = inp.block_kv_f64(l, b, h)
+def oracle_block(inp: Inputs, l: int, b: int, h: int, sm_scale=None, dequant: bool = False) -> np.ndarray:
+    K, V = inp.block_kv_dequant_f64(l, b, h) if dequant else inp.block_kv_f64(l, b, h)
     q, ks, vs = inp.block_q_f64(l, b, h)
     return oracle.attn_block(q, K, V, ks, vs, scale=sm_scale)
 
 
-def oracle_all(inp: Inputs, sm_scale=None) -> np.ndarray:
+def oracle_all(inp: Inputs, sm_scale=None, dequant: bool = False) -> np.ndarray:
     w = inp.w
     out = np.zeros((w.n_layers, w.total_q, w.H, w.d))
     co = w.cand_offsets
     for l in range(w.n_layers):
-        for b in range(w.B):
-            if co[b + 1] == co[b]:
-                continue
-            for h in range(w.H):
-                out[l, co[b]:co[b + 1], h] = oracle_block(inp, l, b, h, sm_scale)
+        for h in range(w.H):
+            for b in range(w.B):
+                if co[b + 1] == co[b]:
+                    continue
+                out[l, co[b]:co[b + 1], h] = oracle_block(inp, l, b, h, sm_scale, dequant)
     return out
 
 
