@@ -40,13 +40,14 @@
 namespace upr {
 
 constexpr int kTileM = 128;     // candidate rows per MMA tile == TMEM lanes
-constexpr int kTileN = 128;     // keys per K/V tile
+constexpr int kTileN = 128;     // keys per K/V smem tile
+constexpr int kSubN = 64;       // keys per softmax / MMA step (two S buffers per candidate tile)
 constexpr int kQBlock = 256;    // candidate rows per work item (two tiles)
 constexpr int kRowAlign = 16;   // UPR_ROW_ALIGN
 constexpr int kAttnThreads = 512;     // 2 softmax warpgroups + {TMA, MMA, 2 converters} + epilogue
-constexpr int kSoftmaxRegs = 200;     // setmaxnreg budgets (sum over 512 threads <= 64 K registers)
-constexpr int kOtherRegs = 48;        //   producer / MMA / converter warpgroup
-constexpr int kEpilogueRegs = 64;     //   epilogue warpgroup
+constexpr int kSoftmaxRegs = 168;     // setmaxnreg budgets (sum over 512 threads <= 64 K registers)
+constexpr int kOtherRegs = 56;        //   producer / MMA / converter warpgroup
+constexpr int kEpilogueRegs = 88;     //   epilogue warpgroup
 constexpr int kProducerWarp = 8;
 constexpr int kMmaWarp = 9;
 constexpr int kConvWarp0 = 10;        // warps 10, 11
@@ -108,7 +109,7 @@ struct AttnCfg {
   static constexpr int kSmemCtrl = 6144;
   static constexpr int kSmemTotal =
       kSmemQ + kSmemKV + kSmemRaw + kSmemEpi + kSmemCtrl + 1024;  // + alignment slack
-  static constexpr uint32_t kIdescQK = make_idesc_bf16(kTileM, kTileN, 0, 0);
+  static constexpr uint32_t kIdescQK = make_idesc_bf16(kTileM, kSubN, 0, 0);
   static constexpr uint32_t kIdescPV = make_idesc_bf16(kTileM, D, 0, 1);
   static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
 };
@@ -119,8 +120,9 @@ struct __align__(16) AttnCtrl {
   uint64_t raw_full[4];
   uint64_t raw_empty[4];
   uint64_t q_full[2];
-  uint64_t s_full[2];
-  uint64_t p_full[2];
+  uint64_t s_full[2][2];   // [tile][S buffer]
+  uint64_t p_full[2][2];
+  uint64_t pv_done[2];     // one completion per PV sub-tile MMA of tile t
   uint64_t o_full[2];
   uint64_t o_empty[2];
   uint64_t l_ready[2];
@@ -312,8 +314,11 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     }
     for (int t = 0; t < 2; ++t) {
       mbar_init(smem_u32(&ctrl->q_full[t]), 128);
-      mbar_init(smem_u32(&ctrl->s_full[t]), 1);
-      mbar_init(smem_u32(&ctrl->p_full[t]), 128);
+      for (int bf = 0; bf < 2; ++bf) {
+        mbar_init(smem_u32(&ctrl->s_full[t][bf]), 1);
+        mbar_init(smem_u32(&ctrl->p_full[t][bf]), 128);
+      }
+      mbar_init(smem_u32(&ctrl->pv_done[t]), 1);
       mbar_init(smem_u32(&ctrl->o_full[t]), 1);
       mbar_init(smem_u32(&ctrl->o_empty[t]), 4);
       mbar_init(smem_u32(&ctrl->l_ready[t]), 128);
@@ -411,7 +416,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       const int key0 = t0 * kTileN;
       const int n_keys = (t1 > t0) ? (min(Lb, t1 * kTileN) - key0) : 0;
       const int kv_row0 = (layer * args.H + h) * R + row_off_b + key0;
-      if (lane == 0) {
+      if (elect_one()) {
         WorkItem& it = ctrl->items[islot];
         it.valid = 1;
         it.layer = layer;
@@ -463,104 +468,127 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     }
   } else if (warp == kMmaWarp) {
     // ================================================================= MMA issuer
+    // Keys are processed in sub-tiles of 64 (two per 128-key smem tile).  Each candidate tile
+    // t owns two 64-column S buffers, so S(s+2) is issued right behind PV(s) -- i.e. S(s+1) is
+    // being computed while the softmax group works on S(s): the softmax warps never wait for
+    // the tensor pipe in steady state.  P(s) aliases the first 32 columns of S buffer s & 1.
     setmaxnreg_dec<kOtherRegs>();
-    uint32_t kv_it = 0, q_it[2] = {0, 0}, sp_it[2] = {0, 0}, od_it[2] = {0, 0};
-    const uint32_t tm_s[2] = {tmem_base, tmem_base + 128};
-    const uint32_t tm_o[2] = {tmem_base + 256, tmem_base + 256 + D};
+    uint32_t kv_it = 0, q_it[2] = {0, 0}, od_it[2] = {0, 0};
+    uint32_t pf_it[2][2] = {{0, 0}, {0, 0}};   // p_full phase counters [tile][buffer]
+    // Everything that feeds an MMA operand is made provably warp-uniform (shuffle from lane
+    // 0), so that descriptors are built on the uniform datapath: a value loaded from shared
+    // memory is per-thread to the compiler, which otherwise wraps every tcgen05.mma in a
+    // R2UR waterfall loop (measured: ~15 instructions per MMA, the MMA warp became the
+    // bottleneck of the whole CTA).
+    auto uni = [](int v) { return __shfl_sync(0xffffffffu, v, 0); };
+    const uint32_t tmem_u = static_cast<uint32_t>(uni(static_cast<int>(tmem_base)));
+    const uint32_t tm_o[2] = {tmem_u + 256, tmem_u + 256 + D};
+    // descriptor words: lo = addr >> 4 | (LBO >> 4) << 16, hi = SBO >> 4 | version 1 | SWIZZLE_128B
+    constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
+    constexpr uint32_t kLoKmajor = (16u >> 4) << 16;                    // Q, K: K-major
+    constexpr uint32_t kLoMNmajor = (static_cast<uint32_t>(Cfg::kBoxBytes) >> 4) << 16;   // V: MN-major
+    auto mk_desc = [](uint32_t lo) {
+      return (static_cast<uint64_t>(kDescHi) << 32) | static_cast<uint64_t>(lo);
+    };
+    const uint32_t q_lo = ((q_smem & 0x3FFFFu) >> 4) | kLoKmajor;
+    const uint32_t kv_lo = (kv_smem & 0x3FFFFu) >> 4;
     for (uint32_t n = 0;; ++n) {
       const int islot = n & 1;
       mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
-      const WorkItem it = ctrl->items[islot];
-      if (!it.valid) break;
-      const int nt = (it.n_keys + kTileN - 1) / kTileN;
-      const int ntile = (it.n_rows > kTileM) ? 2 : 1;
+      const int it_valid = uni(ctrl->items[islot].valid);
+      if (!it_valid) break;
+      const int it_n_keys = uni(ctrl->items[islot].n_keys);
+      const int it_n_rows = uni(ctrl->items[islot].n_rows);
+      const int nt = (it_n_keys + kTileN - 1) / kTileN;
+      const int nsub = (it_n_keys + kSubN - 1) / kSubN;
+      const int ntile = (it_n_rows > kTileM) ? 2 : 1;
       if (nt > 0) {
         for (int t = 0; t < ntile; ++t) {
           mbar_wait(smem_u32(&ctrl->q_full[t]), q_it[t] & 1);
           ++q_it[t];
         }
         tc_fence_after();
-        // S_t(0) = Q_t K(0)^T
-        {
-          const uint32_t slot = kv_it % Cfg::kStages, ph = (kv_it / Cfg::kStages) & 1;
-          mbar_wait(smem_u32(&ctrl->kv_full[slot]), ph);
-          tc_fence_after();
-          if (lane == 0) {
-            const uint32_t kb = kv_smem + slot * Cfg::kTileBytes;
-            for (int t = 0; t < ntile; ++t) {
-              const uint32_t qb = q_smem + t * Cfg::kTileBytes;
+        const uint32_t base = kv_it;   // ring position of K tile 0; K_j at base+2j, V_j at base+2j+1
+        auto slot_of = [&](uint32_t pos) { return pos % Cfg::kStages; };
+        auto phase_of = [&](uint32_t pos) { return (pos / Cfg::kStages) & 1u; };
+        // S_t(sub) = Q_t K[sub]^T into S buffer sub & 1 (lane 0 only)
+        auto issue_qk = [&](int t, int sub) {
+          const uint32_t k_lo = kv_lo + kLoKmajor +
+                                ((slot_of(base + 2 * (sub >> 1)) * Cfg::kTileBytes +
+                                  (sub & 1) * (kSubN * 128)) >> 4);
+          const uint32_t qt_lo = q_lo + ((t * Cfg::kTileBytes) >> 4);
+          const uint32_t ts = tmem_u + t * 128 + (sub & 1) * kSubN;
 #pragma unroll
-              for (int k = 0; k < D / 16; ++k) {
-                const uint32_t off = (k >> 2) * Cfg::kBoxBytes + (k & 3) * 32;
-                umma_ss(tm_s[t], make_smem_desc_sw128(qb + off, 16, 1024),
-                        make_smem_desc_sw128(kb + off, 16, 1024), Cfg::kIdescQK, k > 0);
-              }
-              umma_commit(smem_u32(&ctrl->s_full[t]));
-            }
-            umma_commit(smem_u32(&ctrl->kv_empty[slot]));
+          for (int k = 0; k < D / 16; ++k) {
+            const uint32_t off = ((k >> 2) * Cfg::kBoxBytes + (k & 3) * 32) >> 4;
+            umma_ss(ts, mk_desc(qt_lo + off), mk_desc(k_lo + off), Cfg::kIdescQK, k > 0);
           }
-          __syncwarp();
-          ++kv_it;
+          umma_commit(smem_u32(&ctrl->s_full[t][sub & 1]));
+        };
+        // prologue: S(0), S(1)
+        mbar_wait(smem_u32(&ctrl->kv_full[slot_of(base)]), phase_of(base));
+        tc_fence_after();
+        if (elect_one()) {
+          for (int sub = 0; sub < 2 && sub < nsub; ++sub)
+            for (int t = 0; t < ntile; ++t) issue_qk(t, sub);
+          umma_commit(smem_u32(&ctrl->kv_empty[slot_of(base)]));   // K tile 0: both sub-tiles issued
         }
-        for (int j = 0; j < nt; ++j) {
-          const uint32_t vslot = kv_it % Cfg::kStages, vph = (kv_it / Cfg::kStages) & 1;
-          ++kv_it;
-          const bool has_next = (j + 1 < nt);
-          const uint32_t kslot = kv_it % Cfg::kStages, kph = (kv_it / Cfg::kStages) & 1;
-          mbar_wait(smem_u32(&ctrl->kv_full[vslot]), vph);
-          const int keys_here = min(kTileN, it.n_keys - j * kTileN);
+        __syncwarp();
+        for (int sub = 0; sub < nsub; ++sub) {
+          const int bufi = sub & 1;
+          const uint32_t vpos = base + 2 * (sub >> 1) + 1;
+          if (bufi == 0) mbar_wait(smem_u32(&ctrl->kv_full[slot_of(vpos)]), phase_of(vpos));
+          const int nxt = sub + 2;                     // S sub-tile issued behind this PV
+          const bool has_next = nxt < nsub;
+          const uint32_t kpos = base + 2 * (nxt >> 1);
+          const int keys_here = min(kSubN, it_n_keys - sub * kSubN);
           const int ksteps = (keys_here + 15) >> 4;
           for (int t = 0; t < ntile; ++t) {
-            if (j == 0) {
+            if (sub == 0) {
               // the epilogue group must have drained O_t of the previous item
               mbar_wait(smem_u32(&ctrl->o_empty[t]), (od_it[t] & 1) ^ 1);
               ++od_it[t];
             }
-            mbar_wait(smem_u32(&ctrl->p_full[t]), sp_it[t] & 1);
-            ++sp_it[t];
+            mbar_wait(smem_u32(&ctrl->p_full[t][bufi]), pf_it[t][bufi] & 1);
+            ++pf_it[t][bufi];
             tc_fence_after();
-            if (lane == 0) {
-              const uint32_t vb = kv_smem + vslot * Cfg::kTileBytes;
-              for (int k = 0; k < ksteps; ++k) {
+            if (elect_one()) {
+              const uint32_t v_lo = kv_lo + kLoMNmajor +
+                                    ((slot_of(vpos) * Cfg::kTileBytes + bufi * (kSubN * 128)) >> 4);
+              const uint32_t tp = tmem_u + t * 128 + bufi * kSubN;
+#pragma unroll
+              for (int k = 0; k < kSubN / 16; ++k) {
                 // A = P_t[:, 16k..16k+16) : 8 TMEM columns of packed bf16 pairs
-                // B = V rows [16k, 16k+16) : MN-major, 8-row groups 1024 B apart, the two
-                //     64-column halves (D = 128) one box apart
-                umma_ts(tm_o[t], tm_s[t] + k * 8,
-                        make_smem_desc_sw128(vb + k * 2048, Cfg::kBoxBytes, 1024), Cfg::kIdescPV,
-                        (j > 0 || k > 0) ? 1u : 0u);
+                // B = V rows [16k, 16k+16) of the sub-tile: MN-major, 8-row groups 1024 B
+                //     apart, the two 64-column halves (D = 128) one box apart
+                if (k < ksteps)
+                  umma_ts(tm_o[t], tp + k * 8, mk_desc(v_lo + k * (2048 >> 4)), Cfg::kIdescPV,
+                          (sub > 0 || k > 0) ? 1u : 0u);
               }
+              umma_commit(smem_u32(&ctrl->pv_done[t]));
             }
             __syncwarp();
-            if (has_next && t == 0) {
-              mbar_wait(smem_u32(&ctrl->kv_full[kslot]), kph);
+            if (has_next && t == 0 && (nxt & 1) == 0) {
+              mbar_wait(smem_u32(&ctrl->kv_full[slot_of(kpos)]), phase_of(kpos));
               tc_fence_after();
             }
-            if (lane == 0) {
-              if (has_next) {
-                const uint32_t kb = kv_smem + kslot * Cfg::kTileBytes;
-                const uint32_t qb = q_smem + t * Cfg::kTileBytes;
-#pragma unroll
-                for (int k = 0; k < D / 16; ++k) {
-                  const uint32_t off = (k >> 2) * Cfg::kBoxBytes + (k & 3) * 32;
-                  umma_ss(tm_s[t], make_smem_desc_sw128(qb + off, 16, 1024),
-                          make_smem_desc_sw128(kb + off, 16, 1024), Cfg::kIdescQK, k > 0);
-                }
-                umma_commit(smem_u32(&ctrl->s_full[t]));
-              } else {
-                umma_commit(smem_u32(&ctrl->o_full[t]));
-              }
+            if (elect_one()) {
+              if (has_next) issue_qk(t, nxt);
+              else if (sub == nsub - 1) umma_commit(smem_u32(&ctrl->o_full[t]));
             }
             __syncwarp();
           }
-          if (lane == 0) {
-            umma_commit(smem_u32(&ctrl->kv_empty[vslot]));
-            if (has_next) umma_commit(smem_u32(&ctrl->kv_empty[kslot]));
+          if (elect_one()) {
+            // V tile done after its last sub-tile; K tile done after its last S sub-tile
+            if (bufi == 1 || sub == nsub - 1) umma_commit(smem_u32(&ctrl->kv_empty[slot_of(vpos)]));
+            if (has_next && ((nxt & 1) == 1 || nxt == nsub - 1))
+              umma_commit(smem_u32(&ctrl->kv_empty[slot_of(kpos)]));
           }
           __syncwarp();
-          if (has_next) ++kv_it;
         }
+        kv_it = base + 2 * nt;
       }
-      if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+      if (elect_one()) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
       __syncwarp();
     }
   } else if (warp == kConvWarp0 || warp == kConvWarp0 + 1) {
@@ -638,7 +666,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     const uint32_t tm_s = tmem_base + lane_base + t * 128;
     const uint32_t tm_o = tmem_base + lane_base + 256 + t * D;
     const uint32_t q_tile_smem = q_smem + t * Cfg::kTileBytes;
-    uint32_t sp_it = 0;
+    uint32_t sf_it[2] = {0, 0};              // s_full phase counters per S buffer
+    uint32_t pv_cnt = 0;                     // PV sub-tile MMAs of this tile issued so far (all items)
     const bool has_self = (args.k_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
     const size_t row_stride = static_cast<size_t>(args.H) * D;
@@ -662,7 +691,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       const WorkItem it = ctrl->items[islot];
       if (!it.valid) break;
       const int rows_here = min(kTileM, it.n_rows - t * kTileM);  // <= 0: tile inactive
-      const int nt = (rows_here > 0) ? (it.n_keys + kTileN - 1) / kTileN : 0;
+      const int nsub = (rows_here > 0) ? (it.n_keys + kSubN - 1) / kSubN : 0;
       // Prefetch the NEXT item's Q tile as soon as this item's last S_t MMA has read Q_t.
       auto prefetch_next_q = [&]() {
         const uint32_t n1 = n + 1;
@@ -676,7 +705,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       if (rows_here > 0) {
         const bool row_valid = tid128 < rows_here;
         const size_t my_elem0 = tile_elem0_of(it) + static_cast<size_t>(tid128) * row_stride;
-        if (nt > 0) {
+        if (nsub > 0) {
           if (!q_prefetched) issue_q(it);
           cp_async_wait_all();
           fence_proxy_async_smem();
@@ -696,33 +725,29 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           m_used = s_self;
           l = 1.f;
         }
-        // exp-phase ping-pong between the two groups (both tiles active): the MUFU-heavy
-        // phase of one group overlaps the MMAs of the other instead of colliding with its
-        // exp phase.  Barrier 1 = "group 0 may go", barrier 2 = "group 1 may go".
-        const bool pingpong = (it.n_rows > kTileM) && nt > 0;
-        if (pingpong && t == 1) named_bar_arrive(1, 256);
 
-        for (int j = 0; j < nt; ++j) {
-          mbar_wait(smem_u32(&ctrl->s_full[t]), sp_it & 1);
+        for (int sub = 0; sub < nsub; ++sub) {
+          const int bufi = sub & 1;
+          const uint32_t tm_sb = tm_s + bufi * kSubN;
+          mbar_wait(smem_u32(&ctrl->s_full[t][bufi]), sf_it[bufi] & 1);
+          ++sf_it[bufi];
           tc_fence_after();
-          if (j == nt - 1) prefetch_next_q();   // every S_t MMA of this item is complete
-          uint32_t sr[128];
-          tmem_ld32(tm_s + 0, &sr[0]);
-          tmem_ld32(tm_s + 32, &sr[32]);
-          tmem_ld32(tm_s + 64, &sr[64]);
-          tmem_ld32(tm_s + 96, &sr[96]);
+          if (sub == nsub - 1) prefetch_next_q();   // every S_t MMA of this item is complete
+          uint32_t sr[kSubN];
+          tmem_ld32(tm_sb + 0, &sr[0]);
+          tmem_ld32(tm_sb + 32, &sr[32]);
           tmem_wait_ld_regs(sr);
-          const int keys_here = it.n_keys - j * kTileN;  // may exceed 128
-          if (keys_here < kTileN) {
+          const int keys_here = it.n_keys - sub * kSubN;  // may exceed 64
+          if (keys_here < kSubN) {
 #pragma unroll
-            for (int c = 0; c < kTileN; ++c)
+            for (int c = 0; c < kSubN; ++c)
               if (c >= keys_here) sr[c] = 0xff800000u;  // -inf
           }
           // row max: 4 independent chains
           float mx0 = __uint_as_float(sr[0]), mx1 = __uint_as_float(sr[1]);
           float mx2 = __uint_as_float(sr[2]), mx3 = __uint_as_float(sr[3]);
 #pragma unroll
-          for (int c = 4; c < kTileN; c += 4) {
+          for (int c = 4; c < kSubN; c += 4) {
             mx0 = fmaxf(mx0, __uint_as_float(sr[c + 0]));
             mx1 = fmaxf(mx1, __uint_as_float(sr[c + 1]));
             mx2 = fmaxf(mx2, __uint_as_float(sr[c + 2]));
@@ -731,13 +756,16 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3));
           const float m_new = fmaxf(m_used, mx * c_log2);
           const bool need = m_new > m_used + kRescaleTau;
-          if (j == 0) {
+          if (sub == 0) {
             // nothing accumulated in O yet (first PV overwrites); only l may hold the self weight
             if (need) {
               l *= ex2_approx(m_used - m_new);
               m_used = m_new;
             }
           } else if (__any_sync(0xffffffffu, need)) {
+            // PV(sub-1) may still be accumulating into O_t: wait for it before touching O
+            mbar_wait(smem_u32(&ctrl->pv_done[t]), (pv_cnt - 1) & 1);
+            tc_fence_after();
             const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
 #pragma unroll
             for (int c0 = 0; c0 < D; c0 += 16) {
@@ -752,14 +780,13 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             l *= alpha;
             if (need) m_used = m_new;
           }
-          if (pingpong) named_bar_sync(1 + t, 256);
           // P = exp2(S*c - m) as bf16 pairs for the PV MMA, written back over S in chunks of
           // 32 keys.  The row sum (4 chains) adds the bf16-ROUNDED weights, i.e. exactly
           // what the MMA multiplies, so out = sum(p~ v) / sum(p~) stays a convex combination
           // of V rows (matters when few keys dominate).
           float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
 #pragma unroll
-          for (int c0 = 0; c0 < kTileN; c0 += 32) {
+          for (int c0 = 0; c0 < kSubN; c0 += 32) {
             uint32_t pr[16];
 #pragma unroll
             for (int c = 0; c < 32; c += 4) {
@@ -779,16 +806,15 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               sum0 += p0; sum1 += p1; sum2 += p2; sum3 += p3;
 #endif
             }
-            tmem_st16(tm_s + (c0 >> 1), pr);
+            tmem_st16(tm_sb + (c0 >> 1), pr);
           }
-          if (pingpong && !(t == 1 && j == nt - 1)) named_bar_arrive(2 - t, 256);
           l += (sum0 + sum1) + (sum2 + sum3);
           tmem_wait_st();
           tc_fence_before();
-          mbar_arrive(smem_u32(&ctrl->p_full[t]));
-          ++sp_it;
+          mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
+          ++pv_cnt;
         }
-        if (nt == 0) prefetch_next_q();
+        if (nsub == 0) prefetch_next_q();
 
         // ---------------------------------------------------------- hand over to the epilogue
         const bool partial = args.num_splits > 1;
