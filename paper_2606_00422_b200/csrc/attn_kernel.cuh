@@ -365,7 +365,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     uint32_t kv_it = 0;   // bf16 ring position (TMA mode) / raw ring position (convert mode)
     for (uint32_t n = 0;; ++n) {
       const int islot = n & 1;
-      mbar_wait(smem_u32(&ctrl->item_empty[islot]), ((n >> 1) & 1) ^ 1);
+      mbar_wait<1>(smem_u32(&ctrl->item_empty[islot]), ((n >> 1) & 1) ^ 1);
       int idx;
       if (args.counter != nullptr) {
         idx = 0;
@@ -437,7 +437,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             if constexpr (!kConvert) {
               const uint32_t slot = kv_it % Cfg::kStages;
               const uint32_t ph = (kv_it / Cfg::kStages) & 1;
-              mbar_wait(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
+              mbar_wait<2>(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
               const uint32_t full = smem_u32(&ctrl->kv_full[slot]);
               mbar_arrive_expect_tx(full, Cfg::kTileBytes);
               const uint32_t dst = kv_smem + slot * Cfg::kTileBytes;
@@ -452,7 +452,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               for (int c = 0; c < Cfg::kRawPerTile; ++c) {
                 const uint32_t slot = kv_it % Cfg::kRawStages;
                 const uint32_t ph = (kv_it / Cfg::kRawStages) & 1;
-                mbar_wait(smem_u32(&ctrl->raw_empty[slot]), ph ^ 1);
+                mbar_wait<3>(smem_u32(&ctrl->raw_empty[slot]), ph ^ 1);
                 const uint32_t full = smem_u32(&ctrl->raw_full[slot]);
                 mbar_arrive_expect_tx(full, Cfg::kRawSlotBytes);
                 const size_t row = static_cast<size_t>(kv_row0) + j * kTileN + c * Cfg::kRawRows;
@@ -470,127 +470,127 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     // ================================================================= MMA issuer
     // Keys are processed in sub-tiles of 64 (two per 128-key smem tile).  Each candidate tile
     // t owns two 64-column S buffers, so S(s+2) is issued right behind PV(s) -- i.e. S(s+1) is
-    // being computed while the softmax group works on S(s): the softmax warps never wait for
+    // being computed while the softmax group works on S(s): the softmax warps do not wait for
     // the tensor pipe in steady state.  P(s) aliases the first 32 columns of S buffer s & 1.
+    //
+    // The whole role runs in ONE elected thread: inside an elect.sync region the compiler
+    // knows every value is warp-uniform and builds descriptors on the uniform datapath (with
+    // a plain lane test it wraps each tcgen05.mma in a R2UR waterfall loop), and there is no
+    // reconvergence or warp-sync traffic on what is the serial critical path of the CTA.
     setmaxnreg_dec<kOtherRegs>();
-    uint32_t kv_it = 0, q_it[2] = {0, 0}, od_it[2] = {0, 0};
-    uint32_t pf_it[2][2] = {{0, 0}, {0, 0}};   // p_full phase counters [tile][buffer]
-    // Everything that feeds an MMA operand is made provably warp-uniform (shuffle from lane
-    // 0), so that descriptors are built on the uniform datapath: a value loaded from shared
-    // memory is per-thread to the compiler, which otherwise wraps every tcgen05.mma in a
-    // R2UR waterfall loop (measured: ~15 instructions per MMA, the MMA warp became the
-    // bottleneck of the whole CTA).
-    auto uni = [](int v) { return __shfl_sync(0xffffffffu, v, 0); };
-    const uint32_t tmem_u = static_cast<uint32_t>(uni(static_cast<int>(tmem_base)));
-    const uint32_t tm_o[2] = {tmem_u + 256, tmem_u + 256 + D};
-    // descriptor words: lo = addr >> 4 | (LBO >> 4) << 16, hi = SBO >> 4 | version 1 | SWIZZLE_128B
-    constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
-    constexpr uint32_t kLoKmajor = (16u >> 4) << 16;                    // Q, K: K-major
-    constexpr uint32_t kLoMNmajor = (static_cast<uint32_t>(Cfg::kBoxBytes) >> 4) << 16;   // V: MN-major
-    auto mk_desc = [](uint32_t lo) {
-      return (static_cast<uint64_t>(kDescHi) << 32) | static_cast<uint64_t>(lo);
-    };
-    const uint32_t q_lo = ((q_smem & 0x3FFFFu) >> 4) | kLoKmajor;
-    const uint32_t kv_lo = (kv_smem & 0x3FFFFu) >> 4;
-    for (uint32_t n = 0;; ++n) {
-      const int islot = n & 1;
-      mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
-      const int it_valid = uni(ctrl->items[islot].valid);
-      if (!it_valid) break;
-      const int it_n_keys = uni(ctrl->items[islot].n_keys);
-      const int it_n_rows = uni(ctrl->items[islot].n_rows);
-      const int nt = (it_n_keys + kTileN - 1) / kTileN;
-      const int nsub = (it_n_keys + kSubN - 1) / kSubN;
-      const int ntile = (it_n_rows > kTileM) ? 2 : 1;
-      if (nt > 0) {
-        for (int t = 0; t < ntile; ++t) {
-          mbar_wait(smem_u32(&ctrl->q_full[t]), q_it[t] & 1);
-          ++q_it[t];
-        }
-        tc_fence_after();
-        const uint32_t base = kv_it;   // ring position of K tile 0; K_j at base+2j, V_j at base+2j+1
-        auto slot_of = [&](uint32_t pos) { return pos % Cfg::kStages; };
-        auto phase_of = [&](uint32_t pos) { return (pos / Cfg::kStages) & 1u; };
-        // S_t(sub) = Q_t K[sub]^T into S buffer sub & 1 (lane 0 only)
-        auto issue_qk = [&](int t, int sub) {
-          const uint32_t k_lo = kv_lo + kLoKmajor +
-                                ((slot_of(base + 2 * (sub >> 1)) * Cfg::kTileBytes +
-                                  (sub & 1) * (kSubN * 128)) >> 4);
-          const uint32_t qt_lo = q_lo + ((t * Cfg::kTileBytes) >> 4);
-          const uint32_t ts = tmem_u + t * 128 + (sub & 1) * kSubN;
+    if (elect_one()) {
+      uint32_t kv_pos = 0;                       // ring position of the next item's K tile 0
+      uint32_t q_ph = 0, od_ph = 0, pf_ph = 0;   // phase bits: q_full[t], o_empty[t], p_full[t][buf]
+      // descriptor words: lo = addr >> 4 | (LBO >> 4) << 16, hi = SBO >> 4 | version 1 | SWIZZLE_128B
+      constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
+      constexpr uint32_t kLoKmajor = (16u >> 4) << 16;                                     // Q, K
+      constexpr uint32_t kLoMNmajor = (static_cast<uint32_t>(Cfg::kBoxBytes) >> 4) << 16;  // V
+      auto mk_desc = [](uint32_t lo) {
+        return (static_cast<uint64_t>(kDescHi) << 32) | static_cast<uint64_t>(lo);
+      };
+      const uint32_t q_lo = ((q_smem & 0x3FFFFu) >> 4) | kLoKmajor;
+      const uint32_t kv_lo = (kv_smem & 0x3FFFFu) >> 4;
+      const uint32_t bar_s = smem_u32(&ctrl->s_full[0][0]);    // [t][buf] -> + (2t + buf) * 8
+      const uint32_t bar_p = smem_u32(&ctrl->p_full[0][0]);
+      for (uint32_t n = 0;; ++n) {
+        const int islot = n & 1;
+        mbar_wait<4>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+        if (!ctrl->items[islot].valid) break;
+        const int n_keys = ctrl->items[islot].n_keys;
+        const int nt = (n_keys + kTileN - 1) / kTileN;
+        const int nsub = (n_keys + kSubN - 1) / kSubN;
+        const int ntile = (ctrl->items[islot].n_rows > kTileM) ? 2 : 1;
+        if (nsub > 0) {
 #pragma unroll
-          for (int k = 0; k < D / 16; ++k) {
-            const uint32_t off = ((k >> 2) * Cfg::kBoxBytes + (k & 3) * 32) >> 4;
-            umma_ss(ts, mk_desc(qt_lo + off), mk_desc(k_lo + off), Cfg::kIdescQK, k > 0);
-          }
-          umma_commit(smem_u32(&ctrl->s_full[t][sub & 1]));
-        };
-        // prologue: S(0), S(1)
-        mbar_wait(smem_u32(&ctrl->kv_full[slot_of(base)]), phase_of(base));
-        tc_fence_after();
-        if (elect_one()) {
-          for (int sub = 0; sub < 2 && sub < nsub; ++sub)
-            for (int t = 0; t < ntile; ++t) issue_qk(t, sub);
-          umma_commit(smem_u32(&ctrl->kv_empty[slot_of(base)]));   // K tile 0: both sub-tiles issued
-        }
-        __syncwarp();
-        for (int sub = 0; sub < nsub; ++sub) {
-          const int bufi = sub & 1;
-          const uint32_t vpos = base + 2 * (sub >> 1) + 1;
-          if (bufi == 0) mbar_wait(smem_u32(&ctrl->kv_full[slot_of(vpos)]), phase_of(vpos));
-          const int nxt = sub + 2;                     // S sub-tile issued behind this PV
-          const bool has_next = nxt < nsub;
-          const uint32_t kpos = base + 2 * (nxt >> 1);
-          const int keys_here = min(kSubN, it_n_keys - sub * kSubN);
-          const int ksteps = (keys_here + 15) >> 4;
-          for (int t = 0; t < ntile; ++t) {
-            if (sub == 0) {
-              // the epilogue group must have drained O_t of the previous item
-              mbar_wait(smem_u32(&ctrl->o_empty[t]), (od_it[t] & 1) ^ 1);
-              ++od_it[t];
+          for (int t = 0; t < 2; ++t)
+            if (t < ntile) {
+              mbar_wait<5>(smem_u32(&ctrl->q_full[t]), (q_ph >> t) & 1);
+              q_ph ^= 1u << t;
             }
-            mbar_wait(smem_u32(&ctrl->p_full[t][bufi]), pf_it[t][bufi] & 1);
-            ++pf_it[t][bufi];
+          // S_t(sub) = Q_t K[sub]^T into S buffer sub & 1; k_lo = descriptor word of the K tile
+          auto issue_qk = [&](int t, int sub, uint32_t k_lo) {
+            const uint32_t kk = k_lo + (((sub & 1) * (kSubN * 128)) >> 4);
+            const uint32_t qt_lo = q_lo + ((t * Cfg::kTileBytes) >> 4);
+            const uint32_t ts = tmem_base + t * 128 + (sub & 1) * kSubN;
+#pragma unroll
+            for (int k = 0; k < D / 16; ++k) {
+              const uint32_t off = ((k >> 2) * Cfg::kBoxBytes + (k & 3) * 32) >> 4;
+              umma_ss(ts, mk_desc(qt_lo + off), mk_desc(kk + off), Cfg::kIdescQK, k > 0);
+            }
+            umma_commit(bar_s + (2 * t + (sub & 1)) * 8);
+          };
+          // prologue: S(0), S(1) from K tile 0
+          {
+            const uint32_t slot = kv_pos % Cfg::kStages;
+            mbar_wait<6>(smem_u32(&ctrl->kv_full[slot]), (kv_pos / Cfg::kStages) & 1);
             tc_fence_after();
-            if (elect_one()) {
-              const uint32_t v_lo = kv_lo + kLoMNmajor +
-                                    ((slot_of(vpos) * Cfg::kTileBytes + bufi * (kSubN * 128)) >> 4);
-              const uint32_t tp = tmem_u + t * 128 + bufi * kSubN;
+            const uint32_t k_lo = kv_lo + kLoKmajor + ((slot * Cfg::kTileBytes) >> 4);
+            for (int sub = 0; sub < 2 && sub < nsub; ++sub)
 #pragma unroll
-              for (int k = 0; k < kSubN / 16; ++k) {
-                // A = P_t[:, 16k..16k+16) : 8 TMEM columns of packed bf16 pairs
-                // B = V rows [16k, 16k+16) of the sub-tile: MN-major, 8-row groups 1024 B
-                //     apart, the two 64-column halves (D = 128) one box apart
-                if (k < ksteps)
-                  umma_ts(tm_o[t], tp + k * 8, mk_desc(v_lo + k * (2048 >> 4)), Cfg::kIdescPV,
-                          (sub > 0 || k > 0) ? 1u : 0u);
+              for (int t = 0; t < 2; ++t)
+                if (t < ntile) issue_qk(t, sub, k_lo);
+            umma_commit(smem_u32(&ctrl->kv_empty[slot]));   // K tile 0: both sub-tiles issued
+          }
+          uint32_t vslot = 0, kslot = 0;
+          for (int sub = 0; sub < nsub; ++sub) {
+            const int bufi = sub & 1;
+            if (bufi == 0) {
+              const uint32_t vpos = kv_pos + sub + 1;            // V tile sub/2
+              vslot = vpos % Cfg::kStages;
+              mbar_wait<7>(smem_u32(&ctrl->kv_full[vslot]), (vpos / Cfg::kStages) & 1);
+            }
+            const int nxt = sub + 2;                     // S sub-tile issued behind this PV
+            const bool has_next = nxt < nsub;
+            const int ksteps = (min(kSubN, n_keys - sub * kSubN) + 15) >> 4;
+            const uint32_t v_lo =
+                kv_lo + kLoMNmajor + ((vslot * Cfg::kTileBytes + bufi * (kSubN * 128)) >> 4);
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+              if (t < ntile) {
+                if (sub == 0) {
+                  // the epilogue group must have drained O_t of the previous item
+                  mbar_wait<8>(smem_u32(&ctrl->o_empty[t]), ((od_ph >> t) & 1) ^ 1);
+                  od_ph ^= 1u << t;
+                }
+                mbar_wait<9>(bar_p + (2 * t + bufi) * 8, (pf_ph >> (2 * t + bufi)) & 1);
+                pf_ph ^= 1u << (2 * t + bufi);
+                tc_fence_after();
+                const uint32_t tp = tmem_base + t * 128 + bufi * kSubN;
+                const uint32_t to = tmem_base + 256 + t * D;
+#pragma unroll
+                for (int k = 0; k < kSubN / 16; ++k) {
+                  // A = P_t[:, 16k..16k+16) : 8 TMEM columns of packed bf16 pairs
+                  // B = V rows [16k, 16k+16) of the sub-tile: MN-major, 8-row groups 1024 B
+                  //     apart, the two 64-column halves (D = 128) one box apart
+                  if (k < ksteps)
+                    umma_ts(to, tp + k * 8, mk_desc(v_lo + k * (2048 >> 4)), Cfg::kIdescPV,
+                            (sub > 0 || k > 0) ? 1u : 0u);
+                }
+                umma_commit(smem_u32(&ctrl->pv_done[t]));
+                if (has_next) {
+                  if (t == 0 && (nxt & 1) == 0) {
+                    const uint32_t kpos = kv_pos + nxt;            // K tile nxt/2
+                    kslot = kpos % Cfg::kStages;
+                    mbar_wait<10>(smem_u32(&ctrl->kv_full[kslot]), (kpos / Cfg::kStages) & 1);
+                    tc_fence_after();
+                  }
+                  issue_qk(t, nxt, kv_lo + kLoKmajor + ((kslot * Cfg::kTileBytes) >> 4));
+                } else if (sub == nsub - 1) {
+                  umma_commit(smem_u32(&ctrl->o_full[t]));
+                }
               }
-              umma_commit(smem_u32(&ctrl->pv_done[t]));
             }
-            __syncwarp();
-            if (has_next && t == 0 && (nxt & 1) == 0) {
-              mbar_wait(smem_u32(&ctrl->kv_full[slot_of(kpos)]), phase_of(kpos));
-              tc_fence_after();
-            }
-            if (elect_one()) {
-              if (has_next) issue_qk(t, nxt);
-              else if (sub == nsub - 1) umma_commit(smem_u32(&ctrl->o_full[t]));
-            }
-            __syncwarp();
-          }
-          if (elect_one()) {
             // V tile done after its last sub-tile; K tile done after its last S sub-tile
-            if (bufi == 1 || sub == nsub - 1) umma_commit(smem_u32(&ctrl->kv_empty[slot_of(vpos)]));
+            if (bufi == 1 || sub == nsub - 1) umma_commit(smem_u32(&ctrl->kv_empty[vslot]));
             if (has_next && ((nxt & 1) == 1 || nxt == nsub - 1))
-              umma_commit(smem_u32(&ctrl->kv_empty[slot_of(kpos)]));
+              umma_commit(smem_u32(&ctrl->kv_empty[kslot]));
           }
-          __syncwarp();
+          kv_pos += 2 * nt;
         }
-        kv_it = base + 2 * nt;
+        mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
       }
-      if (elect_one()) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
-      __syncwarp();
     }
+    __syncwarp();
   } else if (warp == kConvWarp0 || warp == kConvWarp0 + 1) {
     // ================================================================= converters
     setmaxnreg_dec<kOtherRegs>();
@@ -599,18 +599,18 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       uint32_t kv_it = 0, raw_it = 0;
       for (uint32_t n = 0;; ++n) {
         const int islot = n & 1;
-        mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+        mbar_wait<11>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
         const WorkItem it = ctrl->items[islot];
         if (!it.valid) break;
         const int nt = (it.n_keys + kTileN - 1) / kTileN;
         for (int jj = 0; jj < 2 * nt; ++jj) {  // K0 V0 K1 V1 ...
           const uint32_t slot = kv_it % Cfg::kStages, ph = (kv_it / Cfg::kStages) & 1;
-          mbar_wait(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
+          mbar_wait<12>(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
           const uint32_t tile = kv_smem + slot * Cfg::kTileBytes;
 #pragma unroll 1
           for (int c = 0; c < Cfg::kRawPerTile; ++c) {
             const uint32_t rslot = raw_it % Cfg::kRawStages, rph = (raw_it / Cfg::kRawStages) & 1;
-            mbar_wait(smem_u32(&ctrl->raw_full[rslot]), rph);
+            mbar_wait<13>(smem_u32(&ctrl->raw_full[rslot]), rph);
             const uint32_t raw = raw_smem + rslot * Cfg::kRawSlotBytes;
             if constexpr (KV == KV_FP8) {
               constexpr int PPR = D / 16;                   // 16-byte pieces per row
@@ -687,7 +687,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
 
     for (uint32_t n = 0;; ++n) {
       const int islot = n & 1;
-      mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+      mbar_wait<14>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
       const WorkItem it = ctrl->items[islot];
       if (!it.valid) break;
       const int rows_here = min(kTileM, it.n_rows - t * kTileM);  // <= 0: tile inactive
@@ -695,7 +695,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       // Prefetch the NEXT item's Q tile as soon as this item's last S_t MMA has read Q_t.
       auto prefetch_next_q = [&]() {
         const uint32_t n1 = n + 1;
-        mbar_wait(smem_u32(&ctrl->item_full[n1 & 1]), (n1 >> 1) & 1);
+        mbar_wait<15>(smem_u32(&ctrl->item_full[n1 & 1]), (n1 >> 1) & 1);
         const WorkItem nx = ctrl->items[n1 & 1];
         if (nx.valid && nx.n_rows > t * kTileM && nx.n_keys > 0) {
           issue_q(nx);
@@ -729,7 +729,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         for (int sub = 0; sub < nsub; ++sub) {
           const int bufi = sub & 1;
           const uint32_t tm_sb = tm_s + bufi * kSubN;
-          mbar_wait(smem_u32(&ctrl->s_full[t][bufi]), sf_it[bufi] & 1);
+          mbar_wait<16>(smem_u32(&ctrl->s_full[t][bufi]), sf_it[bufi] & 1);
           ++sf_it[bufi];
           tc_fence_after();
           if (sub == nsub - 1) prefetch_next_q();   // every S_t MMA of this item is complete
@@ -764,7 +764,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             }
           } else if (__any_sync(0xffffffffu, need)) {
             // PV(sub-1) may still be accumulating into O_t: wait for it before touching O
-            mbar_wait(smem_u32(&ctrl->pv_done[t]), (pv_cnt - 1) & 1);
+            mbar_wait<17>(smem_u32(&ctrl->pv_done[t]), (pv_cnt - 1) & 1);
             tc_fence_after();
             const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
 #pragma unroll
@@ -846,7 +846,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     uint32_t lr_it[2] = {0, 0}, of_it[2] = {0, 0};
     for (uint32_t n = 0;; ++n) {
       const int islot = n & 1;
-      mbar_wait(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
+      mbar_wait<18>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
       const WorkItem it = ctrl->items[islot];
       if (!it.valid) break;
       const int nt = (it.n_keys + kTileN - 1) / kTileN;
@@ -856,10 +856,10 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       for (int t = 0; t < 2; ++t) {
         const int rows_here = min(kTileM, it.n_rows - t * kTileM);
         if (rows_here <= 0) break;
-        mbar_wait(smem_u32(&ctrl->l_ready[t]), lr_it[t] & 1);
+        mbar_wait<19>(smem_u32(&ctrl->l_ready[t]), lr_it[t] & 1);
         ++lr_it[t];
         if (nt > 0) {
-          mbar_wait(smem_u32(&ctrl->o_full[t]), of_it[t] & 1);
+          mbar_wait<20>(smem_u32(&ctrl->o_full[t]), of_it[t] & 1);
           ++of_it[t];
           tc_fence_after();
         }

@@ -33,19 +33,25 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t byt
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
                : "memory");
 }
+// TAG only makes each call site's wait loop a distinct instruction sequence (it is the
+// suspend-time hint, an upper bound in ns on how long the hardware may park the warp), so the
+// assembler cannot merge the loops of different roles and a profile attributes every stall
+// to the barrier it is actually waiting on.
+template <int TAG>
 __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
       "{\n\t.reg .pred P;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 P, [%1], %2;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P, [%1], %2, %3;\n\t"
       "selp.b32 %0, 1, 0, P;\n\t}\n"
       : "=r"(ok)
-      : "r"(bar), "r"(parity)
+      : "r"(bar), "r"(parity), "n"(1000000 + TAG)
       : "memory");
   return ok != 0;
 }
+template <int TAG = 0>
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  while (!mbar_try_wait(bar, parity)) {
+  while (!mbar_try_wait<TAG>(bar, parity)) {
   }
 }
 
