@@ -784,31 +784,35 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           // 32 keys.  The row sum (4 chains) adds the bf16-ROUNDED weights, i.e. exactly
           // what the MMA multiplies, so out = sum(p~ v) / sum(p~) stays a convex combination
           // of V rows (matters when few keys dominate).
-          float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
+          float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
+          const float2 c2 = make_float2(c_log2, c_log2), nm2 = make_float2(-m_used, -m_used);
 #pragma unroll
           for (int c0 = 0; c0 < kSubN; c0 += 32) {
             uint32_t pr[16];
 #pragma unroll
             for (int c = 0; c < 32; c += 4) {
-              const float p0 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 0]), c_log2, -m_used));
-              const float p1 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 1]), c_log2, -m_used));
-              const float p2 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 2]), c_log2, -m_used));
-              const float p3 = ex2_approx(fmaf(__uint_as_float(sr[c0 + c + 3]), c_log2, -m_used));
+              const float2 x01 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 0]),
+                                                   __uint_as_float(sr[c0 + c + 1])), c2, nm2);
+              const float2 x23 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 2]),
+                                                   __uint_as_float(sr[c0 + c + 3])), c2, nm2);
+              const float p0 = ex2_approx(x01.x), p1 = ex2_approx(x01.y);
+              const float p2 = ex2_approx(x23.x), p3 = ex2_approx(x23.y);
               const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
               pr[(c >> 1) + 0] = w01;
               pr[(c >> 1) + 1] = w23;
 #if UPR_CONSISTENT_ROWSUM
-              sum0 += __uint_as_float(w01 << 16);
-              sum1 += __uint_as_float(w01 & 0xffff0000u);
-              sum2 += __uint_as_float(w23 << 16);
-              sum3 += __uint_as_float(w23 & 0xffff0000u);
+              sumA = fadd2(sumA, make_float2(__uint_as_float(w01 << 16),
+                                             __uint_as_float(w01 & 0xffff0000u)));
+              sumB = fadd2(sumB, make_float2(__uint_as_float(w23 << 16),
+                                             __uint_as_float(w23 & 0xffff0000u)));
 #else
-              sum0 += p0; sum1 += p1; sum2 += p2; sum3 += p3;
+              sumA = fadd2(sumA, make_float2(p0, p1));
+              sumB = fadd2(sumB, make_float2(p2, p3));
 #endif
             }
             tmem_st16(tm_sb + (c0 >> 1), pr);
           }
-          l += (sum0 + sum1) + (sum2 + sum3);
+          l += (sumA.x + sumA.y) + (sumB.x + sumB.y);
           tmem_wait_st();
           tc_fence_before();
           mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
@@ -865,7 +869,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         }
         const int row = ew * 32 + lane;                  // row of this thread within the tile
         const float inv = ctrl->epi_inv[islot][t][row];
-        const float wself = ctrl->epi_wself[islot][t][row];
+        const float sc = vs * inv;                                     // out = O * sc + ws * v_self
+        const float ws = ctrl->epi_wself[islot][t][row] * inv;
         const size_t grow0 = static_cast<size_t>(it.layer) * it.total_q + it.q_row0 + t * kTileM;
         // candidate-side element offset of (row 0 of the tile, head h)
         const size_t q_elem0 = (grow0 * args.H + it.h) * D;
@@ -878,7 +883,17 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           dst0 = args.part_o + ((grow0 * args.H + it.h) * args.num_splits + it.split) * D;
           dst_stride = static_cast<size_t>(args.H) * args.num_splits * D;
         }
+        // transposed read-back: 8 lanes cover one row's 128-byte line, 4 rows per access
+        const int rr = lane >> 3, cq = lane & 7;
+        float* gp = dst0 + static_cast<size_t>(ew * 32 + rr) * dst_stride + cq * 4;
+        const size_t gstep = 4 * dst_stride;
+        const int rem = rows_here - (ew * 32 + rr);      // row 4k + rr of this warp valid iff 4k < rem
+        const uint32_t st_w = stage + lane * kEpiRowBytes;
+        const uint32_t st_r = stage + rr * kEpiRowBytes + cq * 16;
+        const bool add_self = self_here && row < rows_here;
+        const size_t se0 = q_elem0 + static_cast<size_t>(row) * args.H * D;
         const uint32_t tm_o = tmem_base + lane_base + 256 + t * D;
+        const float2 sc2 = make_float2(sc, sc);
 #pragma unroll 1
         for (int c0 = 0; c0 < D; c0 += 32) {
           uint32_t orr[32];
@@ -889,51 +904,52 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
 #pragma unroll
             for (int c = 0; c < 32; ++c) orr[c] = 0u;
           }
-          const bool add_self = self_here && row < rows_here;
-          const size_t se = q_elem0 + static_cast<size_t>(row) * args.H * D + c0;
+          if (!self_here) {
 #pragma unroll
-          for (int c = 0; c < 32; c += 8) {
-            float sv[8];
-#pragma unroll
-            for (int k = 0; k < 8; ++k) sv[k] = 0.f;
-            if (add_self) {
-              if (!q32) {
-                const uint4 x = __ldg(reinterpret_cast<const uint4*>(
-                    static_cast<const __nv_bfloat16*>(args.v_self) + se + c));
-                const uint32_t w[4] = {x.x, x.y, x.z, x.w};
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                  sv[2 * k + 0] = __uint_as_float(w[k] << 16);
-                  sv[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
-                }
-              } else {
-                const float4* s4 =
-                    reinterpret_cast<const float4*>(static_cast<const float*>(args.v_self) + se + c);
-                const float4 a = __ldg(s4), b = __ldg(s4 + 1);
-                sv[0] = a.x; sv[1] = a.y; sv[2] = a.z; sv[3] = a.w;
-                sv[4] = b.x; sv[5] = b.y; sv[6] = b.z; sv[7] = b.w;
-              }
+            for (int c = 0; c < 32; c += 4) {
+              const float2 a = fmul2(make_float2(__uint_as_float(orr[c]), __uint_as_float(orr[c + 1])), sc2);
+              const float2 b2 = fmul2(make_float2(__uint_as_float(orr[c + 2]), __uint_as_float(orr[c + 3])), sc2);
+              sts128(st_w + c * 4, __float_as_uint(a.x), __float_as_uint(a.y), __float_as_uint(b2.x),
+                     __float_as_uint(b2.y));
             }
-            float o[8];
+          } else {
 #pragma unroll
-            for (int k = 0; k < 8; ++k)
-              o[k] = fmaf(wself, sv[k], __uint_as_float(orr[c + k]) * vs) * inv;
-            const uint32_t a = stage + lane * kEpiRowBytes + c * 4;
-            sts128(a, __float_as_uint(o[0]), __float_as_uint(o[1]), __float_as_uint(o[2]),
-                   __float_as_uint(o[3]));
-            sts128(a + 16, __float_as_uint(o[4]), __float_as_uint(o[5]), __float_as_uint(o[6]),
-                   __float_as_uint(o[7]));
+            for (int c = 0; c < 32; c += 8) {
+              float sv[8];
+#pragma unroll
+              for (int k = 0; k < 8; ++k) sv[k] = 0.f;
+              if (add_self) {
+                if (!q32) {
+                  const uint4 x = __ldg(reinterpret_cast<const uint4*>(
+                      static_cast<const __nv_bfloat16*>(args.v_self) + se0 + c0 + c));
+                  const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                  for (int k = 0; k < 4; ++k) {
+                    sv[2 * k + 0] = __uint_as_float(w[k] << 16);
+                    sv[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+                  }
+                } else {
+                  const float4* s4 = reinterpret_cast<const float4*>(
+                      static_cast<const float*>(args.v_self) + se0 + c0 + c);
+                  const float4 a = __ldg(s4), b4 = __ldg(s4 + 1);
+                  sv[0] = a.x; sv[1] = a.y; sv[2] = a.z; sv[3] = a.w;
+                  sv[4] = b4.x; sv[5] = b4.y; sv[6] = b4.z; sv[7] = b4.w;
+                }
+              }
+              float o[8];
+#pragma unroll
+              for (int k = 0; k < 8; ++k) o[k] = fmaf(ws, sv[k], __uint_as_float(orr[c + k]) * sc);
+              sts128(st_w + c * 4, __float_as_uint(o[0]), __float_as_uint(o[1]), __float_as_uint(o[2]),
+                     __float_as_uint(o[3]));
+              sts128(st_w + c * 4 + 16, __float_as_uint(o[4]), __float_as_uint(o[5]),
+                     __float_as_uint(o[6]), __float_as_uint(o[7]));
+            }
           }
           __syncwarp();
-          // transposed read-back: 8 lanes cover one row's 128-byte line, 4 rows per access
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
-            const int r = 4 * k + (lane >> 3);
-            const uint4 v = lds128(stage + r * kEpiRowBytes + (lane & 7) * 16);
-            const int trow = ew * 32 + r;
-            if (trow < rows_here)
-              *reinterpret_cast<uint4*>(dst0 + static_cast<size_t>(trow) * dst_stride + c0 +
-                                        (lane & 7) * 4) = v;
+            const uint4 v = lds128(st_r + k * (4 * kEpiRowBytes));
+            if (4 * k < rem) *reinterpret_cast<uint4*>(gp + k * gstep + c0) = v;
           }
           __syncwarp();
         }
