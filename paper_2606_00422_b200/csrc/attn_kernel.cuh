@@ -33,6 +33,12 @@
 
 #include "ptx.cuh"
 
+#ifndef UPR_DIAG
+#define UPR_DIAG 0   // timing experiments only: 1 = softmax math skipped, 2 = MMAs skipped
+#endif
+#ifndef UPR_PINGPONG
+#define UPR_PINGPONG 1
+#endif
 #ifndef UPR_CONSISTENT_ROWSUM
 #define UPR_CONSISTENT_ROWSUM 1
 #endif
@@ -41,13 +47,22 @@ namespace upr {
 
 constexpr int kTileM = 128;     // candidate rows per MMA tile == TMEM lanes
 constexpr int kTileN = 128;     // keys per K/V smem tile
-constexpr int kSubN = 64;       // keys per softmax / MMA step (two S buffers per candidate tile)
+#ifndef UPR_NB
+#define UPR_NB 2
+#endif
+constexpr int kNB = UPR_NB;        // S buffers per candidate tile (1 or 2)
+constexpr int kSubN = kTileN / kNB;   // keys per softmax / MMA step: S(s + kNB) is issued behind PV(s)
 constexpr int kQBlock = 256;    // candidate rows per work item (two tiles)
 constexpr int kRowAlign = 16;   // UPR_ROW_ALIGN
 constexpr int kAttnThreads = 512;     // 2 softmax warpgroups + {TMA, MMA, 2 converters} + epilogue
-constexpr int kSoftmaxRegs = 168;     // setmaxnreg budgets (sum over 512 threads <= 64 K registers)
-constexpr int kOtherRegs = 56;        //   producer / MMA / converter warpgroup
-constexpr int kEpilogueRegs = 88;     //   epilogue warpgroup
+// setmaxnreg budgets.  The pool is what the CTA was given at launch (512 threads x 128
+// registers), not the whole register file: an .inc beyond it blocks forever.
+constexpr int kLaunchRegs = 128;
+constexpr int kSoftmaxRegs = (UPR_NB == 1) ? 200 : 168;   //   2 softmax warpgroups
+constexpr int kOtherRegs = (UPR_NB == 1) ? 48 : 56;       //   producer / MMA / converter warpgroup
+constexpr int kEpilogueRegs = (UPR_NB == 1) ? 64 : 88;    //   epilogue warpgroup
+static_assert(256 * kSoftmaxRegs + 128 * kOtherRegs + 128 * kEpilogueRegs <= kAttnThreads * kLaunchRegs,
+              "setmaxnreg budgets exceed the CTA's register allocation");
 constexpr int kProducerWarp = 8;
 constexpr int kMmaWarp = 9;
 constexpr int kConvWarp0 = 10;        // warps 10, 11
@@ -58,6 +73,26 @@ constexpr float kRescaleTau = 8.0f;  // lazy-rescale threshold, log2 units
 constexpr int kEpiRowBytes = 144;     // 32 floats + 16 B pad: conflict-free 16-byte accesses
 
 enum : int { KV_BF16 = 0, KV_FP8 = 1, KV_F32 = 2 };
+
+// Timeline tracing for experiments (-DUPR_TRACE=1 builds only; never in the product library):
+// CTA 0 records (event id, clock64) pairs into a device array read back by upr_debug_trace.
+#ifndef UPR_TRACE
+#define UPR_TRACE 0
+#endif
+#if UPR_TRACE
+__device__ unsigned long long g_trace[16][2048];
+__device__ __forceinline__ void trace(int role, uint32_t& cnt, int ev) {
+  if (blockIdx.x == 0 && cnt < 2047) {
+    g_trace[role][1 + cnt] = (static_cast<unsigned long long>(ev) << 48) |
+                             (static_cast<unsigned long long>(clock64()) & 0xFFFFFFFFFFFFull);
+    ++cnt;
+    g_trace[role][0] = cnt;
+  }
+}
+#define UPR_TR(role, cnt, ev) trace(role, cnt, ev)
+#else
+#define UPR_TR(role, cnt, ev)
+#endif
 
 struct AttnArgs {
   const void* q;
@@ -481,6 +516,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     if (elect_one()) {
       uint32_t kv_pos = 0;                       // ring position of the next item's K tile 0
       uint32_t q_ph = 0, od_ph = 0, pf_ph = 0;   // phase bits: q_full[t], o_empty[t], p_full[t][buf]
+      uint32_t trc = 0; (void)trc;
       // descriptor words: lo = addr >> 4 | (LBO >> 4) << 16, hi = SBO >> 4 | version 1 | SWIZZLE_128B
       constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
       constexpr uint32_t kLoKmajor = (16u >> 4) << 16;                                     // Q, K
@@ -496,6 +532,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         const int islot = n & 1;
         mbar_wait<4>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
         if (!ctrl->items[islot].valid) break;
+        UPR_TR(2, trc, 1);   // item acquired
         const int n_keys = ctrl->items[islot].n_keys;
         const int nt = (n_keys + kTileN - 1) / kTileN;
         const int nsub = (n_keys + kSubN - 1) / kSubN;
@@ -504,20 +541,22 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
 #pragma unroll
           for (int t = 0; t < 2; ++t)
             if (t < ntile) {
+#if UPR_DIAG != 6
               mbar_wait<5>(smem_u32(&ctrl->q_full[t]), (q_ph >> t) & 1);
+#endif
               q_ph ^= 1u << t;
             }
           // S_t(sub) = Q_t K[sub]^T into S buffer sub & 1; k_lo = descriptor word of the K tile
           auto issue_qk = [&](int t, int sub, uint32_t k_lo) {
-            const uint32_t kk = k_lo + (((sub & 1) * (kSubN * 128)) >> 4);
+            const uint32_t kk = k_lo + (((sub % kNB) * (kSubN * 128)) >> 4);
             const uint32_t qt_lo = q_lo + ((t * Cfg::kTileBytes) >> 4);
-            const uint32_t ts = tmem_base + t * 128 + (sub & 1) * kSubN;
+            const uint32_t ts = tmem_base + t * 128 + (sub % kNB) * kSubN;
 #pragma unroll
             for (int k = 0; k < D / 16; ++k) {
               const uint32_t off = ((k >> 2) * Cfg::kBoxBytes + (k & 3) * 32) >> 4;
               umma_ss(ts, mk_desc(qt_lo + off), mk_desc(kk + off), Cfg::kIdescQK, k > 0);
             }
-            umma_commit(bar_s + (2 * t + (sub & 1)) * 8);
+            umma_commit(bar_s + (2 * t + (sub % kNB)) * 8);
           };
           // prologue: S(0), S(1) from K tile 0
           {
@@ -525,21 +564,22 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             mbar_wait<6>(smem_u32(&ctrl->kv_full[slot]), (kv_pos / Cfg::kStages) & 1);
             tc_fence_after();
             const uint32_t k_lo = kv_lo + kLoKmajor + ((slot * Cfg::kTileBytes) >> 4);
-            for (int sub = 0; sub < 2 && sub < nsub; ++sub)
+            for (int sub = 0; sub < kNB && sub < nsub; ++sub)
 #pragma unroll
               for (int t = 0; t < 2; ++t)
                 if (t < ntile) issue_qk(t, sub, k_lo);
             umma_commit(smem_u32(&ctrl->kv_empty[slot]));   // K tile 0: both sub-tiles issued
+            UPR_TR(2, trc, 3);   // prologue issued
           }
           uint32_t vslot = 0, kslot = 0;
           for (int sub = 0; sub < nsub; ++sub) {
-            const int bufi = sub & 1;
+            const int bufi = sub % kNB;
             if (bufi == 0) {
-              const uint32_t vpos = kv_pos + sub + 1;            // V tile sub/2
+              const uint32_t vpos = kv_pos + 2 * (sub / kNB) + 1;   // V tile sub / kNB
               vslot = vpos % Cfg::kStages;
               mbar_wait<7>(smem_u32(&ctrl->kv_full[vslot]), (vpos / Cfg::kStages) & 1);
             }
-            const int nxt = sub + 2;                     // S sub-tile issued behind this PV
+            const int nxt = sub + kNB;                   // S sub-tile issued behind this PV
             const bool has_next = nxt < nsub;
             const int ksteps = (min(kSubN, n_keys - sub * kSubN) + 15) >> 4;
             const uint32_t v_lo =
@@ -549,12 +589,16 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               if (t < ntile) {
                 if (sub == 0) {
                   // the epilogue group must have drained O_t of the previous item
+#if UPR_DIAG != 5
                   mbar_wait<8>(smem_u32(&ctrl->o_empty[t]), ((od_ph >> t) & 1) ^ 1);
+#endif
                   od_ph ^= 1u << t;
+                  UPR_TR(2, trc, 4 + t);   // o_empty acquired
                 }
                 mbar_wait<9>(bar_p + (2 * t + bufi) * 8, (pf_ph >> (2 * t + bufi)) & 1);
                 pf_ph ^= 1u << (2 * t + bufi);
                 tc_fence_after();
+                UPR_TR(2, trc, 10 + t);   // p_full acquired
                 const uint32_t tp = tmem_base + t * 128 + bufi * kSubN;
                 const uint32_t to = tmem_base + 256 + t * D;
 #pragma unroll
@@ -568,8 +612,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
                 }
                 umma_commit(smem_u32(&ctrl->pv_done[t]));
                 if (has_next) {
-                  if (t == 0 && (nxt & 1) == 0) {
-                    const uint32_t kpos = kv_pos + nxt;            // K tile nxt/2
+                  if (t == 0 && (nxt % kNB) == 0) {
+                    const uint32_t kpos = kv_pos + 2 * (nxt / kNB);   // K tile nxt / kNB
                     kslot = kpos % Cfg::kStages;
                     mbar_wait<10>(smem_u32(&ctrl->kv_full[kslot]), (kpos / Cfg::kStages) & 1);
                     tc_fence_after();
@@ -581,12 +625,13 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               }
             }
             // V tile done after its last sub-tile; K tile done after its last S sub-tile
-            if (bufi == 1 || sub == nsub - 1) umma_commit(smem_u32(&ctrl->kv_empty[vslot]));
-            if (has_next && ((nxt & 1) == 1 || nxt == nsub - 1))
+            if (bufi == kNB - 1 || sub == nsub - 1) umma_commit(smem_u32(&ctrl->kv_empty[vslot]));
+            if (has_next && ((nxt % kNB) == kNB - 1 || nxt == nsub - 1))
               umma_commit(smem_u32(&ctrl->kv_empty[kslot]));
           }
           kv_pos += 2 * nt;
         }
+        UPR_TR(2, trc, 9);   // item issued
         mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
       }
     }
@@ -668,6 +713,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     const uint32_t q_tile_smem = q_smem + t * Cfg::kTileBytes;
     uint32_t sf_it[2] = {0, 0};              // s_full phase counters per S buffer
     uint32_t pv_cnt = 0;                     // PV sub-tile MMAs of this tile issued so far (all items)
+    uint32_t trc = 0; (void)trc;
+    const bool tr_on = (tid128 == 0); (void)tr_on;
     const bool has_self = (args.k_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
     const size_t row_stride = static_cast<size_t>(args.H) * D;
@@ -690,6 +737,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       mbar_wait<14>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
       const WorkItem it = ctrl->items[islot];
       if (!it.valid) break;
+      if (tr_on) UPR_TR(t, trc, 1);   // item acquired
       const int rows_here = min(kTileM, it.n_rows - t * kTileM);  // <= 0: tile inactive
       const int nsub = (rows_here > 0) ? (it.n_keys + kSubN - 1) / kSubN : 0;
       // Prefetch the NEXT item's Q tile as soon as this item's last S_t MMA has read Q_t.
@@ -710,6 +758,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           cp_async_wait_all();
           fence_proxy_async_smem();
           mbar_arrive(smem_u32(&ctrl->q_full[t]));
+          if (tr_on) UPR_TR(t, trc, 4);   // q_full arrived
           q_prefetched = false;
         }
         const int sidx = it.layer * args.H + it.h;
@@ -726,16 +775,30 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           l = 1.f;
         }
 
+        // exp-phase ping-pong between the two groups (both tiles active): a warp's step is a
+        // latency-bound part (barrier, TMEM load, row max) and a MUFU-bound part (64 ex2 at
+        // 8 cycles each per SMSP).  The two softmax warps of an SMSP drift into lockstep
+        // unless forced apart, and then nothing hides either part; handing the MUFU phase
+        // back and forth keeps them in anti-phase.  Barrier 1 = "group 0 may go", 2 = "group 1".
+        const bool pingpong = UPR_PINGPONG && (it.n_rows > kTileM) && nsub > 0;
+        if (pingpong && t == 1) named_bar_arrive(1, 256);
+
         for (int sub = 0; sub < nsub; ++sub) {
-          const int bufi = sub & 1;
+          const int bufi = sub % kNB;
           const uint32_t tm_sb = tm_s + bufi * kSubN;
           mbar_wait<16>(smem_u32(&ctrl->s_full[t][bufi]), sf_it[bufi] & 1);
           ++sf_it[bufi];
           tc_fence_after();
+          if (tr_on) UPR_TR(t, trc, 2);   // s_full acquired
           if (sub == nsub - 1) prefetch_next_q();   // every S_t MMA of this item is complete
+#if UPR_DIAG == 1 || UPR_DIAG == 3 || UPR_DIAG == 4
+          mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
+          ++pv_cnt;
+          continue;
+#endif
           uint32_t sr[kSubN];
-          tmem_ld32(tm_sb + 0, &sr[0]);
-          tmem_ld32(tm_sb + 32, &sr[32]);
+#pragma unroll
+          for (int c0 = 0; c0 < kSubN; c0 += 32) tmem_ld32(tm_sb + c0, &sr[c0]);
           tmem_wait_ld_regs(sr);
           const int keys_here = it.n_keys - sub * kSubN;  // may exceed 64
           if (keys_here < kSubN) {
@@ -784,6 +847,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           // 32 keys.  The row sum (4 chains) adds the bf16-ROUNDED weights, i.e. exactly
           // what the MMA multiplies, so out = sum(p~ v) / sum(p~) stays a convex combination
           // of V rows (matters when few keys dominate).
+          if (pingpong) named_bar_sync(1 + t, 256);
           float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
           const float2 c2 = make_float2(c_log2, c_log2), nm2 = make_float2(-m_used, -m_used);
 #pragma unroll
@@ -812,10 +876,12 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             }
             tmem_st16(tm_sb + (c0 >> 1), pr);
           }
+          if (pingpong && !(t == 1 && sub == nsub - 1)) named_bar_arrive(2 - t, 256);
           l += (sumA.x + sumA.y) + (sumB.x + sumB.y);
           tmem_wait_st();
           tc_fence_before();
           mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
+          if (tr_on) UPR_TR(t, trc, 3);   // p_full arrived
           ++pv_cnt;
         }
         if (nsub == 0) prefetch_next_q();

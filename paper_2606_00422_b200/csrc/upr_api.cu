@@ -247,6 +247,13 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
 // ================================================================================= C ABI
 extern "C" {
 
+#if UPR_TRACE
+// experiments only: copy the timeline of CTA 0 to the host (16 x 2048 u64)
+int upr_debug_trace(unsigned long long* host) {
+  return (int)cudaMemcpyFromSymbol(host, upr::g_trace, sizeof(unsigned long long) * 16 * 2048);
+}
+#endif
+
 const char* upr_last_error(void) { return g_err; }
 const char* upr_version(void) { return "upr 0.1 sm_100a"; }
 int upr_last_launch_count(void) { return g_launches; }
