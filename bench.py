@@ -308,13 +308,19 @@ def run_ours(args):
     roof_ms = 1e3 * max(t_flop, t_mem)
     roofline = {"bound": "tensor" if t_flop >= t_mem else "hbm", "kernel": "upr_attn_fwd_kernel",
                 "achieved": tflops, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
-                "frac": tflops / peaks["bf16_tflops"], "traffic": None,
+                "frac": tflops / peaks["bf16_tflops"],
+                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the ncu --set full
+                # capture summarised in profiles/r1h_attn_cfg3.md (config 3 only)
+                "traffic": (6.383e9 + 2.164e9) if w.cfg == 3 and world == 1 else None,
+                "traffic_algorithmic": w.kv_bytes + 6 * w.total_q * w.H * w.d * w.n_layers,
                 "peak_source": peaks["source"] + " (burst cuBLAS bf16)",
                 "frac_of_sustained": tflops / peaks["bf16_tflops_sustained"],
                 "kernel_ms": attn_ms, "roofline_ms": roof_ms, "frac_of_roofline_time": roof_ms / attn_ms,
                 "flops_per_launch": flops, "kv_bytes_per_launch": w.kv_bytes,
                 "kv_gbs": w.kv_bytes / (attn_ms * 1e-3) / 1e9}
-    pack_bytes = 2 * w.kv_bytes  # read pool rows + write cache rows (bf16)
+    # pack: read the valid pool rows (bf16) + write the cache rows; FP8 reads the pool twice (amax, quantise)
+    pool_bytes = int(w.seq_lens.astype(np.int64).sum()) * w.H * w.d * w.n_layers * 2 * 2
+    pack_bytes = pool_bytes * (2 if w.kv_dtype == "fp8" else 1) + w.kv_bytes
     extra = {"pack_ms": pack_ms, "attn_ms": attn_ms, "pack_gbs": pack_bytes / (pack_ms * 1e-3) / 1e9,
              "attn_candidates_per_s": w.total_q / (attn_ms * 1e-3), "splits": attn.splits}
 
