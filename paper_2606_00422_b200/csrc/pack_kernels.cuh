@@ -65,7 +65,10 @@ struct PackArgs {
 };
 
 // MODE 0: bf16 copy, 1: fp8 quantise, 2: fp32 widen, 3: amax pass (no cache write)
-template <int MODE>
+// Each warp owns a CONTIGUOUS range of 16-row blocks (it streams a contiguous piece of the
+// cache; the amax pass then needs one atomic per (layer, head) change instead of one per
+// block) and keeps U blocks' worth of 16-byte loads in flight before it converts and stores.
+template <int MODE, int D>
 __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a) {
   extern __shared__ int row_off[];  // [B+1]
   build_row_off(a.seq_lens, a.B, row_off);
@@ -73,80 +76,127 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
   const int blocks_per_head = R / kPackRowBlock;
   const long long n_blocks = static_cast<long long>(a.n_layers) * a.H * blocks_per_head;
   const int lane = threadIdx.x & 31;
-  const int warps_per_cta = kPackThreads / 32;
-  const long long warp0 = static_cast<long long>(blockIdx.x) * warps_per_cta + (threadIdx.x >> 5);
-  const long long warp_stride = static_cast<long long>(gridDim.x) * warps_per_cta;
-  const int chunks_per_row = a.d / 8;                    // 16-byte bf16 chunks
-  const int chunks = kPackRowBlock * chunks_per_row;     // per 16-row block: 128 (d=64) / 256
+  constexpr int kWarpsPerCta = kPackThreads / 32;
+  const long long n_warps = static_cast<long long>(gridDim.x) * kWarpsPerCta;
+  const long long wid = static_cast<long long>(blockIdx.x) * kWarpsPerCta + (threadIdx.x >> 5);
+  const long long per = (n_blocks + n_warps - 1) / n_warps;
+  const long long blk0 = wid * per;
+  const long long blk1 = (blk0 + per < n_blocks) ? (blk0 + per) : n_blocks;
+  constexpr int CPR = D / 8;                       // 16-byte bf16 chunks per row
+  constexpr int CH = kPackRowBlock * CPR;          // chunks per 16-row block: 128 (d=64) / 256
+  constexpr int NI = CH / 32;                      // chunks per lane per block
+  constexpr int U = (D == 64) ? 4 : 2;             // blocks in flight per warp
 
-  for (long long blk = warp0; blk < n_blocks; blk += warp_stride) {
-    const int rb = static_cast<int>(blk % blocks_per_head);
-    const long long lh = blk / blocks_per_head;
-    const int h = static_cast<int>(lh % a.H), l = static_cast<int>(lh / a.H);
-    const int row = rb * kPackRowBlock;
-    const int b = find_user(row_off, a.B, row);
-    const int j0 = row - row_off[b];                     // first key index of this block
-    const int valid_rows = max(0, min(kPackRowBlock, __ldg(a.seq_lens + b) - j0));
-    const int slot = __ldg(a.slot_ids + b);
-    const __nv_bfloat16* src =
-        a.pool + ((((static_cast<size_t>(l) * a.S + slot) * a.H + h) * a.n_max) + j0) * a.d;
-    const size_t dst_elem = ((static_cast<size_t>(l) * a.H + h) * R + row) * a.d;
-    const int valid_chunks = valid_rows * chunks_per_row;
-    float mult = 1.0f;
-    if (MODE == 1) {
-      const float amax = a.scale[l * a.H + h];
-      mult = amax > 0.f ? __fdiv_rn(448.0f, amax) : 1.0f;
-    }
-    float wmax = 0.f;
-    for (int c = lane; c < chunks; c += 32) {
-      uint4 v = make_uint4(0u, 0u, 0u, 0u);
-      if (c < valid_chunks) v = __ldg(reinterpret_cast<const uint4*>(src) + c);
-      const __nv_bfloat162* p2 = reinterpret_cast<const __nv_bfloat162*>(&v);
-      if (MODE == 0) {
-        reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(a.cache) + dst_elem)[c] = v;
-      } else if (MODE == 1) {
-        uint32_t w[2];
+  int cur_lh = -1;        // amax pass: (layer, head) of the running maximum
+  float run_max = 0.f;
+  for (long long blk = blk0; blk < blk1; blk += U) {
+    uint4 v[U][NI];
+    size_t dst_elem[U];
+    int lh_u[U];
+    float mult[U];
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {
-          float2 f0 = __bfloat1622float2(p2[2 * k]), f1 = __bfloat1622float2(p2[2 * k + 1]);
-          uint16_t lo16 = __nv_cvt_float2_to_fp8x2(make_float2(__fmul_rn(f0.x, mult), __fmul_rn(f0.y, mult)),
-                                                   __NV_SATFINITE, __NV_E4M3);
-          uint16_t hi16 = __nv_cvt_float2_to_fp8x2(make_float2(__fmul_rn(f1.x, mult), __fmul_rn(f1.y, mult)),
-                                                   __NV_SATFINITE, __NV_E4M3);
-          w[k] = static_cast<uint32_t>(lo16) | (static_cast<uint32_t>(hi16) << 16);
+    for (int u = 0; u < U; ++u) {
+      const long long bk = blk + u;
+      lh_u[u] = -1;
+      dst_elem[u] = 0;
+      mult[u] = 1.0f;
+#pragma unroll
+      for (int i = 0; i < NI; ++i) v[u][i] = make_uint4(0u, 0u, 0u, 0u);
+      if (bk < blk1) {
+        const int rb = static_cast<int>(bk % blocks_per_head);
+        const int lh = static_cast<int>(bk / blocks_per_head);
+        const int h = lh % a.H, l = lh / a.H;
+        const int row = rb * kPackRowBlock;
+        const int b = find_user(row_off, a.B, row);
+        const int j0 = row - row_off[b];                     // first key index of this block
+        const int valid_rows = max(0, min(kPackRowBlock, __ldg(a.seq_lens + b) - j0));
+        const int slot = __ldg(a.slot_ids + b);
+        const __nv_bfloat16* src =
+            a.pool + ((((static_cast<size_t>(l) * a.S + slot) * a.H + h) * a.n_max) + j0) * D;
+        lh_u[u] = lh;
+        dst_elem[u] = (static_cast<size_t>(lh) * R + row) * D;
+        const int valid_chunks = valid_rows * CPR;
+        if (MODE == 1) {
+          const float amax = a.scale[lh];
+          mult[u] = amax > 0.f ? __fdiv_rn(448.0f, amax) : 1.0f;
         }
-        reinterpret_cast<uint2*>(static_cast<uint8_t*>(a.cache) + dst_elem)[c] = make_uint2(w[0], w[1]);
-      } else if (MODE == 2) {
-        float4 o0, o1;
-        float2 f;
-        f = __bfloat1622float2(p2[0]); o0.x = f.x; o0.y = f.y;
-        f = __bfloat1622float2(p2[1]); o0.z = f.x; o0.w = f.y;
-        f = __bfloat1622float2(p2[2]); o1.x = f.x; o1.y = f.y;
-        f = __bfloat1622float2(p2[3]); o1.z = f.x; o1.w = f.y;
-        float4* dp = reinterpret_cast<float4*>(static_cast<float*>(a.cache) + dst_elem) + 2 * c;
-        dp[0] = o0;
-        dp[1] = o1;
-      } else {
 #pragma unroll
-        for (int k = 0; k < 4; ++k) {
-          float2 f = __bfloat1622float2(p2[k]);
-          wmax = fmaxf(wmax, fmaxf(fabsf(f.x), fabsf(f.y)));
+        for (int i = 0; i < NI; ++i) {
+          const int c = i * 32 + lane;
+          if (c < valid_chunks) v[u][i] = __ldg(reinterpret_cast<const uint4*>(src) + c);
         }
       }
     }
-    if (MODE == 3) {
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) wmax = fmaxf(wmax, __shfl_xor_sync(0xffffffffu, wmax, o));
-      // non-negative floats order like their bit patterns
-      if (lane == 0 && wmax > 0.f)
-        atomicMax(reinterpret_cast<unsigned int*>(a.scale + l * a.H + h), __float_as_uint(wmax));
+    for (int u = 0; u < U; ++u) {
+      if (lh_u[u] < 0) continue;
+      if (MODE == 3) {
+        float wmax = 0.f;
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+          const __nv_bfloat162* p2 = reinterpret_cast<const __nv_bfloat162*>(&v[u][i]);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) {
+            const float2 f = __bfloat1622float2(p2[k]);
+            wmax = fmaxf(wmax, fmaxf(fabsf(f.x), fabsf(f.y)));
+          }
+        }
+        if (lh_u[u] != cur_lh) {
+          // flush the finished (layer, head): non-negative floats order like their bit patterns
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) run_max = fmaxf(run_max, __shfl_xor_sync(0xffffffffu, run_max, o));
+          if (lane == 0 && cur_lh >= 0 && run_max > 0.f)
+            atomicMax(reinterpret_cast<unsigned int*>(a.scale + cur_lh), __float_as_uint(run_max));
+          cur_lh = lh_u[u];
+          run_max = 0.f;
+        }
+        run_max = fmaxf(run_max, wmax);
+        continue;
+      }
+#pragma unroll
+      for (int i = 0; i < NI; ++i) {
+        const int c = i * 32 + lane;
+        const uint4 x = v[u][i];
+        const __nv_bfloat162* p2 = reinterpret_cast<const __nv_bfloat162*>(&x);
+        if (MODE == 0) {
+          reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(a.cache) + dst_elem[u])[c] = x;
+        } else if (MODE == 1) {
+          uint32_t w[2];
+#pragma unroll
+          for (int k = 0; k < 2; ++k) {
+            const float2 f0 = __bfloat1622float2(p2[2 * k]), f1 = __bfloat1622float2(p2[2 * k + 1]);
+            const uint16_t lo16 = __nv_cvt_float2_to_fp8x2(
+                make_float2(__fmul_rn(f0.x, mult[u]), __fmul_rn(f0.y, mult[u])), __NV_SATFINITE, __NV_E4M3);
+            const uint16_t hi16 = __nv_cvt_float2_to_fp8x2(
+                make_float2(__fmul_rn(f1.x, mult[u]), __fmul_rn(f1.y, mult[u])), __NV_SATFINITE, __NV_E4M3);
+            w[k] = static_cast<uint32_t>(lo16) | (static_cast<uint32_t>(hi16) << 16);
+          }
+          reinterpret_cast<uint2*>(static_cast<uint8_t*>(a.cache) + dst_elem[u])[c] = make_uint2(w[0], w[1]);
+        } else {
+          float4 o0, o1;
+          float2 f;
+          f = __bfloat1622float2(p2[0]); o0.x = f.x; o0.y = f.y;
+          f = __bfloat1622float2(p2[1]); o0.z = f.x; o0.w = f.y;
+          f = __bfloat1622float2(p2[2]); o1.x = f.x; o1.y = f.y;
+          f = __bfloat1622float2(p2[3]); o1.z = f.x; o1.w = f.y;
+          float4* dp = reinterpret_cast<float4*>(static_cast<float*>(a.cache) + dst_elem[u]) + 2 * c;
+          dp[0] = o0;
+          dp[1] = o1;
+        }
+      }
     }
+  }
+  if (MODE == 3) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) run_max = fmaxf(run_max, __shfl_xor_sync(0xffffffffu, run_max, o));
+    if (lane == 0 && cur_lh >= 0 && run_max > 0.f)
+      atomicMax(reinterpret_cast<unsigned int*>(a.scale + cur_lh), __float_as_uint(run_max));
   }
   if (MODE != 3) {
     // zero the tail rows after the last (layer, head) block
-    const size_t tail0 = static_cast<size_t>(a.n_layers) * a.H * R * a.d;  // element index
+    const size_t tail0 = static_cast<size_t>(a.n_layers) * a.H * R * D;  // element index
     const size_t eb = (MODE == 0) ? 2 : (MODE == 1) ? 1 : 4;
-    const size_t n16 = static_cast<size_t>(a.tail_rows) * a.d * eb / 16;
+    const size_t n16 = static_cast<size_t>(a.tail_rows) * D * eb / 16;
     uint4* tp = reinterpret_cast<uint4*>(static_cast<uint8_t*>(a.cache) + tail0 * eb);
     for (size_t i = static_cast<size_t>(blockIdx.x) * blockDim.x + threadIdx.x; i < n16;
          i += static_cast<size_t>(gridDim.x) * blockDim.x)

@@ -332,19 +332,26 @@ upr_status upr_kv_pack(const void* k_pool, const void* v_pool, int S, int n_max,
     a.S = S;
     a.n_max = n_max;
     a.tail_rows = lay->tail_rows;
+    const bool d64 = lay->d == 64;
+#define UPR_PACK_LAUNCH(MODE)                                                              \
+  do {                                                                                     \
+    if (d64) upr::upr_pack_kernel<MODE, 64><<<grid, upr::kPackThreads, smem, st>>>(a);     \
+    else upr::upr_pack_kernel<MODE, 128><<<grid, upr::kPackThreads, smem, st>>>(a);        \
+  } while (0)
     if (lay->dtype == UPR_BF16) {
-      upr::upr_pack_kernel<0><<<grid, upr::kPackThreads, smem, st>>>(a);
+      UPR_PACK_LAUNCH(0);
       g_launches += 1;
     } else if (lay->dtype == UPR_F32) {
-      upr::upr_pack_kernel<2><<<grid, upr::kPackThreads, smem, st>>>(a);
+      UPR_PACK_LAUNCH(2);
       g_launches += 1;
     } else {
       UPR_CUDA_CHECK(cudaMemsetAsync(a.scale, 0, n_scale * sizeof(float), st));
-      upr::upr_pack_kernel<3><<<grid, upr::kPackThreads, smem, st>>>(a);
-      upr::upr_pack_kernel<1><<<grid, upr::kPackThreads, smem, st>>>(a);
+      UPR_PACK_LAUNCH(3);
+      UPR_PACK_LAUNCH(1);
       upr::upr_scale_finalize_kernel<<<(n_scale + 127) / 128, 128, 0, st>>>(a.scale, n_scale);
       g_launches += 3;
     }
+#undef UPR_PACK_LAUNCH
     UPR_CUDA_CHECK(cudaGetLastError());
   }
   return UPR_OK;
