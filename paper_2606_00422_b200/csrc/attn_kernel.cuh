@@ -348,15 +348,15 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       mbar_init(smem_u32(&ctrl->raw_empty[i]), kConvThreads);
     }
     for (int t = 0; t < 2; ++t) {
-      mbar_init(smem_u32(&ctrl->q_full[t]), 128);
+      mbar_init(smem_u32(&ctrl->q_full[t]), 4);       // one arrival per softmax warp
       for (int bf = 0; bf < 2; ++bf) {
         mbar_init(smem_u32(&ctrl->s_full[t][bf]), 1);
-        mbar_init(smem_u32(&ctrl->p_full[t][bf]), 128);
+        mbar_init(smem_u32(&ctrl->p_full[t][bf]), 4);
       }
       mbar_init(smem_u32(&ctrl->pv_done[t]), 1);
       mbar_init(smem_u32(&ctrl->o_full[t]), 1);
       mbar_init(smem_u32(&ctrl->o_empty[t]), 4);
-      mbar_init(smem_u32(&ctrl->l_ready[t]), 128);
+      mbar_init(smem_u32(&ctrl->l_ready[t]), 4);
       mbar_init(smem_u32(&ctrl->item_full[t]), 1);
       mbar_init(smem_u32(&ctrl->item_empty[t]), kItemReaders);
     }
@@ -757,7 +757,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           if (!q_prefetched) issue_q(it);
           cp_async_wait_all();
           fence_proxy_async_smem();
-          mbar_arrive(smem_u32(&ctrl->q_full[t]));
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&ctrl->q_full[t]));
           if (tr_on) UPR_TR(t, trc, 4);   // q_full arrived
           q_prefetched = false;
         }
@@ -792,7 +793,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           if (tr_on) UPR_TR(t, trc, 2);   // s_full acquired
           if (sub == nsub - 1) prefetch_next_q();   // every S_t MMA of this item is complete
 #if UPR_DIAG == 1 || UPR_DIAG == 3 || UPR_DIAG == 4
-          mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
           ++pv_cnt;
           continue;
 #endif
@@ -880,7 +882,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           l += (sumA.x + sumA.y) + (sumB.x + sumB.y);
           tmem_wait_st();
           tc_fence_before();
-          mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
           if (tr_on) UPR_TR(t, trc, 3);   // p_full arrived
           ++pv_cnt;
         }
@@ -897,7 +900,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           args.part_ml[prow * 2 + 0] = m_used;
           args.part_ml[prow * 2 + 1] = l;
         }
-        mbar_arrive(smem_u32(&ctrl->l_ready[t]));
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl->l_ready[t]));
       } else {
         // inactive tile: its Q buffer is idle, so the next item's tile can be staged now
         prefetch_next_q();
