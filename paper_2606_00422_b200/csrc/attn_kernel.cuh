@@ -36,6 +36,12 @@
 #ifndef UPR_DIAG
 #define UPR_DIAG 0   // timing experiments only: 1 = softmax math skipped, 2 = MMAs skipped
 #endif
+#ifndef UPR_POLY_D64
+#define UPR_POLY_D64 1
+#endif
+#ifndef UPR_POLY_D128
+#define UPR_POLY_D128 (-1)
+#endif
 #ifndef UPR_PINGPONG
 #define UPR_PINGPONG 1
 #endif
@@ -715,6 +721,10 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     uint32_t pv_cnt = 0;                     // PV sub-tile MMAs of this tile issued so far (all items)
     uint32_t trc = 0; (void)trc;
     const bool tr_on = (tid128 == 0); (void)tr_on;
+    // share of exponentials on the FMA pipe: -1 none, 1 -> 25 %, 0 -> 50 %.  Measured (A/B in one
+    // run): d = 64 bf16 cache +7.5 % at 25 %, +3.6 % at 50 %; d = 128 -2.5 %; FP8 cache -7 % (the
+    // converter warps already load the FMA / ALU pipes) -- so only d = 64 with a bf16 cache uses it.
+    constexpr int kPolyMask = (D == 64) ? (KV == KV_BF16 ? UPR_POLY_D64 : -1) : UPR_POLY_D128;
     const bool has_self = (args.k_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
     const size_t row_stride = static_cast<size_t>(args.H) * D;
@@ -862,7 +872,17 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               const float2 x23 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 2]),
                                                    __uint_as_float(sr[c0 + c + 3])), c2, nm2);
               const float p0 = ex2_approx(x01.x), p1 = ex2_approx(x01.y);
-              const float p2 = ex2_approx(x23.x), p3 = ex2_approx(x23.y);
+              float p2, p3;
+              // d = 64: one ex2 per 256 tensor FLOPs makes MUFU (16 / clk / SM) the ceiling, so
+              // a share of the exponentials is evaluated as a polynomial on the FMA pipe
+              if (kPolyMask >= 0 && ((c >> 2) & kPolyMask) == 0) {
+                const float2 e = ex2_poly2(x23);
+                p2 = e.x;
+                p3 = e.y;
+              } else {
+                p2 = ex2_approx(x23.x);
+                p3 = ex2_approx(x23.y);
+              }
               const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
               pr[(c >> 1) + 0] = w01;
               pr[(c >> 1) + 1] = w23;

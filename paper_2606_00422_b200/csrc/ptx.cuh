@@ -356,6 +356,27 @@ __device__ __forceinline__ float2 fmul2(float2 a, float2 b) {
   return d;
 }
 
+// exp2 of two values on the FMA pipe (no MUFU): round-to-nearest split x = n + f, |f| <= 0.5,
+// a degree-3 minimax polynomial for 2^f (max relative error 7.5e-5, far below the bf16
+// rounding of P) and an integer add of n into the exponent field.  x is clamped at -126 so
+// that the exponent never wraps (the result 2^-126 is absorbed by any real weight).
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  const float kMagic = 12582912.0f;   // 1.5 * 2^23: ulp 1, so (x + kMagic) holds round(x) in its low bits
+  x.x = fmaxf(x.x, -126.0f);
+  x.y = fmaxf(x.y, -126.0f);
+  const float2 t = fadd2(x, make_float2(kMagic, kMagic));
+  const float2 n = fadd2(t, make_float2(-kMagic, -kMagic));
+  const float2 f = fadd2(x, make_float2(-n.x, -n.y));
+  float2 p = ffma2(make_float2(0.05517164617776871f, 0.05517164617776871f), f,
+                   make_float2(0.2426111251115799f, 0.2426111251115799f));
+  p = ffma2(p, f, make_float2(0.6932609677314758f, 0.6932609677314758f));
+  p = ffma2(p, f, make_float2(0.9999280571937561f, 0.9999280571937561f));
+  float2 r;
+  r.x = __uint_as_float(__float_as_uint(p.x) + (__float_as_uint(t.x) << 23));
+  r.y = __uint_as_float(__float_as_uint(p.y) + (__float_as_uint(t.y) << 23));
+  return r;
+}
+
 // ------------------------------------------------------------------------------ misc
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
