@@ -1039,7 +1039,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
             const uint4 v = lds128(st_r + k * (4 * kEpiRowBytes));
-            if (4 * k < rem) *reinterpret_cast<uint4*>(gp + k * gstep + c0) = v;
+            if (4 * k < rem) stg128_stream(gp + k * gstep + c0, v);
           }
           __syncwarp();
         }
