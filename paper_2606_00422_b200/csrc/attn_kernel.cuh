@@ -990,6 +990,13 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           if (nt > 0) {
             tmem_ld32(tm_o + c0, orr);
             tmem_wait_ld_regs(orr);
+            if (c0 + 32 == D) {
+              // the accumulator is in registers: hand O_t back before staging / storing the
+              // last block, so the next item's first PV waits one block less
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive(smem_u32(&ctrl->o_empty[t]));
+            }
           } else {
 #pragma unroll
             for (int c = 0; c < 32; ++c) orr[c] = 0u;
@@ -1043,11 +1050,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           }
           __syncwarp();
         }
-        if (nt > 0) {
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&ctrl->o_empty[t]));
-        }
+
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
