@@ -31,6 +31,8 @@
 #include <math.h>
 #include <stdint.h>
 
+#include <cuda/std/type_traits>
+
 #include "ptx.cuh"
 
 #ifndef UPR_DIAG
@@ -794,26 +796,30 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         const bool pingpong = UPR_PINGPONG && (it.n_rows > kTileM) && nsub > 0;
         if (pingpong && t == 1) named_bar_arrive(1, 256);
 
-        for (int sub = 0; sub < nsub; ++sub) {
+        // One 64-key step.  The last step of an item (tail masking, next Q prefetch) is a separate
+        // instantiation so that the steady-state loop body stays as small as possible: the kernel
+        // is sensitive to the instruction footprint of this loop.
+        auto step = [&](const int sub, auto last_tag) {
+          constexpr bool kLast = decltype(last_tag)::value;
           const int bufi = sub % kNB;
           const uint32_t tm_sb = tm_s + bufi * kSubN;
           mbar_wait<16>(smem_u32(&ctrl->s_full[t][bufi]), sf_it[bufi] & 1);
           ++sf_it[bufi];
           tc_fence_after();
           if (tr_on) UPR_TR(t, trc, 2);   // s_full acquired
-          if (sub == nsub - 1) prefetch_next_q();   // every S_t MMA of this item is complete
+          if (kLast) prefetch_next_q();   // every S_t MMA of this item is complete
 #if UPR_DIAG == 1 || UPR_DIAG == 3 || UPR_DIAG == 4
           __syncwarp();
           if (lane == 0) mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
           ++pv_cnt;
-          continue;
+          return;
 #endif
           uint32_t sr[kSubN];
 #pragma unroll
           for (int c0 = 0; c0 < kSubN; c0 += 32) tmem_ld32(tm_sb + c0, &sr[c0]);
           tmem_wait_ld_regs(sr);
           const int keys_here = it.n_keys - sub * kSubN;  // may exceed 64
-          if (keys_here < kSubN) {
+          if (kLast && keys_here < kSubN) {
 #pragma unroll
             for (int c = 0; c < kSubN; ++c)
               if (c >= keys_here) sr[c] = 0xff800000u;  // -inf
@@ -898,7 +904,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             }
             tmem_st16(tm_sb + (c0 >> 1), pr);
           }
-          if (pingpong && !(t == 1 && sub == nsub - 1)) named_bar_arrive(2 - t, 256);
+          if (pingpong && !(t == 1 && kLast)) named_bar_arrive(2 - t, 256);
           l += (sumA.x + sumA.y) + (sumB.x + sumB.y);
           tmem_wait_st();
           tc_fence_before();
@@ -906,7 +912,9 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           if (lane == 0) mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
           if (tr_on) UPR_TR(t, trc, 3);   // p_full arrived
           ++pv_cnt;
-        }
+        };
+        for (int sub = 0; sub + 1 < nsub; ++sub) step(sub, cuda::std::false_type{});
+        if (nsub > 0) step(nsub - 1, cuda::std::true_type{});
         if (nsub == 0) prefetch_next_q();
 
         // ---------------------------------------------------------- hand over to the epilogue
