@@ -130,7 +130,7 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
 #pragma unroll
     for (int u = 0; u < U; ++u) {
       if (lh_u[u] < 0) continue;
-      if (MODE == 3) {
+      if constexpr (MODE == 3) {
         float wmax = 0.f;
 #pragma unroll
         for (int i = 0; i < NI; ++i) {
@@ -151,8 +151,7 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
           run_max = 0.f;
         }
         run_max = fmaxf(run_max, wmax);
-        continue;
-      }
+      } else {
 #pragma unroll
       for (int i = 0; i < NI; ++i) {
         const int c = i * 32 + lane;
@@ -183,6 +182,7 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
           dp[0] = o0;
           dp[1] = o1;
         }
+      }
       }
     }
   }
