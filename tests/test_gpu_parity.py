@@ -306,3 +306,27 @@ def test_baseline_configs_full_size_sampled(P, cfg):
             mx_pre, _ = error_stats(got[l, co[b]:co[b + 1], h], oracle_block(inp, l, b, h))
             assert mx_pre <= TOL_FP8, (b, l, h, mx_pre)
     assert worst <= TOL_BF16
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_random_ragged_shapes(P, seed):
+    """Seeded random shapes: ragged histories (incl. empty and multi-tile), ragged candidate counts
+    (incl. empty users and partial tiles), random head dim / cache dtype / self term / split count."""
+    rng = np.random.default_rng(1000 + seed)
+    B = int(rng.integers(1, 7))
+    L = [int(x) for x in rng.choice([0, 1, 15, 63, 64, 65, 127, 128, 129, 200, 513, 1100], size=B)]
+    C = [int(x) for x in rng.choice([0, 1, 31, 127, 128, 129, 255, 256, 257, 400], size=B)]
+    if sum(C) == 0:
+        C[0] = 5
+    d = int(rng.choice([64, 128]))
+    H = int(rng.integers(1, 4))
+    layers = int(rng.integers(1, 3))
+    kv = str(rng.choice(["bf16", "bf16", "fp8", "f32"]))
+    self_on = bool(rng.integers(0, 2))
+    ns = int(rng.choice([1, 1, 2, 5]))
+    w = S.custom_workload(f"fuzz{seed}", 7000 + seed, L, C, H, d, layers, kv_dtype=kv,
+                          q_dtype="f32" if kv == "f32" else "bf16", self_term=self_on)
+    inp = Inputs(w, "cuda")
+    got, _, _ = run_cuda(P, inp, num_splits=ns)
+    want = oracle_all(inp, dequant=(kv == "fp8"))
+    check(got, want, strict=TOL_BF16 if kv == "f32" else TOL_STRICT)
