@@ -223,7 +223,9 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
                         static_cast<long long>(p->H) * p->n_layers * ns;
   int grid = sm_count();
   if (grid <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
-  if (max_items < grid) grid = static_cast<int>(max_items < 1 ? 1 : max_items);
+  // (the plain entry point does not know total_q on the host: it always launches one CTA per SM;
+  // CTAs without an item leave at once)
+  if (have_workspace && max_items < grid) grid = static_cast<int>(max_items < 1 ? 1 : max_items);
 
   s = (p->d == 64) ? launch_attn_d<64>(p->kv_dtype, a, tk, tv, grid, st)
                    : launch_attn_d<128>(p->kv_dtype, a, tk, tv, grid, st);
