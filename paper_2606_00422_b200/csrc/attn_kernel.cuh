@@ -79,6 +79,8 @@ constexpr int kEpiWarp0 = 12;         // warps 12..15
 constexpr int kTmemCols = 512;
 constexpr float kRescaleTau = 8.0f;  // lazy-rescale threshold, log2 units
 constexpr int kEpiRowBytes = 144;     // 32 floats + 16 B pad: conflict-free 16-byte accesses
+// (a warp's staging block is 32 x 144 B = 4608 B; the TMA-store path uses its first 4096 B as a
+// dense, 128-byte-swizzled 32 x 32 fp32 box, so the block must start on a 1024-byte boundary)
 
 enum : int { KV_BF16 = 0, KV_FP8 = 1, KV_F32 = 2 };
 
@@ -118,6 +120,7 @@ struct AttnArgs {
   unsigned int* counter;  // dynamic work counter (zeroed before launch) or nullptr = static
   int B, H, n_layers, num_splits;
   int q_is_f32;
+  int out_tma;            // 1: tmap_out describes `out` as [n_layers*total_q, H*D] fp32 (full tiles use TMA stores)
   float scale_log2;       // sm_scale * log2(e)
 };
 
@@ -148,7 +151,8 @@ struct AttnCfg {
   static constexpr int kSmemQ = 2 * kTileBytes;
   static constexpr int kSmemKV = kStages * kTileBytes;
   static constexpr int kSmemRaw = kRawStages * kRawSlotBytes;
-  static constexpr int kSmemEpi = 4 * 32 * kEpiRowBytes;    // one 32 x 32 fp32 block per warp
+  static constexpr int kEpiWarpBytes = 5120;                // 32 x 144 B rounded up to 1024
+  static constexpr int kSmemEpi = 4 * kEpiWarpBytes;        // one 32 x 32 fp32 block per warp
   static constexpr int kSmemCtrl = 6144;
   static constexpr int kSmemTotal =
       kSmemQ + kSmemKV + kSmemRaw + kSmemEpi + kSmemCtrl + 1024;  // + alignment slack
@@ -326,7 +330,8 @@ __device__ __forceinline__ void e4m3x4_to_bf16x4(uint32_t w, uint32_t& lo, uint3
 template <int D, int KV>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
-                    const __grid_constant__ CUtensorMap tmap_v, const AttnArgs args) {
+                    const __grid_constant__ CUtensorMap tmap_v,
+                    const __grid_constant__ CUtensorMap tmap_out, const AttnArgs args) {
   using Cfg = AttnCfg<D, KV>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -941,7 +946,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     setmaxnreg_dec<kEpilogueRegs>();
     const int ew = warp - kEpiWarp0;                     // TMEM lane quarter of this warp
     const uint32_t lane_base = static_cast<uint32_t>(ew * 32) << 16;
-    const uint32_t stage = epi_smem + ew * (32 * kEpiRowBytes);
+    const uint32_t stage = epi_smem + ew * Cfg::kEpiWarpBytes;
     const bool has_self = (args.v_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
     const bool partial = args.num_splits > 1;
@@ -992,6 +997,41 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         const size_t se0 = q_elem0 + static_cast<size_t>(row) * args.H * D;
         const uint32_t tm_o = tmem_base + lane_base + 256 + t * D;
         const float2 sc2 = make_float2(sc, sc);
+        if (args.out_tma && !partial && !self_here && nt > 0 && rows_here == kTileM) {
+          // full tile, plain output: each 32 x 32 block is staged as a dense 128-byte-swizzled box
+          // and leaves through one TMA store; the warp only waits until the engine has READ the
+          // box before refilling it, never for the write to land
+          const int grow = static_cast<int>(grow0) + ew * 32;
+          const uint32_t sw_row = stage + lane * 128;
+#pragma unroll 1
+          for (int c0 = 0; c0 < D; c0 += 32) {
+            uint32_t orr[32];
+            tmem_ld32(tm_o + c0, orr);
+            tmem_wait_ld_regs(orr);
+            if (c0 + 32 == D) {
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive(smem_u32(&ctrl->o_empty[t]));
+            }
+            if (lane == 0) bulk_wait_read_all();
+            __syncwarp();
+#pragma unroll
+            for (int c = 0; c < 32; c += 4) {
+              const float2 a = fmul2(make_float2(__uint_as_float(orr[c]), __uint_as_float(orr[c + 1])), sc2);
+              const float2 b2 = fmul2(make_float2(__uint_as_float(orr[c + 2]), __uint_as_float(orr[c + 3])), sc2);
+              sts128(sw_row + (((c >> 2) ^ (lane & 7)) << 4), __float_as_uint(a.x), __float_as_uint(a.y),
+                     __float_as_uint(b2.x), __float_as_uint(b2.y));
+            }
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_2d(&tmap_out, stage, it.h * D + c0, grow);
+              bulk_commit();
+            }
+          }
+        } else {
+        if (lane == 0) bulk_wait_read_all();   // a TMA store of an earlier tile may still read the block
+        __syncwarp();
 #pragma unroll 1
         for (int c0 = 0; c0 < D; c0 += 32) {
           uint32_t orr[32];
@@ -1058,11 +1098,13 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           }
           __syncwarp();
         }
+        }
 
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
     }
+    if (lane == 0) bulk_wait_all();   // outstanding TMA stores must land before the CTA retires
   }
 
   // ------------------------------------------------------------------ teardown
