@@ -1003,10 +1003,10 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           // box before refilling it, never for the write to land
           const int grow = static_cast<int>(grow0) + ew * 32;
           const uint32_t sw_row = stage + lane * 128;
+          uint32_t orr[32];
+          tmem_ld32(tm_o, orr);
 #pragma unroll 1
           for (int c0 = 0; c0 < D; c0 += 32) {
-            uint32_t orr[32];
-            tmem_ld32(tm_o + c0, orr);
             tmem_wait_ld_regs(orr);
             if (c0 + 32 == D) {
               tc_fence_before();
@@ -1022,6 +1022,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               sts128(sw_row + (((c >> 2) ^ (lane & 7)) << 4), __float_as_uint(a.x), __float_as_uint(a.y),
                      __float_as_uint(b2.x), __float_as_uint(b2.y));
             }
+            if (c0 + 32 < D) tmem_ld32(tm_o + c0 + 32, orr);   // next block: overlaps the store hand-off
             fence_proxy_async_smem();
             __syncwarp();
             if (lane == 0) {
