@@ -120,6 +120,7 @@ struct AttnArgs {
   unsigned int* counter;  // dynamic work counter (zeroed before launch) or nullptr = static
   int B, H, n_layers, num_splits;
   int q_is_f32;
+  int q_tma;              // 1: tmap_q describes `q` as [n_layers*total_q, H*D] bf16: the producer loads Q tiles by TMA
   int out_tma;            // 1: tmap_out describes `out` as [n_layers*total_q, H*D] fp32 (full tiles use TMA stores)
   float scale_log2;       // sm_scale * log2(e)
 };
@@ -167,6 +168,7 @@ struct __align__(16) AttnCtrl {
   uint64_t raw_full[4];
   uint64_t raw_empty[4];
   uint64_t q_full[2];
+  uint64_t q_empty[2];     // the item's last S MMA of tile t has read Q_t (TMA Q loads only)
   uint64_t s_full[2][2];   // [tile][S buffer]
   uint64_t p_full[2][2];
   uint64_t pv_done[2];     // one completion per PV sub-tile MMA of tile t
@@ -331,7 +333,8 @@ template <int D, int KV>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v,
-                    const __grid_constant__ CUtensorMap tmap_out, const AttnArgs args) {
+                    const __grid_constant__ CUtensorMap tmap_out,
+                    const __grid_constant__ CUtensorMap tmap_q, const AttnArgs args) {
   using Cfg = AttnCfg<D, KV>;
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -349,6 +352,10 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
   // arrivals that release an item slot: 256 softmax threads, MMA lane 0, one lane of each
   // epilogue warp, one lane of each converter warp
   constexpr uint32_t kItemReaders = 256 + 1 + 4 + (kConvert ? 2 : 0);
+  // bf16 caches with a host-known total_q: Q tiles arrive by TMA, issued by the producer as soon
+  // as the previous item's last S MMA has released the tile (the cp.async path of the softmax
+  // warps could only start one step before the item's end and its latency showed at every item)
+  const bool q_by_tma = !kConvert && args.q_tma != 0;
 
   // ------------------------------------------------------------------ one-time setup
   if (threadIdx.x == 0) {
@@ -361,7 +368,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       mbar_init(smem_u32(&ctrl->raw_empty[i]), kConvThreads);
     }
     for (int t = 0; t < 2; ++t) {
-      mbar_init(smem_u32(&ctrl->q_full[t]), 4);       // one arrival per softmax warp
+      mbar_init(smem_u32(&ctrl->q_full[t]), q_by_tma ? 1 : 4);   // TMA transaction / one arrival per softmax warp
+      mbar_init(smem_u32(&ctrl->q_empty[t]), 1);
       for (int bf = 0; bf < 2; ++bf) {
         mbar_init(smem_u32(&ctrl->s_full[t][bf]), 1);
         mbar_init(smem_u32(&ctrl->p_full[t][bf]), 4);
@@ -410,6 +418,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     const int total_q = (args.B > 0) ? __ldg(args.cand_offsets + args.B) : 0;
 
     UserCursor cur{0, 0, 0};
+    uint32_t q_uses[2] = {0, 0};   // Q tile loads issued so far, per tile (TMA Q loads)
     uint32_t kv_it = 0;   // bf16 ring position (TMA mode) / raw ring position (convert mode)
     for (uint32_t n = 0;; ++n) {
       const int islot = n & 1;
@@ -479,13 +488,36 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         mbar_arrive(smem_u32(&ctrl->item_full[islot]));
         // stream this item's K/V tiles: K0 V0 K1 V1 ...
         const int nt = (n_keys + kTileN - 1) / kTileN;
+        // ... and its Q tiles, each as soon as the tile buffer is free again
+        bool pendq[2] = {false, false};
+        if (q_by_tma && nt > 0) {
+          pendq[0] = true;
+          pendq[1] = it.n_rows > kTileM;
+        }
+        auto try_issue_q = [&]() {
+#pragma unroll
+          for (int t = 0; t < 2; ++t) {
+            if (!pendq[t]) continue;
+            if (q_uses[t] > 0 && !mbar_test(smem_u32(&ctrl->q_empty[t]), (q_uses[t] - 1) & 1)) continue;
+            const uint32_t full = smem_u32(&ctrl->q_full[t]);
+            mbar_arrive_expect_tx(full, Cfg::kTileBytes);
+            const int qrow = layer * total_q + it.q_row0 + t * kTileM;
+#pragma unroll
+            for (int bx = 0; bx < Cfg::kBoxes; ++bx)
+              tma_load_2d(q_smem + t * Cfg::kTileBytes + bx * Cfg::kBoxBytes, &tmap_q, h * D + bx * 64, qrow,
+                          full);
+            ++q_uses[t];
+            pendq[t] = false;
+          }
+        };
+        try_issue_q();
         for (int j = 0; j < nt; ++j) {
 #pragma unroll
           for (int kv = 0; kv < 2; ++kv) {
             if constexpr (!kConvert) {
               const uint32_t slot = kv_it % Cfg::kStages;
               const uint32_t ph = (kv_it / Cfg::kStages) & 1;
-              mbar_wait<2>(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
+              while (!mbar_try_wait<2>(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1)) try_issue_q();
               const uint32_t full = smem_u32(&ctrl->kv_full[slot]);
               mbar_arrive_expect_tx(full, Cfg::kTileBytes);
               const uint32_t dst = kv_smem + slot * Cfg::kTileBytes;
@@ -511,6 +543,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
             }
           }
         }
+        while (pendq[0] || pendq[1]) try_issue_q();
       }
       __syncwarp();
     }
@@ -570,6 +603,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               umma_ss(ts, mk_desc(qt_lo + off), mk_desc(kk + off), Cfg::kIdescQK, k > 0);
             }
             umma_commit(bar_s + (2 * t + (sub % kNB)) * 8);
+            if (sub == nsub - 1) umma_commit(smem_u32(&ctrl->q_empty[t]));   // Q_t may be refilled
           };
           // prologue: S(0), S(1) from K tile 0
           {
@@ -759,8 +793,11 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       const int nsub = (rows_here > 0) ? (it.n_keys + kSubN - 1) / kSubN : 0;
       // Prefetch the NEXT item's Q tile as soon as this item's last S_t MMA has read Q_t.
       auto prefetch_next_q = [&]() {
+        // (the wait stays even when the producer loads Q by TMA: a group must not release item n
+        // before item n+1 is published -- without it, CTAs with key-less items in between hung)
         const uint32_t n1 = n + 1;
         mbar_wait<15>(smem_u32(&ctrl->item_full[n1 & 1]), (n1 >> 1) & 1);
+        if (q_by_tma) return;
         const WorkItem nx = ctrl->items[n1 & 1];
         if (nx.valid && nx.n_rows > t * kTileM && nx.n_keys > 0) {
           issue_q(nx);
@@ -770,7 +807,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       if (rows_here > 0) {
         const bool row_valid = tid128 < rows_here;
         const size_t my_elem0 = tile_elem0_of(it) + static_cast<size_t>(tid128) * row_stride;
-        if (nsub > 0) {
+        if (nsub > 0 && !q_by_tma) {
           if (!q_prefetched) issue_q(it);
           cp_async_wait_all();
           fence_proxy_async_smem();

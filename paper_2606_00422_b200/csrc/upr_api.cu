@@ -134,7 +134,7 @@ upr_status validate(const upr_attn_params* p) {
 
 template <int D, int KV>
 upr_status launch_attn(const upr::AttnArgs& a, const CUtensorMap& tk, const CUtensorMap& tv,
-                       const CUtensorMap& to, int grid, cudaStream_t st) {
+                       const CUtensorMap& to, const CUtensorMap& tq, int grid, cudaStream_t st) {
   using Cfg = upr::AttnCfg<D, KV>;
   static bool attr_set = false;
   if (!attr_set) {
@@ -143,18 +143,19 @@ upr_status launch_attn(const upr::AttnArgs& a, const CUtensorMap& tk, const CUte
                                         Cfg::kSmemTotal));
     attr_set = true;
   }
-  upr::upr_attn_fwd_kernel<D, KV><<<grid, upr::kAttnThreads, Cfg::kSmemTotal, st>>>(tk, tv, to, a);
+  upr::upr_attn_fwd_kernel<D, KV><<<grid, upr::kAttnThreads, Cfg::kSmemTotal, st>>>(tk, tv, to, tq, a);
   UPR_CUDA_CHECK(cudaGetLastError());
   return UPR_OK;
 }
 
 template <int D>
 upr_status launch_attn_d(int kv_dtype, const upr::AttnArgs& a, const CUtensorMap& tk,
-                         const CUtensorMap& tv, const CUtensorMap& to, int grid, cudaStream_t st) {
+                         const CUtensorMap& tv, const CUtensorMap& to, const CUtensorMap& tq, int grid,
+                         cudaStream_t st) {
   switch (kv_dtype) {
-    case UPR_BF16: return launch_attn<D, upr::KV_BF16>(a, tk, tv, to, grid, st);
-    case UPR_FP8_E4M3: return launch_attn<D, upr::KV_FP8>(a, tk, tv, to, grid, st);
-    default: return launch_attn<D, upr::KV_F32>(a, tk, tv, to, grid, st);
+    case UPR_BF16: return launch_attn<D, upr::KV_BF16>(a, tk, tv, to, tq, grid, st);
+    case UPR_FP8_E4M3: return launch_attn<D, upr::KV_FP8>(a, tk, tv, to, tq, grid, st);
+    default: return launch_attn<D, upr::KV_F32>(a, tk, tv, to, tq, grid, st);
   }
 }
 
@@ -245,8 +246,25 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS)
       a.out_tma = 1;
   }
-  s = (p->d == 64) ? launch_attn_d<64>(p->kv_dtype, a, tk, tv, to, grid, st)
-                   : launch_attn_d<128>(p->kv_dtype, a, tk, tv, to, grid, st);
+  // `q` as a 2-D bf16 tensor [n_layers * total_q, H * d]: Q tiles by TMA (bf16 q and cache only)
+  CUtensorMap tq;
+  memset(&tq, 0, sizeof(tq));
+  if (have_workspace && p->total_q > 0 && p->q_dtype == UPR_BF16 && p->kv_dtype == UPR_BF16 &&
+      static_cast<long long>(p->n_layers) * p->total_q < (1LL << 31)) {
+    EncodeTiledFn enc = get_encode_fn();
+    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(p->H) * p->d,
+                          static_cast<cuuint64_t>(p->n_layers) * static_cast<cuuint64_t>(p->total_q)};
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(p->H) * p->d * 2};
+    cuuint32_t box[2] = {64, 128};
+    cuuint32_t estr[2] = {1, 1};
+    if (enc != nullptr &&
+        enc(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(p->q), gdim, gstride, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS)
+      a.q_tma = 1;
+  }
+  s = (p->d == 64) ? launch_attn_d<64>(p->kv_dtype, a, tk, tv, to, tq, grid, st)
+                   : launch_attn_d<128>(p->kv_dtype, a, tk, tv, to, tq, grid, st);
   if (s != UPR_OK) return s;
   g_launches = 1;
   if (ns > 1) {

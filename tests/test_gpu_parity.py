@@ -330,3 +330,25 @@ def test_random_ragged_shapes(P, seed):
     got, _, _ = run_cuda(P, inp, num_splits=ns)
     want = oracle_all(inp, dequant=(kv == "fp8"))
     check(got, want, strict=TOL_BF16 if kv == "f32" else TOL_STRICT)
+
+
+@pytest.mark.parametrize("name,L,ns", [
+    ("empty_between_real", [0, 512] * 32, 1),
+    ("mostly_empty", [0] * 40 + [512] * 24, 1),
+    ("empty_split_ranges", [64] * 32 + [2000] * 32, 3),
+])
+def test_many_items_per_cta_with_keyless_items(P, name, L, ns):
+    """Several work items per CTA (more items than SMs) with items that have no key at all in
+    between (empty histories; history splits whose tile range is empty): the cross-item hand-over
+    of the Q tiles and accumulators must not depend on every item doing MMA work.  Sampled
+    (layer, user, head) blocks are checked row by row; everything must be finite."""
+    w = S.custom_workload(name, 515, L, [512] * len(L), 8, 128, 2)
+    inp = Inputs(w, "cuda")
+    got, _, attn = run_cuda(P, inp, num_splits=ns)
+    assert attn.splits == ns and np.all(np.isfinite(got))
+    co = w.cand_offsets
+    rng = np.random.default_rng(5)
+    for b in sorted(set([0, 1, len(L) - 1] + [int(x) for x in rng.integers(0, len(L), size=5)])):
+        l, h = int(rng.integers(0, 2)), int(rng.integers(0, 8))
+        mx, rel = error_stats(got[l, co[b]:co[b + 1], h], oracle_block(inp, l, b, h))
+        assert mx <= TOL_STRICT and rel <= TOL_RMS, (b, l, h, mx, rel)
