@@ -347,8 +347,8 @@ def run_ours(args):
                 "achieved": tflops, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": tflops / peaks["bf16_tflops"],
                 # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the ncu --set full
-                # capture summarised in profiles/r1k_final.md (config 3 only)
-                "traffic": (6.347e9 + 2.165e9) if w.cfg == 3 and world == 1 else None,
+                # capture summarised in profiles/r1l_final.md (config 3 only)
+                "traffic": (6.343e9 + 2.164e9) if w.cfg == 3 and world == 1 else None,
                 "traffic_algorithmic": w.kv_bytes + 6 * w.total_q * w.H * w.d * w.n_layers,
                 "peak_source": peaks["source"] + " (burst cuBLAS bf16)",
                 "frac_of_sustained": tflops / peaks["bf16_tflops_sustained"],
