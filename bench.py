@@ -346,9 +346,9 @@ def run_ours(args):
     roofline = {"bound": "tensor" if t_flop >= t_mem else "hbm", "kernel": "upr_attn_fwd_kernel",
                 "achieved": tflops, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": tflops / peaks["bf16_tflops"],
-                # dram__bytes_read.sum + dram__bytes_write.sum of one launch, from the ncu --set full
-                # capture summarised in profiles/r1l_final.md (config 3 only)
-                "traffic": (6.343e9 + 2.164e9) if w.cfg == 3 and world == 1 else None,
+                # ncu counters cannot be read from inside an unprofiled run: the DRAM bytes of the ncu
+                # --set full capture of this build are recorded under profiles/ (keyed by commit)
+                "traffic": None, "traffic_source": "profiles/ (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
                 "traffic_algorithmic": w.kv_bytes + 6 * w.total_q * w.H * w.d * w.n_layers,
                 "peak_source": peaks["source"] + " (burst cuBLAS bf16)",
                 "frac_of_sustained": tflops / peaks["bf16_tflops_sustained"],
@@ -392,7 +392,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="3")

@@ -25,7 +25,7 @@ ROW_ALIGN = 16  # DESIGN.md reading Q14
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (no CUDA involved)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        cmd = ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", _SRC, "-o", _LIB, "-lm"]
+        cmd = ["gcc", "-O3", "-fopenmp", "-ffp-contract=off", "-shared", "-fPIC", _SRC, "-o", _LIB, "-lm"]
         subprocess.run(cmd, check=True, capture_output=True)
     return _LIB
 
@@ -204,4 +204,35 @@ def cross_attn_packed(q, q_dtype: int, k_cache, v_cache, kv_dtype: int, seq_lens
                                       ctypes.c_double(sm_scale), lo, hi, _p(out))
     if rc:
         raise ValueError("upro_cross_attn_packed: invalid argument")
+    return out
+
+
+def cross_attn_pool(q, q_dtype: int, k_pool_bits, v_pool_bits, slot_ids, seq_lens, cand_offsets, H_q: int,
+                    kself=None, vself=None, sm_scale=None, users=None):
+    """Whole ragged batch read straight from the pool [n_layers,S,H_kv,n_max,d] (bf16 bits), no pack
+    (zero-copy addressing); H_q may be a multiple of H_kv (grouped queries: head hq -> KV head hq // G).
+    Returns out [n_layers, total_q, H_q, d] float64; rows of users outside ``users`` stay zero."""
+    k_pool_bits = np.ascontiguousarray(k_pool_bits, dtype=np.uint16)
+    v_pool_bits = np.ascontiguousarray(v_pool_bits, dtype=np.uint16)
+    n_layers, S, H_kv, n_max, d = k_pool_bits.shape
+    assert v_pool_bits.shape == k_pool_bits.shape
+    slot_ids = np.ascontiguousarray(slot_ids, dtype=np.int32)
+    seq_lens = np.ascontiguousarray(seq_lens, dtype=np.int32)
+    cand_offsets = np.ascontiguousarray(cand_offsets, dtype=np.int32)
+    B = int(seq_lens.shape[0])
+    total_q = int(cand_offsets[B])
+    if sm_scale is None:
+        sm_scale = 1.0 / np.sqrt(d)
+    qdt = np.float32 if q_dtype == F32 else np.uint16
+    q = np.ascontiguousarray(q, dtype=qdt)
+    assert q.size == n_layers * total_q * H_q * d
+    ks = np.ascontiguousarray(kself, dtype=qdt) if kself is not None else None
+    vs = np.ascontiguousarray(vself, dtype=qdt) if vself is not None else None
+    lo, hi = (0, B) if users is None else users
+    out = np.zeros((n_layers, total_q, H_q, d), dtype=np.float64)
+    rc = lib().upro_cross_attn_pool(_p(q), q_dtype, _p(k_pool_bits), _p(v_pool_bits), n_layers, S, H_kv, n_max, d,
+                                    H_q, _p(slot_ids), _p(seq_lens), _p(cand_offsets), B, _p(ks), _p(vs),
+                                    ctypes.c_double(sm_scale), lo, hi, _p(out))
+    if rc:
+        raise ValueError("upro_cross_attn_pool: invalid argument")
     return out

@@ -23,7 +23,7 @@
  * constructed ties; layout tables against hand-written tiny cases.  No function in this
  * file is "parity unpinned".
  *
- * Build: gcc -O2 -fopenmp -ffp-contract=off -shared -fPIC upr_oracle.c -o libupr_oracle.so -lm
+ * Build: gcc -O3 -fopenmp -ffp-contract=off -shared -fPIC upr_oracle.c -o libupr_oracle.so -lm
  * (-ffp-contract=off: the fp32 steps of the quantiser must round once per operation.)
  */
 #include <math.h>
@@ -482,5 +482,75 @@ int upro_cross_attn_packed(const void* q, int q_dtype, const void* k_cache, cons
     free(vsb);
   }
   free(row_off);
+  return 0;
+}
+
+/* ------------------------------------------------------------------------------------
+ * Whole batch straight from the paper's pool (zero-copy addressing): the
+ * history K/V of user b are rows [0, L_b) of slot slot_ids[b] of the pool
+ * [n_layers][S][H_kv][n_max][d] ("[L,S,H,n,D] ... KV heads"), read in place
+ * instead of through the slot copy of PAPER.md:204.  Grouped queries ("KV
+ * heads", reading Q5): query head hq attends over KV head hq / (H_q / H_kv); H_q == H_kv is
+ * the ungrouped case.  Plain indexing + upro_attn_block, nothing else.
+ *   q, kself, vself : [n_layers][total_q][H_q][d], q_dtype F32 or BF16 bits
+ *   k_pool, v_pool  : bf16 bits
+ *   out             : [n_layers][total_q][H_q][d] fp64
+ * Returns 1 on invalid arguments (H_q not a multiple of H_kv, slot or length out of range).
+ * ---------------------------------------------------------------------------------- */
+int upro_cross_attn_pool(const void* q, int q_dtype, const uint16_t* k_pool,
+                         const uint16_t* v_pool, int n_layers, int S, int H_kv, int n_max, int d,
+                         int H_q, const int32_t* slot_ids, const int32_t* seq_lens,
+                         const int32_t* cand_offsets, int B, const void* kself, const void* vself,
+                         double sm_scale, int users_lo, int users_hi, double* out) {
+  if (H_kv <= 0 || H_q <= 0 || H_q % H_kv != 0) return 1;
+  for (int b = 0; b < B; ++b)
+    if (seq_lens[b] < 0 || seq_lens[b] > n_max || slot_ids[b] < 0 || slot_ids[b] >= S) return 1;
+  int G = H_q / H_kv;
+  int64_t total_q = cand_offsets[B];
+  if (users_lo < 0) users_lo = 0;
+  if (users_hi > B) users_hi = B;
+  int64_t n_blocks = (int64_t)n_layers * (users_hi - users_lo) * H_q;
+#pragma omp parallel for schedule(dynamic, 1)
+  for (int64_t blk = 0; blk < n_blocks; ++blk) {
+    int hq = (int)(blk % H_q);
+    int b = users_lo + (int)((blk / H_q) % (users_hi - users_lo));
+    int l = (int)(blk / ((int64_t)H_q * (users_hi - users_lo)));
+    int hk = hq / G;
+    int C = cand_offsets[b + 1] - cand_offsets[b];
+    int L = seq_lens[b];
+    if (C <= 0) continue;
+    double* qb = (double*)malloc(sizeof(double) * (size_t)C * d);
+    double* ob = (double*)malloc(sizeof(double) * (size_t)C * d);
+    double* Kb = (double*)malloc(sizeof(double) * (size_t)(L > 0 ? L : 1) * d);
+    double* Vb = (double*)malloc(sizeof(double) * (size_t)(L > 0 ? L : 1) * d);
+    double* ksb = kself ? (double*)malloc(sizeof(double) * (size_t)C * d) : NULL;
+    double* vsb = kself ? (double*)malloc(sizeof(double) * (size_t)C * d) : NULL;
+    for (int c = 0; c < C; ++c)
+      for (int t = 0; t < d; ++t) {
+        int64_t gi = ((((int64_t)l * total_q + cand_offsets[b] + c) * H_q) + hq) * d + t;
+        qb[(size_t)c * d + t] = load_elem(q, q_dtype, gi, 1.0);
+        if (kself) {
+          ksb[(size_t)c * d + t] = load_elem(kself, q_dtype, gi, 1.0);
+          vsb[(size_t)c * d + t] = load_elem(vself, q_dtype, gi, 1.0);
+        }
+      }
+    int64_t base = ((((int64_t)l * S + slot_ids[b]) * H_kv + hk) * n_max) * (int64_t)d;
+    for (int64_t i = 0; i < (int64_t)L * d; ++i) {
+      Kb[i] = upro_bf16_to_f64(k_pool[base + i]);
+      Vb[i] = upro_bf16_to_f64(v_pool[base + i]);
+    }
+    upro_attn_block(qb, Kb, Vb, ksb, vsb, C, L, d, sm_scale, ob, NULL);
+    for (int c = 0; c < C; ++c)
+      for (int t = 0; t < d; ++t) {
+        int64_t gi = ((((int64_t)l * total_q + cand_offsets[b] + c) * H_q) + hq) * d + t;
+        out[gi] = ob[(size_t)c * d + t];
+      }
+    free(qb);
+    free(ob);
+    free(Kb);
+    free(Vb);
+    free(ksb);
+    free(vsb);
+  }
   return 0;
 }

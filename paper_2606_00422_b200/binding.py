@@ -20,8 +20,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 
 
 def lib_path() -> str:
-    # UPR_LIB_PATH lets an experiment load an alternative build of the same library
-    return os.environ.get("UPR_LIB_PATH") or os.path.join(_HERE, "libupr.so")
+    return os.path.join(_HERE, "libupr.so")
 
 
 class UprError(RuntimeError):

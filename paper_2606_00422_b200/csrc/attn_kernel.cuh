@@ -35,30 +35,11 @@
 
 #include "ptx.cuh"
 
-#ifndef UPR_DIAG
-#define UPR_DIAG 0   // timing experiments only: 1 = softmax math skipped, 2 = MMAs skipped
-#endif
-#ifndef UPR_POLY_D64
-#define UPR_POLY_D64 1
-#endif
-#ifndef UPR_POLY_D128
-#define UPR_POLY_D128 (-1)
-#endif
-#ifndef UPR_PINGPONG
-#define UPR_PINGPONG 1
-#endif
-#ifndef UPR_CONSISTENT_ROWSUM
-#define UPR_CONSISTENT_ROWSUM 1
-#endif
-
 namespace upr {
 
 constexpr int kTileM = 128;     // candidate rows per MMA tile == TMEM lanes
 constexpr int kTileN = 128;     // keys per K/V smem tile
-#ifndef UPR_NB
-#define UPR_NB 2
-#endif
-constexpr int kNB = UPR_NB;        // S buffers per candidate tile (1 or 2)
+constexpr int kNB = 2;          // S buffers per candidate tile
 constexpr int kSubN = kTileN / kNB;   // keys per softmax / MMA step: S(s + kNB) is issued behind PV(s)
 constexpr int kQBlock = 256;    // candidate rows per work item (two tiles)
 constexpr int kRowAlign = 16;   // UPR_ROW_ALIGN
@@ -66,9 +47,9 @@ constexpr int kAttnThreads = 512;     // 2 softmax warpgroups + {TMA, MMA, 2 con
 // setmaxnreg budgets.  The pool is what the CTA was given at launch (512 threads x 128
 // registers), not the whole register file: an .inc beyond it blocks forever.
 constexpr int kLaunchRegs = 128;
-constexpr int kSoftmaxRegs = (UPR_NB == 1) ? 200 : 168;   //   2 softmax warpgroups
-constexpr int kOtherRegs = (UPR_NB == 1) ? 48 : 56;       //   producer / MMA / converter warpgroup
-constexpr int kEpilogueRegs = (UPR_NB == 1) ? 64 : 88;    //   epilogue warpgroup
+constexpr int kSoftmaxRegs = 168;    //   2 softmax warpgroups
+constexpr int kOtherRegs = 56;       //   producer / MMA / converter warpgroup
+constexpr int kEpilogueRegs = 88;    //   epilogue warpgroup
 static_assert(256 * kSoftmaxRegs + 128 * kOtherRegs + 128 * kEpilogueRegs <= kAttnThreads * kLaunchRegs,
               "setmaxnreg budgets exceed the CTA's register allocation");
 constexpr int kProducerWarp = 8;
@@ -83,26 +64,6 @@ constexpr int kEpiRowBytes = 144;     // 32 floats + 16 B pad: conflict-free 16-
 // dense, 128-byte-swizzled 32 x 32 fp32 box, so the block must start on a 1024-byte boundary)
 
 enum : int { KV_BF16 = 0, KV_FP8 = 1, KV_F32 = 2 };
-
-// Timeline tracing for experiments (-DUPR_TRACE=1 builds only; never in the product library):
-// CTA 0 records (event id, clock64) pairs into a device array read back by upr_debug_trace.
-#ifndef UPR_TRACE
-#define UPR_TRACE 0
-#endif
-#if UPR_TRACE
-__device__ unsigned long long g_trace[16][2048];
-__device__ __forceinline__ void trace(int role, uint32_t& cnt, int ev) {
-  if (blockIdx.x == 0 && cnt < 2047) {
-    g_trace[role][1 + cnt] = (static_cast<unsigned long long>(ev) << 48) |
-                             (static_cast<unsigned long long>(clock64()) & 0xFFFFFFFFFFFFull);
-    ++cnt;
-    g_trace[role][0] = cnt;
-  }
-}
-#define UPR_TR(role, cnt, ev) trace(role, cnt, ev)
-#else
-#define UPR_TR(role, cnt, ev)
-#endif
 
 struct AttnArgs {
   const void* q;
@@ -562,7 +523,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     if (elect_one()) {
       uint32_t kv_pos = 0;                       // ring position of the next item's K tile 0
       uint32_t q_ph = 0, od_ph = 0, pf_ph = 0;   // phase bits: q_full[t], o_empty[t], p_full[t][buf]
-      uint32_t trc = 0; (void)trc;
       // descriptor words: lo = addr >> 4 | (LBO >> 4) << 16, hi = SBO >> 4 | version 1 | SWIZZLE_128B
       constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
       constexpr uint32_t kLoKmajor = (16u >> 4) << 16;                                     // Q, K
@@ -578,7 +538,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         const int islot = n & 1;
         mbar_wait<4>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
         if (!ctrl->items[islot].valid) break;
-        UPR_TR(2, trc, 1);   // item acquired
         const int n_keys = ctrl->items[islot].n_keys;
         const int nt = (n_keys + kTileN - 1) / kTileN;
         const int nsub = (n_keys + kSubN - 1) / kSubN;
@@ -587,9 +546,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
 #pragma unroll
           for (int t = 0; t < 2; ++t)
             if (t < ntile) {
-#if UPR_DIAG != 6
               mbar_wait<5>(smem_u32(&ctrl->q_full[t]), (q_ph >> t) & 1);
-#endif
               q_ph ^= 1u << t;
             }
           // S_t(sub) = Q_t K[sub]^T into S buffer sub & 1; k_lo = descriptor word of the K tile
@@ -616,7 +573,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               for (int t = 0; t < 2; ++t)
                 if (t < ntile) issue_qk(t, sub, k_lo);
             umma_commit(smem_u32(&ctrl->kv_empty[slot]));   // K tile 0: both sub-tiles issued
-            UPR_TR(2, trc, 3);   // prologue issued
           }
           uint32_t vslot = 0, kslot = 0;
           for (int sub = 0; sub < nsub; ++sub) {
@@ -636,16 +592,12 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               if (t < ntile) {
                 if (sub == 0) {
                   // the epilogue group must have drained O_t of the previous item
-#if UPR_DIAG != 5
                   mbar_wait<8>(smem_u32(&ctrl->o_empty[t]), ((od_ph >> t) & 1) ^ 1);
-#endif
                   od_ph ^= 1u << t;
-                  UPR_TR(2, trc, 4 + t);   // o_empty acquired
                 }
                 mbar_wait<9>(bar_p + (2 * t + bufi) * 8, (pf_ph >> (2 * t + bufi)) & 1);
                 pf_ph ^= 1u << (2 * t + bufi);
                 tc_fence_after();
-                UPR_TR(2, trc, 10 + t);   // p_full acquired
                 const uint32_t tp = tmem_base + t * 128 + bufi * kSubN;
                 const uint32_t to = tmem_base + 256 + t * D;
 #pragma unroll
@@ -678,7 +630,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           }
           kv_pos += 2 * nt;
         }
-        UPR_TR(2, trc, 9);   // item issued
         mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
       }
     }
@@ -760,12 +711,10 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     const uint32_t q_tile_smem = q_smem + t * Cfg::kTileBytes;
     uint32_t sf_it[2] = {0, 0};              // s_full phase counters per S buffer
     uint32_t pv_cnt = 0;                     // PV sub-tile MMAs of this tile issued so far (all items)
-    uint32_t trc = 0; (void)trc;
-    const bool tr_on = (tid128 == 0); (void)tr_on;
     // share of exponentials on the FMA pipe: -1 none, 1 -> 25 %, 0 -> 50 %.  Measured (A/B in one
     // run): d = 64 bf16 cache +7.5 % at 25 %, +3.6 % at 50 %; d = 128 -2.5 %; FP8 cache -7 % (the
     // converter warps already load the FMA / ALU pipes) -- so only d = 64 with a bf16 cache uses it.
-    constexpr int kPolyMask = (D == 64) ? (KV == KV_BF16 ? UPR_POLY_D64 : -1) : UPR_POLY_D128;
+    constexpr int kPolyMask = (D == 64 && KV == KV_BF16) ? 1 : -1;
     const bool has_self = (args.k_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
     const size_t row_stride = static_cast<size_t>(args.H) * D;
@@ -788,7 +737,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       mbar_wait<14>(smem_u32(&ctrl->item_full[islot]), (n >> 1) & 1);
       const WorkItem it = ctrl->items[islot];
       if (!it.valid) break;
-      if (tr_on) UPR_TR(t, trc, 1);   // item acquired
       const int rows_here = min(kTileM, it.n_rows - t * kTileM);  // <= 0: tile inactive
       const int nsub = (rows_here > 0) ? (it.n_keys + kSubN - 1) / kSubN : 0;
       // Prefetch the NEXT item's Q tile as soon as this item's last S_t MMA has read Q_t.
@@ -813,7 +761,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) mbar_arrive(smem_u32(&ctrl->q_full[t]));
-          if (tr_on) UPR_TR(t, trc, 4);   // q_full arrived
           q_prefetched = false;
         }
         const int sidx = it.layer * args.H + it.h;
@@ -835,7 +782,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         // 8 cycles each per SMSP).  The two softmax warps of an SMSP drift into lockstep
         // unless forced apart, and then nothing hides either part; handing the MUFU phase
         // back and forth keeps them in anti-phase.  Barrier 1 = "group 0 may go", 2 = "group 1".
-        const bool pingpong = UPR_PINGPONG && (it.n_rows > kTileM) && nsub > 0;
+        const bool pingpong = (it.n_rows > kTileM) && nsub > 0;
         if (pingpong && t == 1) named_bar_arrive(1, 256);
 
         // One 64-key step.  The last step of an item (tail masking, next Q prefetch) is a separate
@@ -848,14 +795,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           mbar_wait<16>(smem_u32(&ctrl->s_full[t][bufi]), sf_it[bufi] & 1);
           ++sf_it[bufi];
           tc_fence_after();
-          if (tr_on) UPR_TR(t, trc, 2);   // s_full acquired
           if (kLast) prefetch_next_q();   // every S_t MMA of this item is complete
-#if UPR_DIAG == 1 || UPR_DIAG == 3 || UPR_DIAG == 4
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
-          ++pv_cnt;
-          return;
-#endif
           uint32_t sr[kSubN];
 #pragma unroll
           for (int c0 = 0; c0 < kSubN; c0 += 32) tmem_ld32(tm_sb + c0, &sr[c0]);
@@ -934,15 +874,10 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
               pr[(c >> 1) + 0] = w01;
               pr[(c >> 1) + 1] = w23;
-#if UPR_CONSISTENT_ROWSUM
               sumA = fadd2(sumA, make_float2(__uint_as_float(w01 << 16),
                                              __uint_as_float(w01 & 0xffff0000u)));
               sumB = fadd2(sumB, make_float2(__uint_as_float(w23 << 16),
                                              __uint_as_float(w23 & 0xffff0000u)));
-#else
-              sumA = fadd2(sumA, make_float2(p0, p1));
-              sumB = fadd2(sumB, make_float2(p2, p3));
-#endif
             }
             tmem_st16(tm_sb + (c0 >> 1), pr);
           }
@@ -952,7 +887,6 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(smem_u32(&ctrl->p_full[t][bufi]));
-          if (tr_on) UPR_TR(t, trc, 3);   // p_full arrived
           ++pv_cnt;
         };
         for (int sub = 0; sub + 1 < nsub; ++sub) step(sub, cuda::std::false_type{});

@@ -7,6 +7,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <atomic>
+
 #include "../../include/upr.h"
 #include "attn_kernel.cuh"
 #include "pack_kernels.cuh"
@@ -39,16 +41,20 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 EncodeTiledFn get_encode_fn() {
-  static EncodeTiledFn fn = nullptr;
-  if (fn == nullptr) {
+  // the driver entry point is process-wide and immutable; a racing first call stores the same value
+  static std::atomic<EncodeTiledFn> fn{nullptr};
+  EncodeTiledFn f = fn.load(std::memory_order_acquire);
+  if (f == nullptr) {
     void* p = nullptr;
     cudaDriverEntryPointQueryResult qres;
     if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) ==
             cudaSuccess &&
-        qres == cudaDriverEntryPointSuccess)
-      fn = reinterpret_cast<EncodeTiledFn>(p);
+        qres == cudaDriverEntryPointSuccess) {
+      f = reinterpret_cast<EncodeTiledFn>(p);
+      fn.store(f, std::memory_order_release);
+    }
   }
-  return fn;
+  return f;
 }
 
 // 2-D bf16 view [rows, d] of a packed cache; box = [128 rows x 64 cols], 128-byte swizzle.
@@ -68,26 +74,21 @@ upr_status make_kv_tmap(CUtensorMap* m, const void* base, int d) {
   return UPR_OK;
 }
 
+// Per-device facts, queried on every call (two cheap runtime calls): nothing is cached across
+// devices or threads, so a process may use the library on any number of devices and threads.
 int sm_count() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess ||
-        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
-      n = 0;
-  }
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+    return 0;
   return n;
 }
 
 upr_status check_device() {
-  static int ok = -1;
-  if (ok < 0) {
-    int dev = 0, major = 0;
-    UPR_CUDA_CHECK(cudaGetDevice(&dev));
-    UPR_CUDA_CHECK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
-    ok = (major == 10) ? 1 : 0;
-  }
-  if (!ok) return fail(UPR_ERR_UNSUPPORTED, "libupr requires an sm_100a (B200) device");
+  int dev = 0, major = 0;
+  UPR_CUDA_CHECK(cudaGetDevice(&dev));
+  UPR_CUDA_CHECK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+  if (major != 10) return fail(UPR_ERR_UNSUPPORTED, "libupr requires an sm_100a (B200) device");
   return UPR_OK;
 }
 
@@ -136,13 +137,9 @@ template <int D, int KV>
 upr_status launch_attn(const upr::AttnArgs& a, const CUtensorMap& tk, const CUtensorMap& tv,
                        const CUtensorMap& to, const CUtensorMap& tq, int grid, cudaStream_t st) {
   using Cfg = upr::AttnCfg<D, KV>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::upr_attn_fwd_kernel<D, KV>,
-                                        cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        Cfg::kSmemTotal));
-    attr_set = true;
-  }
+  // per call: the attribute is per device (and per context), the call costs about a microsecond
+  UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::upr_attn_fwd_kernel<D, KV>,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemTotal));
   upr::upr_attn_fwd_kernel<D, KV><<<grid, upr::kAttnThreads, Cfg::kSmemTotal, st>>>(tk, tv, to, tq, a);
   UPR_CUDA_CHECK(cudaGetLastError());
   return UPR_OK;
@@ -284,13 +281,6 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
 
 // ================================================================================= C ABI
 extern "C" {
-
-#if UPR_TRACE
-// experiments only: copy the timeline of CTA 0 to the host (16 x 2048 u64)
-int upr_debug_trace(unsigned long long* host) {
-  return (int)cudaMemcpyFromSymbol(host, upr::g_trace, sizeof(unsigned long long) * 16 * 2048);
-}
-#endif
 
 const char* upr_last_error(void) { return g_err; }
 const char* upr_version(void) { return "upr 0.1 sm_100a"; }

@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 
 TOL_BF16 = 1e-2       # BASELINE.json north_star
 TOL_FP8 = 5e-2        # BASELINE.json north_star (against the PRE-quantisation inputs)
-TOL_STRICT = 5e-3     # self-imposed (SURVEY.md 8(c) "warning on the tolerance"); bf16 P rounding bounds it
+TOL_STRICT = 5e-3     # self-imposed; derived in DESIGN.md section 6 (bf16 rounding of P: 2^-9 max|v|, few-key rows)
 TOL_RMS = 1e-2
 
 
@@ -142,6 +142,7 @@ FP8_CASES = [
     ("fp8_ragged_d128", [1, 15, 16, 17, 127, 129, 300, 640], [1, 129, 256, 257, 600, 3, 128, 40], 2, 128, 2, False),
     ("fp8_self_empty", [0, 50, 0, 128, 1000], [3, 0, 130, 20, 300], 2, 64, 1, True),
     ("fp8_long_d128", [2500], [40], 1, 128, 1, True),
+    ("fp8_mid_histories", [300, 640, 999, 1000], [64, 130, 40, 64], 2, 64, 1, False),
 ]
 
 
@@ -153,16 +154,27 @@ def test_attention_fp8_cache_matches_oracle(P, case):
     w = S.custom_workload(name, 4343, L, C, H, d, layers, kv_dtype="fp8", self_term=self_on)
     inp = Inputs(w, "cuda")
     pre = oracle_all(inp)
-    # the 5e-2 contract is about quantisation noise averaged over a real history: a user with a
-    # handful of keys returns (nearly) one E4M3-rounded V row, whose own rounding step is up to
-    # 2^-4 |v| ~ 0.25 -- so the pre-quantisation bar is asserted for users with L_b >= 1000 only (noise ~ 1/sqrt(L_b); measured 0.052 at L_b = 300)
-    rows = np.concatenate([np.arange(w.cand_offsets[b], w.cand_offsets[b + 1]) for b in range(w.B)
-                           if w.seq_lens[b] >= 1000] + [np.zeros(0, dtype=np.int64)]).astype(np.int64)
+    # DESIGN.md section 6, reading T2: north_star's 5e-2 (against the PRE-quantisation inputs) is a
+    # statement about quantisation noise averaged over a real history.  A user with a handful of keys
+    # returns (nearly) one E4M3-rounded V row whose own rounding step is up to 2^-4 |v| ~ 0.25, so the
+    # bar is asserted where the noise has averaged out (L_b >= 1000); histories of 300..999 keys are
+    # held to the measured bound 8e-2 (0.052 at L_b = 300) so that a regression there stays visible.
+    # EVERY row is held to TOL_STRICT against the oracle fed the dequantised values.
+    def rows_of(lo, hi):
+        return np.concatenate([np.arange(w.cand_offsets[b], w.cand_offsets[b + 1]) for b in range(w.B)
+                               if lo <= w.seq_lens[b] < hi] + [np.zeros(0, dtype=np.int64)]).astype(np.int64)
+    long_rows, mid_rows = rows_of(1000, 1 << 30), rows_of(300, 1000)
     for ns in (1, 3):
         got, _, _ = run_cuda(P, inp, num_splits=ns)
         check(got, oracle_all(inp, dequant=True))
-        mx, _ = error_stats(got[:, rows], pre[:, rows])
-        assert mx <= TOL_FP8, mx
+        if long_rows.size:
+            mx, _ = error_stats(got[:, long_rows], pre[:, long_rows])
+            assert mx <= TOL_FP8, mx
+        if mid_rows.size:
+            mx, _ = error_stats(got[:, mid_rows], pre[:, mid_rows])
+            assert mx <= 8e-2, mx
+    if not long_rows.size and not mid_rows.size:
+        print("no history of >= 300 keys in this case: pre-quantisation bar not applicable (DESIGN.md 6, T2)")
 
 
 def test_fp8_decode_is_exact_for_every_code(P):
@@ -306,6 +318,36 @@ def test_baseline_configs_full_size_sampled(P, cfg):
             mx_pre, _ = error_stats(got[l, co[b]:co[b + 1], h], oracle_block(inp, l, b, h))
             assert mx_pre <= TOL_FP8, (b, l, h, mx_pre)
     assert worst <= TOL_BF16
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_baseline_configs_full_size_all_rows(P, cfg):
+    """Full BASELINE.json sizes in the launch configuration bench.py times, EVERY output row against the
+    oracle: one OpenMP call of oracle.cross_attn_pool per layer (plain indexing of the same pool the
+    CUDA pack read; pinned against pack-then-attend in tests/test_oracle_pins.py).  A scheduler fault
+    that hits one work item in a thousand cannot hide here.  (Config 4 stays sampled: the oracle's
+    E4M3 pack is a nearest-code search, ~0.1 us per element.)"""
+    w = S.workload(cfg)
+    inp = Inputs(w, "cuda")
+    got, _, _ = run_cuda(P, inp, num_splits=0)
+    assert np.all(np.isfinite(got))
+    worst, sq_err, sq_ref = 0.0, 0.0, 0.0
+    for l in range(w.n_layers):
+        kw = {}
+        if w.self_term:
+            kw = dict(kself=bits(inp.k_self[l:l + 1]), vself=bits(inp.v_self[l:l + 1]))
+        want = oracle.cross_attn_pool(bits(inp.q[l:l + 1]), oracle.BF16, bits(inp.k_pool[l:l + 1]),
+                                      bits(inp.v_pool[l:l + 1]), inp.slot_ids_host, w.seq_lens, w.cand_offsets,
+                                      w.H, **kw)[0]
+        diff = np.abs(got[l].astype(np.float64) - want)
+        worst = max(worst, float(diff.max()))
+        sq_err += float((diff ** 2).sum())
+        sq_ref += float((want ** 2).sum())
+        bad = np.argwhere(diff > TOL_STRICT)
+        assert bad.size == 0, f"layer {l}: {len(bad)} elements off, first (row, head, t) = {bad[0]}, {diff.max()}"
+    rel = (sq_err / sq_ref) ** 0.5
+    print(f"cfg {cfg}: all {w.n_layers * w.total_q * w.H} rows, max-abs {worst:.2e} rel-rms {rel:.2e}")
+    assert worst <= TOL_STRICT and rel <= TOL_RMS
 
 
 @pytest.mark.parametrize("seed", range(8))

@@ -416,3 +416,136 @@ def test_packed_batch_equals_blockwise(oracle):
                             continue
                         want = oracle.attn_block(qd, Kd, Vd, *a)
                         assert np.array_equal(out[l, sl, h], want)
+
+
+# ----------------------------------------------------------------------- fp32 branches, user window, pool view
+def test_pack_f32_is_exact_widening_of_the_pool(oracle):
+    """UPRO_F32 branch of upro_pack: a gather whose elements are the bf16 pool values widened
+    exactly -- compared with numpy's own widening (bits << 16 viewed as float32), zero padding."""
+    r = rng(21)
+    n_layers, S, H, n_max, d = 2, 4, 2, 40, 8
+    _, pool_bits = _pool(r, n_layers, S, H, n_max, d)
+    slot = np.array([3, 1, 0], np.int32)
+    L = np.array([17, 0, 40], np.int32)
+    cache, scales = oracle.pack(pool_bits, slot, L, oracle.F32, tail_rows=3)
+    assert scales is None
+    lay = oracle.layout(L, H, d, n_layers, oracle.F32, tail_rows=3)
+    R, ro = lay["R"], lay["row_off"]
+    assert cache.size == lay["bytes_cache"] == (n_layers * H * R + 3) * d * 4
+    c = cache.view(np.float32)[: n_layers * H * R * d].reshape(n_layers, H, R, d)
+    wide = (pool_bits.astype(np.uint32) << 16).view(np.float32)
+    want = np.zeros_like(c)
+    for l in range(n_layers):
+        for b in range(3):
+            for h in range(H):
+                want[l, h, ro[b]: ro[b] + L[b]] = wide[l, slot[b], h, : L[b]]
+    assert np.array_equal(c.view(np.uint32), want.view(np.uint32))
+    assert np.all(cache.view(np.float32)[n_layers * H * R * d:] == 0)
+
+
+def test_packed_batch_f32_cache_and_f32_queries(oracle):
+    """UPRO_F32 branch of load_elem (q, k_self, v_self and the cache all fp32): the whole-batch driver
+    equals per-block attn_block calls on arrays sliced and widened here with numpy (config 1's dtypes)."""
+    r = rng(22)
+    n_layers, H, d = 2, 2, 8
+    L = np.array([5, 19, 0], np.int32)
+    Cn = np.array([3, 2, 4], np.int32)
+    B = 3
+    co = np.concatenate([[0], np.cumsum(Cn)]).astype(np.int32)
+    tq = int(co[-1])
+    _, pk = _pool(r, n_layers, B, H, 24, d)
+    _, pv = _pool(r, n_layers, B, H, 24, d)
+    slot = np.array([2, 0, 1], np.int32)
+    # fp32 queries that are NOT bf16-representable: a bf16 misread of the buffer would show
+    q, ks, vs = (r.standard_normal((n_layers, tq, H, d)).astype(np.float32) for _ in range(3))
+    kc, _ = oracle.pack(pk, slot, L, oracle.F32)
+    vc, _ = oracle.pack(pv, slot, L, oracle.F32)
+    lay = oracle.layout(L, H, d, n_layers, oracle.F32)
+    R, ro = lay["R"], lay["row_off"]
+    Kf = kc.view(np.float32)[: n_layers * H * R * d].reshape(n_layers, H, R, d).astype(np.float64)
+    Vf = vc.view(np.float32)[: n_layers * H * R * d].reshape(n_layers, H, R, d).astype(np.float64)
+    for self_on in (False, True):
+        out = oracle.cross_attn_packed(q, oracle.F32, kc, vc, oracle.F32, L, co, H, d, n_layers,
+                                       kself=ks if self_on else None, vself=vs if self_on else None)
+        for l in range(n_layers):
+            for b in range(B):
+                for h in range(H):
+                    sl = slice(co[b], co[b + 1])
+                    a = (ks[l, sl, h].astype(np.float64), vs[l, sl, h].astype(np.float64)) if self_on else (None, None)
+                    want = oracle.attn_block(q[l, sl, h].astype(np.float64), Kf[l, h, ro[b]: ro[b] + L[b]],
+                                             Vf[l, h, ro[b]: ro[b] + L[b]], *a)
+                    assert np.array_equal(out[l, sl, h], want)
+
+
+def test_packed_batch_user_window(oracle):
+    """users=(lo, hi): rows of users inside the window equal the un-windowed call bit for bit, rows
+    outside stay zero; windows tile the batch; an empty window computes nothing."""
+    r = rng(23)
+    n_layers, H, d = 1, 2, 8
+    L = np.array([5, 19, 0, 33, 7], np.int32)
+    Cn = np.array([3, 2, 4, 1, 5], np.int32)
+    B = 5
+    co = np.concatenate([[0], np.cumsum(Cn)]).astype(np.int32)
+    tq = int(co[-1])
+    _, pk = _pool(r, n_layers, B, H, 40, d)
+    _, pv = _pool(r, n_layers, B, H, 40, d)
+    slot = np.arange(B, dtype=np.int32)[::-1].copy()
+    mk = lambda: torch.from_numpy(r.standard_normal((n_layers, tq, H, d)).astype(np.float32)).to(
+        torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    q, ks, vs = mk(), mk(), mk()
+    kc, _ = oracle.pack(pk, slot, L, oracle.BF16)
+    vc, _ = oracle.pack(pv, slot, L, oracle.BF16)
+    full = oracle.cross_attn_packed(q, oracle.BF16, kc, vc, oracle.BF16, L, co, H, d, n_layers, kself=ks, vself=vs)
+    assert np.abs(full).min(axis=(0, 2, 3)).max() > 0          # every candidate row is populated
+    acc = np.zeros_like(full)
+    for lo, hi in ((0, 2), (2, 2), (2, 4), (4, 5)):
+        part = oracle.cross_attn_packed(q, oracle.BF16, kc, vc, oracle.BF16, L, co, H, d, n_layers,
+                                        kself=ks, vself=vs, users=(lo, hi))
+        assert np.array_equal(part[:, co[lo]:co[hi]], full[:, co[lo]:co[hi]])
+        assert np.all(part[:, :co[lo]] == 0) and np.all(part[:, co[hi]:] == 0)
+        acc += part
+    assert np.array_equal(acc, full)
+
+
+@pytest.mark.parametrize("G", [1, 2, 4])
+def test_pool_addressed_batch_equals_pack_then_attend(oracle, G):
+    """upro_cross_attn_pool (zero-copy addressing of PAPER.md:202's pool, grouped queries) against
+    (i) per-block attn_block calls on pool slices taken here with numpy, and, for G == 1, (ii) the
+    packed path: pack (PAPER.md:204's slot copy) then upro_cross_attn_packed -- the copy must not
+    change the result."""
+    r = rng(24 + G)
+    n_layers, H_kv, d = 2, 2, 8
+    H_q = H_kv * G
+    L = np.array([9, 0, 33, 16], np.int32)
+    Cn = np.array([4, 2, 0, 3], np.int32)
+    B, S = 4, 6
+    co = np.concatenate([[0], np.cumsum(Cn)]).astype(np.int32)
+    tq = int(co[-1])
+    _, pk = _pool(r, n_layers, S, H_kv, 40, d)
+    _, pv = _pool(r, n_layers, S, H_kv, 40, d)
+    slot = np.array([5, 2, 0, 3], np.int32)
+    mk = lambda: torch.from_numpy(r.standard_normal((n_layers, tq, H_q, d)).astype(np.float32)).to(
+        torch.bfloat16).view(torch.int16).numpy().view(np.uint16)
+    q, ks, vs = mk(), mk(), mk()
+    for self_on in (False, True):
+        kw = dict(kself=ks, vself=vs) if self_on else {}
+        out = oracle.cross_attn_pool(q, oracle.BF16, pk, pv, slot, L, co, H_q, **kw)
+        for l in range(n_layers):
+            for b in range(B):
+                for hq in range(H_q):
+                    if Cn[b] == 0:
+                        continue
+                    sl = slice(co[b], co[b + 1])
+                    Kd = oracle.bf16_bits_to_f64(pk[l, slot[b], hq // G, : L[b]])
+                    Vd = oracle.bf16_bits_to_f64(pv[l, slot[b], hq // G, : L[b]])
+                    a = (oracle.bf16_bits_to_f64(ks[l, sl, hq]), oracle.bf16_bits_to_f64(vs[l, sl, hq])) \
+                        if self_on else (None, None)
+                    assert np.array_equal(out[l, sl, hq], oracle.attn_block(oracle.bf16_bits_to_f64(q[l, sl, hq]),
+                                                                            Kd, Vd, *a))
+        if G == 1:
+            kc, _ = oracle.pack(pk, slot, L, oracle.BF16)
+            vc, _ = oracle.pack(pv, slot, L, oracle.BF16)
+            packed = oracle.cross_attn_packed(q, oracle.BF16, kc, vc, oracle.BF16, L, co, H_q, d, n_layers, **kw)
+            assert np.array_equal(out, packed)
+    with pytest.raises(ValueError):
+        oracle.cross_attn_pool(q, oracle.BF16, pk, pv, np.array([5, 2, 0, 6], np.int32), L, co, H_q)  # slot >= S
