@@ -215,58 +215,74 @@ def run_ours(args):
     v_self = S.gen_queries(w, "v_self", dev) if w.self_term else None
     k_pool, v_pool = S.gen_pool(w, "k_pool", dev), S.gen_pool(w, "v_pool", dev)
     slots = torch.as_tensor(S.slot_ids(w), device=dev)
+    # K/V source: bf16 workloads read the pool IN PLACE (zero copy: the slot copy of PAPER.md:204 is gone
+    # from the path); FP8 / fp32 caches need the pack (quantise / widen) and keep it in the step.
+    zero_copy = (args.kv_source == "pool") or (args.kv_source == "auto" and w.kv_dtype == "bf16")
+    if zero_copy and w.kv_dtype != "bf16":
+        raise SystemExit("--kv-source pool needs a bf16 workload (the pool is bf16)")
     cache = pl.alloc_cache(w.seq_lens, w.H, w.d, w.n_layers, kv_id, dev)
-    attn = pl.CrossAttention(cache, w.cand_offsets, q_id, num_splits=0)
+    attn_packed = pl.CrossAttention(cache, w.cand_offsets, q_id, num_splits=0)
+    view = pl.PoolView.of(k_pool, v_pool, slots, w.seq_lens)
+    attn = pl.CrossAttention(view, w.cand_offsets, q_id, num_splits=0) if zero_copy else attn_packed
     stream = torch.cuda.current_stream()
-
-    launches = [0]
-
-    def step(q_dev):
-        # a0: layout is integer-only host work, redone every step like a new batch would
-        P.upr_kv_cache_layout(w.seq_lens, w.H, w.d, w.n_layers, kv_id)
-        pl.pack_cache(cache, k_pool, v_pool, slots, stream)           # a1
-        launches[0] += P.upr_last_launch_count()
-        out = attn(q_dev, k_self, v_self, stream=stream)              # a2-a8
-        launches[0] += P.upr_last_launch_count()
-        return out
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step(q)
-    barrier()
+    def timed(attn_obj, packed: bool, steps: int, sample_clocks: bool):
+        """W warm-ups, then `steps` timed steps with per-kernel events; returns a dict."""
+        def one(marks=None):
+            n = 0
+            if marks:
+                marks[0].record(stream)
+            # a0: layout is integer-only host work, redone every step like a new batch would
+            P.upr_kv_cache_layout(w.seq_lens, w.H, w.d, w.n_layers, kv_id)
+            if packed:
+                pl.pack_cache(cache, k_pool, v_pool, slots, stream)           # a1
+                n += P.upr_last_launch_count()
+            if marks:
+                marks[1].record(stream)
+            attn_obj(q, k_self, v_self, stream=stream)                        # a2-a8
+            n += P.upr_last_launch_count()
+            if marks:
+                marks[2].record(stream)
+            return n
+        for _ in range(max(args.warmup, 3)):
+            one()
+        barrier()
+        e_start, e_end = ev(), ev()
+        marks = [(ev(), ev(), ev()) for _ in range(steps)]
+        sampler = ClockSampler(local_rank) if sample_clocks else None
+        if sampler:
+            sampler.start()
+        n_launch = 0
+        barrier()
+        e_start.record(stream)
+        for i in range(steps):
+            n_launch += one(marks[i])
+        e_end.record(stream)
+        barrier()
+        clocks = sampler.stop() if sampler else None
+        return {"total_ms": e_start.elapsed_time(e_end), "clocks": clocks, "launches": n_launch,
+                "pack_ms": float(np.mean([a.elapsed_time(b) for a, b, c in marks])),
+                "attn_ms": float(np.mean([b.elapsed_time(c) for a, b, c in marks]))}
 
-    # ---- device-resident timed region: K steps, per-kernel events inside
-    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
-    e_start, e_end = ev(), ev()
-    marks = [(ev(), ev(), ev()) for _ in range(args.steps)]
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    launches[0] = 0
-    barrier()
-    e_start.record(stream)
-    for i in range(args.steps):
-        a, b, c = marks[i]
-        a.record(stream)
-        P.upr_kv_cache_layout(w.seq_lens, w.H, w.d, w.n_layers, kv_id)
-        pl.pack_cache(cache, k_pool, v_pool, slots, stream)
-        launches[0] += P.upr_last_launch_count()
-        b.record(stream)
-        attn(q, k_self, v_self, stream=stream)
-        launches[0] += P.upr_last_launch_count()
-        c.record(stream)
-    e_end.record(stream)
-    barrier()
-    clocks = sampler.stop()
-    total_ms = e_start.elapsed_time(e_end)
-    pack_ms = float(np.mean([a.elapsed_time(b) for a, b, c in marks]))
-    attn_ms = float(np.mean([b.elapsed_time(c) for a, b, c in marks]))
+    main = timed(attn, not zero_copy, args.steps, True)
+    clocks, total_ms, pack_ms, attn_ms = main["clocks"], main["total_ms"], main["pack_ms"], main["attn_ms"]
+    launches = [main["launches"]]
     gpu_launches = launches[0]
     ms_step, units = aggregate_over_ranks(total_ms / args.steps, w.total_q, dist)
     value = units / (ms_step * 1e-3)
+    # the other variant of the same step (pack + attention over the packed cache), same run, for comparison
+    other = None
+    if zero_copy and not args.skip_packed_variant:
+        o = timed(attn_packed, True, args.steps, False)
+        o_ms, _ = aggregate_over_ranks(o["total_ms"] / args.steps, w.total_q, dist)
+        other = {"step": "layout + pack(pool->cache) + cross-attention", "ms_per_step": o_ms,
+                 "value": units / (o_ms * 1e-3), "pack_ms": o["pack_ms"], "attn_ms": o["attn_ms"]}
 
     # ---- end-to-end through the public API with HOST buffers (q in, out back), every step.
     # The copies are per layer on their own streams, so layer l+1's queries travel up while layer
@@ -284,12 +300,16 @@ def run_ours(args):
     lstride = int(cache.layout.layer_stride_bytes)
     layer_attn = []
     for l in range(w.n_layers):
-        sub = _dc.replace(cache, layout=lay1,
-                          k_cache=cache.k_cache[l * lstride: l * lstride + lay1.bytes_cache],
-                          v_cache=cache.v_cache[l * lstride: l * lstride + lay1.bytes_cache],
-                          k_scale=None if cache.k_scale is None else cache.k_scale[l * w.H:(l + 1) * w.H],
-                          v_scale=None if cache.v_scale is None else cache.v_scale[l * w.H:(l + 1) * w.H])
+        if zero_copy:
+            sub = _dc.replace(view, k_pool=k_pool[l:l + 1], v_pool=v_pool[l:l + 1])
+        else:
+            sub = _dc.replace(cache, layout=lay1,
+                              k_cache=cache.k_cache[l * lstride: l * lstride + lay1.bytes_cache],
+                              v_cache=cache.v_cache[l * lstride: l * lstride + lay1.bytes_cache],
+                              k_scale=None if cache.k_scale is None else cache.k_scale[l * w.H:(l + 1) * w.H],
+                              v_scale=None if cache.v_scale is None else cache.v_scale[l * w.H:(l + 1) * w.H])
         layer_attn.append(pl.CrossAttention(sub, w.cand_offsets, q_id, num_splits=0))
+    seq_dev = view.seq_lens if zero_copy else cache.seq_lens
     ev_h = [ev() for _ in range(w.n_layers)]
     ev_c = [ev() for _ in range(w.n_layers)]
 
@@ -299,12 +319,13 @@ def run_ours(args):
             for l in range(w.n_layers):
                 q_dev2[l].copy_(q_host[l], non_blocking=True)
                 ev_h[l].record(s_h2d)
-        cache.seq_lens.copy_(sl_host, non_blocking=True)
+        seq_dev.copy_(sl_host, non_blocking=True)
         for la in layer_attn:
             la.cand_offsets.copy_(co_host, non_blocking=True)
         P.upr_kv_cache_layout(w.seq_lens, w.H, w.d, w.n_layers, kv_id)            # a0
-        pl.pack_cache(cache, k_pool, v_pool, slots, stream)                       # a1
-        launches[0] += P.upr_last_launch_count()
+        if not zero_copy:
+            pl.pack_cache(cache, k_pool, v_pool, slots, stream)                   # a1
+            launches[0] += P.upr_last_launch_count()
         for l in range(w.n_layers):
             stream.wait_event(ev_h[l])
             out_l = layer_attn[l](q_dev2[l:l + 1],                                # a2-a8, layer l
@@ -358,8 +379,12 @@ def run_ours(args):
     # pack: read the valid pool rows (bf16) + write the cache rows; FP8 reads the pool twice (amax, quantise)
     pool_bytes = int(w.seq_lens.astype(np.int64).sum()) * w.H * w.d * w.n_layers * 2 * 2
     pack_bytes = pool_bytes * (2 if w.kv_dtype == "fp8" else 1) + w.kv_bytes
-    extra = {"pack_ms": pack_ms, "attn_ms": attn_ms, "pack_gbs": pack_bytes / (pack_ms * 1e-3) / 1e9,
-             "attn_candidates_per_s": w.total_q / (attn_ms * 1e-3), "splits": attn.splits}
+    extra = {"pack_ms": 0.0 if zero_copy else pack_ms, "attn_ms": attn_ms,
+             "pack_gbs": None if zero_copy else pack_bytes / (pack_ms * 1e-3) / 1e9,
+             "attn_candidates_per_s": w.total_q / (attn_ms * 1e-3), "splits": attn.splits,
+             "kv_source": "pool (zero copy)" if zero_copy else "packed decode cache",
+             "packed_variant": None if other is None else dict(
+                 other, pack_gbs=pack_bytes / (other["pack_ms"] * 1e-3) / 1e9)}
 
     # ---- CPU baseline: the oracle as it stands, bounded sample, host cores of this box
     cpu_baseline = None
@@ -377,7 +402,8 @@ def run_ours(args):
             "config": {"workload": w.name, "B": w.B, "H": w.H, "d": w.d, "layers": w.n_layers,
                        "total_candidates": w.total_q, "sum_history": int(w.seq_lens.sum()),
                        "kv_dtype": w.kv_dtype, "self_term": w.self_term,
-                       "step": "layout + pack(pool->cache) + cross-attention, all layers",
+                       "step": ("layout + cross-attention reading the pool in place (zero copy, no slot copy), all "
+                                "layers" if zero_copy else "layout + pack(pool->cache) + cross-attention, all layers"),
                        "l2": "inputs larger than L2 (K/V %.1f GB per step)" % (w.kv_bytes / 1e9),
                        "parallelism": "users sharded by rank, no collective" if world > 1 else "single GPU"},
             "clocks": clocks, "gpu_launches": gpu_launches,
@@ -396,6 +422,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="3")
+    ap.add_argument("--kv-source", default="auto", choices=["auto", "pool", "packed"],
+                    help="auto: bf16 workloads read the pool in place (zero copy), FP8/fp32 pack first")
+    ap.add_argument("--skip-packed-variant", action="store_true",
+                    help="leave out the secondary pack + attention leg of a zero-copy run")
     ap.add_argument("--skip-cpu-baseline", action="store_true",
                     help="leave out the oracle timing leg (used for the ncu captures under profiles/)")
     args = ap.parse_args()

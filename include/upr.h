@@ -53,6 +53,8 @@ typedef enum {
 } upr_status;
 
 typedef enum { UPR_F32 = 0, UPR_BF16 = 1, UPR_FP8_E4M3 = 2 } upr_dtype;
+typedef enum { UPR_KV_PACKED = 0, UPR_KV_POOL = 1 } upr_kv_source;
+typedef enum { UPR_KERNEL_AUTO = 0, UPR_KERNEL_SINGLE = 1, UPR_KERNEL_PAIR = 2 } upr_kernel_choice;
 
 #define UPR_ROW_ALIGN 16  /* rows; every user's block starts on a multiple of this */
 #define UPR_TAIL_ROWS 128 /* rows of slack after the last block (one TMA box) */
@@ -143,8 +145,30 @@ typedef struct upr_attn_params {
   float sm_scale;              /* softmax scale; 0 -> 1/sqrt(d) */
   int32_t num_splits;          /* split-K factor along the history; 0 -> heuristic, 1 -> off */
   int32_t max_seq_len;         /* hint for the heuristic (0 = unknown) */
-  void* workspace;             /* device, >= upr_cross_attn_workspace_bytes(), 256-B aligned */
+  void* workspace;             /* device, >= upr_cross_attn_workspace_bytes(), 256-B aligned; it holds the
+                                  scheduler state of ONE call: two calls in flight at the same time (on
+                                  different streams) must not share a workspace */
   size_t workspace_bytes;
+  /* --- fields below may be left zero: packed cache, H_kv = H, no size check ----------------- */
+  int32_t kv_source;           /* UPR_KV_PACKED (0): k_cache/v_cache are packed decode caches;
+                                  UPR_KV_POOL (1): k_cache/v_cache are the POOLS themselves, bf16
+                                  [n_layers, pool_slots, H_kv, pool_n_max, d], read in place --
+                                  no slot copy (the copy PAPER.md:204 / 278 pays for); kv_dtype must be BF16 */
+  int32_t pool_slots;          /* S      (UPR_KV_POOL only) */
+  int32_t pool_n_max;          /* n      (UPR_KV_POOL only); seq_lens[b] <= n */
+  int32_t H_kv;                /* KV heads ("KV heads"); 0 -> H.  H % H_kv == 0: query head hq
+                                  attends KV head hq / (H / H_kv) (grouped queries folded into M) */
+  const int32_t* slot_ids;     /* device int32 [B], each in [0, pool_slots) (UPR_KV_POOL only) */
+  int64_t kv_bytes;            /* size in bytes of EACH of k_cache / v_cache as allocated by the caller, or 0
+                                  = unchecked.  When set, a buffer shorter than the layout needs (pool:
+                                  n_layers*S*H_kv*n*d*2; packed cache with kv_rows set: layout.bytes_cache) is
+                                  refused with UPR_ERR_INVALID_ARG, and the bf16 K/V tensor maps are clipped
+                                  to it, so no TMA read ever leaves the allocation (rows beyond it read 0). */
+  int64_t kv_rows;             /* packed cache: layout.R of the cache (host copy), or 0 = unknown */
+  int32_t kernel;              /* UPR_KERNEL_AUTO (0): the library picks.  UPR_KERNEL_SINGLE (1) / UPR_KERNEL_PAIR
+                                  (2) force the 1-CTA kernel / the CTA-pair kernel (bf16 q and K/V, d = 128,
+                                  H / H_kv in {1,2,4,8}); a forced kernel that cannot run the arguments
+                                  returns UPR_ERR_UNSUPPORTED.  For tests and tuning. */
 } upr_attn_params;
 
 /* Bytes of workspace upr_cross_attn_fwd_ex needs for these params (dynamic-scheduler

@@ -1,0 +1,849 @@
+// attn2_kernel.cuh -- ranking-head cross-attention forward on a CTA PAIR (steps a2-a7 of
+// SURVEY.md 8(a)) for bf16 K/V, d = 128: the kernel the tensor-bound configs run on.
+//
+// Same mathematics as attn_kernel.cuh (out = softmax(scale * q K^T) V per candidate over its
+// user's cached history; optional self key/value), different mapping:
+//
+//  * a cluster of two CTAs (two SMs) owns a work item = (layer, user, KV head, history split,
+//    block of <= 256 query rows); each CTA holds ONE 128-row Q tile and its 128 lanes of TMEM;
+//    tcgen05.mma.cta_group::2 (M = 256) is issued by one thread of the pair's leader and runs on
+//    both SMs.  The B operand is split between the two CTAs' shared memories: for S = Q K^T each
+//    CTA streams HALF of every 128-key K tile (64 keys), for O += P V each CTA streams half of V's
+//    d columns -- every K/V byte enters the pair once, and per-CTA operand traffic halves.
+//  * S tiles are 128 keys wide (N = 128: the Q operand is re-read half as often as with the
+//    64-key sub-tiles of the 1-CTA kernel), two S buffers per CTA.
+//  * O is DOUBLE-BUFFERED (2 x 128 columns): the epilogue drains item n while the MMAs of item
+//    n+1 accumulate into the other buffer; S and PV issue run as one stream of key tiles across
+//    item boundaries (the S tile two ahead is issued behind each PV), so an item boundary costs
+//    no drain and no pipeline refill.
+//  * the two softmax warpgroups of a CTA work on the SAME 128 rows and take alternate key tiles;
+//    the running (max, sum) of a row lives in shared memory and is owned by whoever holds the
+//    "turn" (named barriers), which also keeps the two groups' MUFU phases in anti-phase.
+//  * grouped queries (H_kv < H_q, "KV heads"): the G = H_q / H_kv query heads that
+//    share a KV head are folded into M -- a tile holds 128/G candidates x G heads (g-major) --
+//    so a K/V tile is reused G times more often.
+//  * K/V come through one 2-D tensor map over [rows, d]: the packed decode cache, or the paper's
+//    pool [L, S, H_kv, n, D] read in place through slot_ids (zero copy).
+//  * work items are handed out longest-first from the tables upr_schedule_kernel builds.
+//
+// Roles per CTA (512 threads): warps 0-3 / 4-7 softmax groups, 8 producer (+ scheduler; the
+// leader's fetches the item index and forwards it to the peer), 9 MMA issuer (leader only), 10-11
+// self-logit helpers, 12-15 epilogue.  TMEM: S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512).
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include <cuda/std/type_traits>
+
+#include "ptx.cuh"
+
+namespace upr {
+namespace pair {
+
+constexpr int kD = 128;
+constexpr int kThreads = 512;
+constexpr int kRows = 128;            // query rows per CTA == TMEM lanes
+constexpr int kKeys = 128;            // keys per tile
+constexpr int kItemSlots = 4;
+constexpr int kKvSlots = 8;           // ring of half tiles: K0 V0 K1 V1 ...
+constexpr int kHalfBytes = 16384;     // K half: 64 keys x 128 d; V half: 128 keys x 64 d (bf16)
+constexpr int kKBoxBytes = 64 * 128;  // one [64 keys x 64 d] box of the K half
+constexpr int kQBoxBytes = kRows * 128;   // one [128 rows x 64 d] box of the Q tile
+constexpr int kQBytes = 2 * kQBoxBytes;
+constexpr int kEpiWarpBytes = 5120;   // 32 x 144 B rounded up to 1024 (see attn_kernel.cuh)
+constexpr int kEpiRowBytes = 144;
+constexpr int kSoftmaxRegs = 192;
+constexpr int kOtherRegs = 56;
+constexpr int kEpilogueRegs = 72;
+static_assert(256 * kSoftmaxRegs + 128 * kOtherRegs + 128 * kEpilogueRegs <= kThreads * 128,
+              "setmaxnreg budgets exceed the CTA's register allocation");
+constexpr int kProducerWarp = 8, kMmaWarp = 9, kHelpWarp0 = 10, kEpiWarp0 = 12;
+constexpr float kTau = 8.0f;          // lazy-rescale threshold, log2 units
+constexpr int kBarTurn0 = 1, kBarTurn1 = 2;   // named barriers: softmax group 0 / 1 may enter
+
+struct Args {
+  const void* q;          // bf16 [n_layers, total_q, H_q, 128]
+  const void* k_self;
+  const void* v_self;
+  float* out;             // fp32, same shape
+  const int32_t* seq_lens;
+  const int32_t* cand_offsets;
+  const int32_t* slot_ids;   // pool mode, else nullptr
+  const int32_t* iprefix;    // tables of upr_schedule_kernel
+  const int32_t* order;
+  const int32_t* rowoff;
+  unsigned int* counter;
+  float* part_o;          // split-K partials [n_layers][total_q][H_q][ns][128]
+  float* part_ml;         //                  [n_layers][total_q][H_q][ns][2]
+  int B, H_q, H_kv, G, cpt;  // cpt = 128 / G candidates per tile
+  int n_layers, num_splits;
+  int pool_S, pool_n;
+  int total_q;
+  int out_tma;
+  float scale_log2;
+};
+
+struct Item {
+  int valid;
+  int layer, hkv, split;
+  int c0;        // first candidate (global index) of the block
+  int cands;     // candidates in the block, 1 .. 2 * cpt
+  int kv_row0;   // row of the split's first key in the [rows, d] view of K / V
+  int n_keys;    // keys of the split's range (>= 0)
+};
+
+struct __align__(16) Ctrl {
+  uint64_t item_full[kItemSlots], item_empty[kItemSlots];
+  uint64_t idx_full[kItemSlots];   // peer: the leader's item index has landed in idx_ring
+  uint64_t idx_free[kItemSlots];   // leader: the peer has read idx_ring[slot] (remote arrive)
+  uint64_t kv_full[kKvSlots], kv_empty[kKvSlots];
+  uint64_t q_full[2], q_empty[2];
+  uint64_t s_full[2], p_full[2];
+  uint64_t pv_done;
+  uint64_t o_full[2], o_empty[2];
+  uint64_t l_ready[kItemSlots], self_full[kItemSlots];
+  Item items[kItemSlots];
+  uint32_t idx_ring[kItemSlots];
+  uint32_t tmem_base;
+  uint32_t pad_[3];
+  int mma_fifo[4][4];                      // MMA thread only: keyed items between its S and PV cursors
+  float m_sh[kRows], l_sh[kRows];          // running max (log2 units) / sum of the CTA's rows
+  float s_self[kItemSlots][kRows];         // self logits, log2 units
+  float epi_inv[kItemSlots][kRows];        // 1/l (1 for split-K partials)
+  float epi_wself[kItemSlots][kRows];      // weight of the candidate's own value row
+};
+constexpr int kSmemQ = 2 * kQBytes;                          //  65536
+constexpr int kSmemKV = kKvSlots * kHalfBytes;               // 131072
+constexpr int kSmemEpi = 4 * kEpiWarpBytes;                  //  20480
+constexpr int kSmemCtrl = 8192;
+constexpr int kSmemTotal = kSmemQ + kSmemKV + kSmemEpi + kSmemCtrl + 1024;
+static_assert(sizeof(Ctrl) <= kSmemCtrl, "control block too large");
+static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
+
+__host__ __device__ constexpr uint32_t idesc_pair(int N, int b_mn_major) {
+  return make_idesc_bf16(256, N, 0, b_mn_major);
+}
+
+// dot(q_row, kself_row), both bf16 rows of 128 in global memory
+__device__ __forceinline__ float row_dot128(const void* a, const void* b, size_t e) {
+  const uint4* pa = reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(a) + e);
+  const uint4* pb = reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(b) + e);
+  float acc = 0.f;
+#pragma unroll 4
+  for (int i = 0; i < kD / 8; ++i) {
+    const uint4 x = __ldg(pa + i), y = __ldg(pb + i);
+    const __nv_bfloat162* xs = reinterpret_cast<const __nv_bfloat162*>(&x);
+    const __nv_bfloat162* ys = reinterpret_cast<const __nv_bfloat162*>(&y);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const float2 fx = __bfloat1622float2(xs[k]), fy = __bfloat1622float2(ys[k]);
+      acc = fmaf(fx.x, fy.x, acc);
+      acc = fmaf(fx.y, fy.y, acc);
+    }
+  }
+  return acc;
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
+upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 128] bf16, box 64 keys x 64 d
+                     const __grid_constant__ CUtensorMap tmap_v,    // [rows, 128] bf16, box 128 keys x 64 d
+                     const __grid_constant__ CUtensorMap tmap_q,    // [n_layers*total_q, H_q*128], box cpt x 64
+                     const __grid_constant__ CUtensorMap tmap_out,  // fp32 [n_layers*total_q, H_q*128], box 32 x 32
+                     const Args args) {
+  extern __shared__ uint8_t smem_raw[];
+  const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  uint8_t* smem_aligned = smem_raw + (smem_base - smem_u32(smem_raw));
+  const uint32_t q_smem = smem_base;
+  const uint32_t kv_smem = q_smem + kSmemQ;
+  const uint32_t epi_smem = kv_smem + kSmemKV;
+  Ctrl* ctrl = reinterpret_cast<Ctrl*>(smem_aligned + kSmemQ + kSmemKV + kSmemEpi);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+  const uint32_t rank = cluster_ctarank();      // 0 = leader; this CTA owns tile `rank` of every item
+  const bool leader = rank == 0;
+  const bool has_self = args.k_self != nullptr;
+  const bool partial = args.num_splits > 1;
+  const int G = args.G, cpt = args.cpt;
+
+  // ------------------------------------------------------------------ one-time setup
+  if (threadIdx.x == 0) {
+    // readers that release an item slot: 8 softmax warps, 4 epilogue warps, 2 helper warps (self
+    // term only), the MMA thread (leader only)
+    const uint32_t readers = 8 + 4 + (has_self ? 2 : 0) + (leader ? 1 : 0);
+    for (int i = 0; i < kItemSlots; ++i) {
+      mbar_init(smem_u32(&ctrl->item_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->item_empty[i]), readers);
+      mbar_init(smem_u32(&ctrl->idx_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->idx_free[i]), 1);
+      mbar_init(smem_u32(&ctrl->l_ready[i]), 4);
+      mbar_init(smem_u32(&ctrl->self_full[i]), 2);
+    }
+    for (int i = 0; i < kKvSlots; ++i) {
+      mbar_init(smem_u32(&ctrl->kv_full[i]), 1);    // leader's arrive.expect_tx; bytes from both CTAs
+      mbar_init(smem_u32(&ctrl->kv_empty[i]), 1);   // multicast commit
+    }
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(smem_u32(&ctrl->q_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->q_empty[i]), 1);
+      mbar_init(smem_u32(&ctrl->s_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->p_full[i]), 8);     // 4 softmax warps of each CTA (leader's copy is used)
+      mbar_init(smem_u32(&ctrl->o_full[i]), 1);
+      mbar_init(smem_u32(&ctrl->o_empty[i]), 8);    // 4 epilogue warps of each CTA (leader's copy)
+    }
+    mbar_init(smem_u32(&ctrl->pv_done), 1);
+    fence_mbar_init();
+  }
+  if (warp == kProducerWarp && lane == 0) {
+    tma_prefetch_desc(&tmap_k);
+    tma_prefetch_desc(&tmap_v);
+    tma_prefetch_desc(&tmap_q);
+  }
+  if (warp == kMmaWarp) {
+    tmem_alloc_pair(smem_u32(&ctrl->tmem_base), 512);
+    tmem_relinquish_pair();
+  }
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();     // both CTAs' barriers are initialised before any remote arrive / TMA signal
+  tc_fence_after();
+  const uint32_t tmem_base = ctrl->tmem_base;
+
+  // Valid rows of this CTA's tile of an item: candidates [rank*cpt, rank*cpt + n_here) x G heads
+  auto cands_here = [&](const Item& it) { return max(0, min(cpt, it.cands - static_cast<int>(rank) * cpt)); };
+
+  if (warp == kProducerWarp) {
+    // ================================================================= scheduler + producer
+    setmaxnreg_dec<kOtherRegs>();
+    const int W = __ldg(args.iprefix + args.B);               // items per layer
+    const long long total_items = static_cast<long long>(W) * args.n_layers;
+    const int cpb = 2 * cpt;                                    // candidates per block
+    // barriers of the pair's leader, as shared::cluster addresses
+    const uint32_t lead_kv_full = mapa_shared(smem_u32(&ctrl->kv_full[0]), 0);
+    const uint32_t lead_q_full = mapa_shared(smem_u32(&ctrl->q_full[0]), 0);
+    const uint32_t peer_idx_full = mapa_shared(smem_u32(&ctrl->idx_full[0]), 1);
+    const uint32_t peer_idx_ring = mapa_shared(smem_u32(&ctrl->idx_ring[0]), 1);
+    const uint32_t lead_idx_free = mapa_shared(smem_u32(&ctrl->idx_free[0]), 0);
+    uint32_t kv_it = 0;      // ring position of the next half tile
+    uint32_t n_keyed = 0;    // items with keys so far (selects the Q buffer)
+    for (uint32_t n = 0;; ++n) {
+      const int islot = n & (kItemSlots - 1);
+      const uint32_t use = n / kItemSlots;
+      mbar_wait<1>(smem_u32(&ctrl->item_empty[islot]), (use & 1) ^ 1);
+      uint32_t idx = 0;
+      if (leader) {
+        if (lane == 0) {
+          idx = atomicAdd(args.counter, 1u);
+          // the peer must have read the previous index held by this ring slot (it may lag behind
+          // the leader by any number of key-less items, which need nothing from the pair)
+          if (use >= 1) mbar_wait_cluster(smem_u32(&ctrl->idx_free[islot]), (use - 1) & 1);
+          st_async_u32(peer_idx_ring + islot * 4, idx, peer_idx_full + islot * 8);
+        }
+        idx = __shfl_sync(0xffffffffu, idx, 0);
+      } else {
+        if (lane == 0) mbar_arrive_expect_tx(smem_u32(&ctrl->idx_full[islot]), 4);
+        mbar_wait<2>(smem_u32(&ctrl->idx_full[islot]), use & 1);
+        idx = ctrl->idx_ring[islot];
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(lead_idx_free + islot * 8);
+      }
+      if (static_cast<long long>(idx) >= total_items) {
+        if (lane == 0) {
+          ctrl->items[islot].valid = 0;
+          mbar_arrive(smem_u32(&ctrl->item_full[islot]));
+        }
+        break;
+      }
+      // ---- decode: position i in the longest-first order with iprefix[i] <= r < iprefix[i+1]
+      const int r = static_cast<int>(idx / static_cast<uint32_t>(args.n_layers));
+      int lo = 0, hi = args.B;   // invariant: iprefix[lo] <= r < iprefix[hi]
+      while (hi - lo > 1) {
+        const int step = (hi - lo + 31) / 32;
+        const int p = lo + lane * step;
+        const int v = (p < hi) ? __ldg(args.iprefix + p) : 0x7fffffff;
+        const unsigned le = __ballot_sync(0xffffffffu, v <= r);
+        const int c = __popc(le);            // lanes 0..c-1 satisfy (prefix is non-decreasing), c >= 1
+        const int nlo = lo + (c - 1) * step;
+        hi = min(hi, nlo + step);
+        lo = nlo;
+      }
+      const int p0 = __ldg(args.iprefix + lo);
+      const int w_user = __ldg(args.iprefix + lo + 1) - p0;                 // items per layer of this user
+      const int local_all = static_cast<int>(idx - static_cast<uint32_t>(args.n_layers) * static_cast<uint32_t>(p0));
+      const int layer = local_all / w_user;
+      const int local = local_all - layer * w_user;
+      const int b = __ldg(args.order + lo);
+      const int cb0 = __ldg(args.cand_offsets + b);
+      const int Cb = __ldg(args.cand_offsets + b + 1) - cb0;
+      const int Lb = __ldg(args.seq_lens + b);
+      const int nq = (Cb + cpb - 1) / cpb;
+      const int per_h = nq * args.num_splits;
+      const int hkv = local / per_h;
+      const int rem = local - hkv * per_h;
+      const int split = rem / nq;
+      const int qblk = rem - split * nq;
+      const int nt_user = (Lb + kKeys - 1) / kKeys;
+      const int t0 = static_cast<int>((static_cast<long long>(split) * nt_user) / args.num_splits);
+      const int t1 = static_cast<int>((static_cast<long long>(split + 1) * nt_user) / args.num_splits);
+      const int key0 = t0 * kKeys;
+      const int n_keys = (t1 > t0) ? (min(Lb, t1 * kKeys) - key0) : 0;
+      const int kv_row0 =
+          (args.slot_ids != nullptr)
+              ? ((layer * args.pool_S + __ldg(args.slot_ids + b)) * args.H_kv + hkv) * args.pool_n + key0
+              : (layer * args.H_kv + hkv) * __ldg(args.rowoff + args.B) + __ldg(args.rowoff + b) + key0;
+      if (lane == 0) {
+        Item& it = ctrl->items[islot];
+        it.valid = 1;
+        it.layer = layer;
+        it.hkv = hkv;
+        it.split = split;
+        it.c0 = cb0 + qblk * cpb;
+        it.cands = min(cpb, Cb - qblk * cpb);
+        it.kv_row0 = kv_row0;
+        it.n_keys = n_keys;
+        mbar_arrive(smem_u32(&ctrl->item_full[islot]));
+        const int nt = (n_keys + kKeys - 1) / kKeys;
+        if (nt > 0) {
+          // ---- this CTA's Q tile: G boxes of cpt candidates x 64 columns per 64-column half
+          const int qb = n_keyed & 1;
+          if (n_keyed >= 2) mbar_wait<3>(smem_u32(&ctrl->q_empty[qb]), ((n_keyed >> 1) - 1) & 1);
+          if (leader) mbar_arrive_expect_tx(smem_u32(&ctrl->q_full[qb]), 2 * kQBytes);
+          const int qrow = layer * args.total_q + it.c0 + static_cast<int>(rank) * cpt;
+          const uint32_t qdst = q_smem + qb * kQBytes;
+          for (int g = 0; g < G; ++g) {
+            const int col = (hkv * G + g) * kD;
+#pragma unroll
+            for (int bx = 0; bx < 2; ++bx)
+              tma_load_2d_pair(qdst + bx * kQBoxBytes + g * cpt * 128, &tmap_q, col + bx * 64, qrow,
+                               lead_q_full + qb * 8);
+          }
+          ++n_keyed;
+          // ---- K / V half tiles: K_j keys [64*rank, +64) of tile j; V_j columns [64*rank, +64)
+          for (int j = 0; j < nt; ++j) {
+#pragma unroll
+            for (int kv = 0; kv < 2; ++kv) {
+              const uint32_t slot = kv_it % kKvSlots;
+              const uint32_t ph = (kv_it / kKvSlots) & 1;
+              mbar_wait<4>(smem_u32(&ctrl->kv_empty[slot]), ph ^ 1);
+              if (leader) mbar_arrive_expect_tx(smem_u32(&ctrl->kv_full[slot]), 2 * kHalfBytes);
+              const uint32_t dst = kv_smem + slot * kHalfBytes;
+              const uint32_t bar = lead_kv_full + slot * 8;
+              if (kv == 0) {
+                const int row = kv_row0 + j * kKeys + static_cast<int>(rank) * 64;
+                tma_load_2d_pair(dst, &tmap_k, 0, row, bar);
+                tma_load_2d_pair(dst + kKBoxBytes, &tmap_k, 64, row, bar);
+              } else {
+                tma_load_2d_pair(dst, &tmap_v, static_cast<int>(rank) * 64, kv_row0 + j * kKeys, bar);
+              }
+              ++kv_it;
+            }
+          }
+        }
+      }
+      __syncwarp();
+    }
+  } else if (warp == kMmaWarp) {
+    // ================================================================= MMA issuer (leader)
+    // One stream of key tiles across items.  Per tile g (global count): S(g) = Q K_g^T into S
+    // buffer g & 1, later O += P(g) V_g.  S runs up to two tiles ahead of PV, across item
+    // boundaries, so the tensor pipe never waits for an item's epilogue or first loads.
+    setmaxnreg_dec<kOtherRegs>();
+    if (leader && elect_one()) {
+      constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);   // SBO 1024, version 1, SWIZZLE_128B
+      constexpr uint32_t kLoK = (16u >> 4) << 16;                               // K-major operands (Q, K)
+      constexpr uint32_t kLoMN = (1024u >> 4) << 16;                            // MN-major V half (one atom wide)
+      constexpr uint32_t kIdescS = idesc_pair(kKeys, 0);
+      constexpr uint32_t kIdescO = idesc_pair(kD, 1);
+      auto mk_desc = [](uint32_t lo) {
+        return (static_cast<uint64_t>(kDescHi) << 32) | static_cast<uint64_t>(lo);
+      };
+      const uint32_t q_lo = ((q_smem & 0x3FFFFu) >> 4) | kLoK;
+      const uint32_t kv_lo = (kv_smem & 0x3FFFFu) >> 4;
+      // S cursor
+      uint32_t s_item = 0;        // next item slot index the S cursor will look at
+      int s_nt = 0, s_j = 0;      // tiles of the S cursor's current item / next tile to issue
+      uint32_t s_kv = 0;          // ring position of the S cursor's current item's K_0
+      uint32_t s_keyed = 0;       // keyed items the S cursor has entered
+      bool s_end = false;
+      uint32_t gs = 0;            // global tiles S-issued
+      // PV cursor: a FIFO (shared memory, private to this thread) of the keyed items between the
+      // two cursors; the head entry is cached in registers
+      uint32_t f_head = 0, f_tail = 0;   // f_tail - f_head = keyed items entered by S and not finished by PV
+      int p_j = 0, p_nkeys = 0, p_slot = 0;
+      uint32_t p_kv = 0;
+      uint32_t gp = 0;            // global tiles PV-issued
+      uint32_t p_keyed = 0;       // keyed items the PV cursor has finished
+      uint32_t kv_next = 0;       // ring position after the last entered item
+      for (;;) {
+        // ---- 1. S issue: keep up to two tiles in flight ahead of PV
+        while (gs - gp < 2 && !s_end) {
+          if (s_j == s_nt) {
+            const int islot = s_item & (kItemSlots - 1);
+            const uint32_t par = (s_item / kItemSlots) & 1;
+            const uint32_t bar = smem_u32(&ctrl->item_full[islot]);
+            if (!mbar_test(bar, par)) {
+              if (gs != gp) break;      // PV work is pending: never block on the look-ahead
+              mbar_wait<5>(bar, par);
+            }
+            const Item& it = ctrl->items[islot];
+            if (!it.valid) {
+              s_end = true;
+              break;
+            }
+            const int nt = (it.n_keys + kKeys - 1) / kKeys;
+            ++s_item;
+            if (nt == 0) {              // key-less item: nothing for the tensor pipe
+              mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+              continue;
+            }
+            s_nt = nt;
+            s_j = 0;
+            s_kv = kv_next;
+            kv_next += 2 * nt;
+            const int fi = f_tail & 3;
+            ctrl->mma_fifo[fi][0] = it.n_keys;
+            ctrl->mma_fifo[fi][1] = islot;
+            ctrl->mma_fifo[fi][2] = static_cast<int>(s_kv);
+            ++f_tail;
+            const int qb = s_keyed & 1;
+            mbar_wait_cluster(smem_u32(&ctrl->q_full[qb]), (s_keyed >> 1) & 1);
+            ++s_keyed;
+          }
+          const int qb = (s_keyed - 1) & 1;
+          const uint32_t kpos = s_kv + 2 * s_j;
+          const uint32_t kslot = kpos % kKvSlots;
+          mbar_wait_cluster(smem_u32(&ctrl->kv_full[kslot]), (kpos / kKvSlots) & 1);
+          tc_fence_after();
+          const uint32_t sb = gs & 1;
+          const uint32_t a_lo = q_lo + ((qb * kQBytes) >> 4);
+          const uint32_t b_lo = kv_lo + kLoK + ((kslot * kHalfBytes) >> 4);
+#pragma unroll
+          for (int k = 0; k < kD / 16; ++k) {
+            const uint32_t a_off = ((k >> 2) * kQBoxBytes + (k & 3) * 32) >> 4;
+            const uint32_t b_off = ((k >> 2) * kKBoxBytes + (k & 3) * 32) >> 4;
+            umma_ss_pair(tmem_base + sb * kKeys, mk_desc(a_lo + a_off), mk_desc(b_lo + b_off), kIdescS, k > 0);
+          }
+          umma_commit_pair(smem_u32(&ctrl->s_full[sb]));
+          umma_commit_pair(smem_u32(&ctrl->kv_empty[kslot]));
+          ++s_j;
+          if (s_j == s_nt) umma_commit_pair(smem_u32(&ctrl->q_empty[qb]));   // Q buffer may be refilled
+          ++gs;
+        }
+        if (gs == gp) break;   // end of work and nothing pending
+        // ---- 2. PV for the oldest S tile
+        {
+          if (p_j == 0) {
+            const int fi = f_head & 3;
+            p_nkeys = ctrl->mma_fifo[fi][0];
+            p_slot = ctrl->mma_fifo[fi][1];
+            p_kv = static_cast<uint32_t>(ctrl->mma_fifo[fi][2]);
+          }
+          const int n_keys = p_nkeys;
+          const int nt = (n_keys + kKeys - 1) / kKeys;
+          const uint32_t ob = p_keyed & 1;
+          if (p_j == 0 && p_keyed >= 2)   // the epilogue must have drained this O buffer (item p_keyed - 2)
+            mbar_wait_cluster(smem_u32(&ctrl->o_empty[ob]), ((p_keyed >> 1) - 1) & 1);
+          const uint32_t sb = gp & 1;
+          mbar_wait_cluster(smem_u32(&ctrl->p_full[sb]), (gp >> 1) & 1);
+          const uint32_t vpos = p_kv + 2 * p_j + 1;
+          const uint32_t vslot = vpos % kKvSlots;
+          mbar_wait_cluster(smem_u32(&ctrl->kv_full[vslot]), (vpos / kKvSlots) & 1);
+          tc_fence_after();
+          const int ksteps = (min(kKeys, n_keys - p_j * kKeys) + 15) >> 4;
+          const uint32_t v_lo = kv_lo + kLoMN + ((vslot * kHalfBytes) >> 4);
+          const uint32_t tp = tmem_base + sb * kKeys;          // P(g): packed bf16 pairs over S(g)
+          const uint32_t to = tmem_base + 256 + ob * kD;
+#pragma unroll
+          for (int k = 0; k < kKeys / 16; ++k)
+            if (k < ksteps)
+              umma_ts_pair(to, tp + k * 8, mk_desc(v_lo + k * (2048 >> 4)), kIdescO, (p_j > 0 || k > 0) ? 1u : 0u);
+          umma_commit_pair(smem_u32(&ctrl->pv_done));
+          umma_commit_pair(smem_u32(&ctrl->kv_empty[vslot]));
+          ++gp;
+          ++p_j;
+          if (p_j == nt) {
+            umma_commit_pair(smem_u32(&ctrl->o_full[ob]));
+            mbar_arrive(smem_u32(&ctrl->item_empty[p_slot]));
+            ++f_head;
+            ++p_keyed;
+            p_j = 0;
+          }
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp == kHelpWarp0 || warp == kHelpWarp0 + 1) {
+    // ================================================================= self-logit helpers
+    // s_self = scale * <q_c, k_self_c> for the NEXT items' rows while the current one runs
+    setmaxnreg_dec<kOtherRegs>();
+    if (has_self) {
+      const int hw = warp - kHelpWarp0;
+      for (uint32_t n = 0;; ++n) {
+        const int islot = n & (kItemSlots - 1);
+        mbar_wait<6>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
+        const Item it = ctrl->items[islot];
+        if (!it.valid) break;
+        if (it.split == 0) {
+          const int nh = cands_here(it);
+#pragma unroll
+          for (int rr = 0; rr < 2; ++rr) {
+            const int row = hw * 64 + rr * 32 + lane;
+            const int g = row / cpt, cl = row - g * cpt;
+            float s = 0.f;
+            if (cl < nh) {
+              const size_t e = ((static_cast<size_t>(it.layer) * args.total_q + it.c0 + rank * cpt + cl) * args.H_q +
+                                it.hkv * G + g) * kD;
+              s = row_dot128(args.q, args.k_self, e) * args.scale_log2;
+            }
+            ctrl->s_self[islot][row] = s;
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(smem_u32(&ctrl->self_full[islot]));
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+      }
+    }
+  } else if (warp < 8) {
+    // ================================================================= softmax groups
+    setmaxnreg_inc<kSoftmaxRegs>();
+    const int wg = warp >> 2;                // this group takes the key tiles with (global index & 1) == wg
+    const int row = threadIdx.x & 127;       // row of the CTA's tile == TMEM lane
+    const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
+    const uint32_t tm_s = tmem_base + lane_base + wg * kKeys;     // S buffer wg
+    const uint32_t p_full_addr = mapa_shared(smem_u32(&ctrl->p_full[wg]), 0);   // the leader's barrier
+    const int turn_mine = wg == 0 ? kBarTurn0 : kBarTurn1;
+    const int turn_other = wg == 0 ? kBarTurn1 : kBarTurn0;
+    uint32_t g0 = 0;          // global key tiles before the current item
+    uint32_t my_tiles = 0;    // tiles this group has processed (phase of s_full[wg])
+    uint32_t n_keyed = 0;     // keyed items before the current one (O buffer)
+    uint32_t self_uses[kItemSlots] = {0, 0, 0, 0};
+    if (wg == 1) named_bar_arrive(kBarTurn0, 256);   // group 0 holds the first turn
+    for (uint32_t n = 0;; ++n) {
+      const int islot = n & (kItemSlots - 1);
+      mbar_wait<7>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
+      const Item it = ctrl->items[islot];
+      if (!it.valid) break;
+      const int nt = (it.n_keys + kKeys - 1) / kKeys;
+      const int nh = cands_here(it);
+      const int g = row / cpt, cl = row - g * cpt;
+      const bool row_valid = cl < nh;
+      const bool self_here = has_self && it.split == 0;
+      const uint32_t ob = n_keyed & 1;
+      const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD;
+      float s_self = 0.f;
+      if (self_here) {
+        mbar_wait<8>(smem_u32(&ctrl->self_full[islot]), self_uses[islot] & 1);
+        ++self_uses[islot];
+        s_self = ctrl->s_self[islot][row];
+      }
+      const size_t prow = ((static_cast<size_t>(it.layer) * args.total_q + it.c0 + rank * cpt + cl) * args.H_q +
+                           it.hkv * G + g) * args.num_splits + it.split;
+      // hand the row's final state to the epilogue (called by the group that closes the item)
+      auto finish = [&](float m_fin, float l_fin) {
+        ctrl->epi_inv[islot][row] = partial ? 1.0f : (l_fin > 0.f ? 1.0f / l_fin : 0.f);
+        ctrl->epi_wself[islot][row] = self_here ? ex2_approx(s_self - m_fin) : 0.f;
+        if (partial && row_valid) {
+          args.part_ml[prow * 2 + 0] = m_fin;
+          args.part_ml[prow * 2 + 1] = l_fin;
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(smem_u32(&ctrl->l_ready[islot]));
+      };
+      if (nt == 0) {
+        if (wg == 0 && nh > 0) finish(self_here ? s_self : -INFINITY, self_here ? 1.f : 0.f);
+      } else {
+        for (int j = 0; j < nt; ++j) {
+          if (static_cast<int>((g0 + j) & 1) != wg) continue;
+          const bool first = (j == 0), last = (j == nt - 1);
+          mbar_wait<9>(smem_u32(&ctrl->s_full[wg]), my_tiles & 1);
+          ++my_tiles;
+          tc_fence_after();
+          if (nh > 0) {
+            uint32_t sr[kKeys];
+#pragma unroll
+            for (int c0 = 0; c0 < kKeys; c0 += 32) tmem_ld32(tm_s + c0, &sr[c0]);
+            tmem_wait_ld_regs(sr);
+            const int keys_here = it.n_keys - j * kKeys;
+            if (last && keys_here < kKeys) {
+#pragma unroll
+              for (int c = 0; c < kKeys; ++c)
+                if (c >= keys_here) sr[c] = 0xff800000u;  // -inf
+            }
+            float mx0 = __uint_as_float(sr[0]), mx1 = __uint_as_float(sr[1]);
+            float mx2 = __uint_as_float(sr[2]), mx3 = __uint_as_float(sr[3]);
+#pragma unroll
+            for (int c = 4; c < kKeys; c += 4) {
+              mx0 = fmaxf(mx0, __uint_as_float(sr[c + 0]));
+              mx1 = fmaxf(mx1, __uint_as_float(sr[c + 1]));
+              mx2 = fmaxf(mx2, __uint_as_float(sr[c + 2]));
+              mx3 = fmaxf(mx3, __uint_as_float(sr[c + 3]));
+            }
+            const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * args.scale_log2;
+            // ---- exclusive section: this group owns the rows' running state and the MUFU phase
+            named_bar_sync(turn_mine, 256);
+            float m_used, l;
+            if (first) {
+              m_used = self_here ? s_self : -INFINITY;
+              l = self_here ? 1.f : 0.f;
+            } else {
+              m_used = ctrl->m_sh[row];
+              l = ctrl->l_sh[row];
+            }
+            const float m_new = fmaxf(m_used, mx);
+            const bool need = m_new > m_used + kTau;
+            if (first) {
+              // nothing accumulated in O yet (the first PV overwrites); only l may hold the self weight
+              if (need) {
+                l *= ex2_approx(m_used - m_new);
+                m_used = m_new;
+              }
+            } else if (__any_sync(0xffffffffu, need)) {
+              // PV(g-1) may still be accumulating into O: it is complete once pv_done has seen g tiles
+              const uint32_t gidx = g0 + j;
+              mbar_wait<10>(smem_u32(&ctrl->pv_done), (gidx - 1) & 1);
+              tc_fence_after();
+              const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
+#pragma unroll
+              for (int c0 = 0; c0 < kD; c0 += 16) {
+                uint32_t orr[16];
+                tmem_ld16(tm_o + c0, orr);
+                tmem_wait_ld_regs(orr);
+#pragma unroll
+                for (int c = 0; c < 16; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
+                tmem_st16(tm_o + c0, orr);
+              }
+              l *= alpha;
+              if (need) m_used = m_new;
+            }
+            float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
+            const float2 c2 = make_float2(args.scale_log2, args.scale_log2), nm2 = make_float2(-m_used, -m_used);
+#pragma unroll
+            for (int c0 = 0; c0 < kKeys; c0 += 32) {
+              uint32_t pr[16];
+#pragma unroll
+              for (int c = 0; c < 32; c += 4) {
+                const float2 x01 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 0]),
+                                                     __uint_as_float(sr[c0 + c + 1])), c2, nm2);
+                const float2 x23 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 2]),
+                                                     __uint_as_float(sr[c0 + c + 3])), c2, nm2);
+                const float p0 = ex2_approx(x01.x), p1 = ex2_approx(x01.y);
+                const float p2 = ex2_approx(x23.x), p3 = ex2_approx(x23.y);
+                const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
+                pr[(c >> 1) + 0] = w01;
+                pr[(c >> 1) + 1] = w23;
+                // the row sum adds the bf16-ROUNDED weights: out stays a convex combination of V rows
+                sumA = fadd2(sumA, make_float2(__uint_as_float(w01 << 16), __uint_as_float(w01 & 0xffff0000u)));
+                sumB = fadd2(sumB, make_float2(__uint_as_float(w23 << 16), __uint_as_float(w23 & 0xffff0000u)));
+              }
+              tmem_st16(tm_s + (c0 >> 1), pr);
+            }
+            l += (sumA.x + sumA.y) + (sumB.x + sumB.y);
+            if (!last) {
+              ctrl->m_sh[row] = m_used;
+              ctrl->l_sh[row] = l;
+            }
+            named_bar_arrive(turn_other, 256);
+            // ---- end of the exclusive section
+            tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(p_full_addr);
+            if (last) finish(m_used, l);
+          } else {
+            // this CTA's tile has no valid row for this item: keep the barriers moving
+            named_bar_sync(turn_mine, 256);
+            named_bar_arrive(turn_other, 256);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(p_full_addr);
+          }
+        }
+        g0 += nt;
+        ++n_keyed;
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+    }
+    // consume the last, unmatched turn hand-over so that no barrier is left half-arrived
+    if (static_cast<int>(g0 & 1) == wg) named_bar_sync(turn_mine, 256);
+  } else {
+    // ================================================================= epilogue group (a7)
+    setmaxnreg_dec<kEpilogueRegs>();
+    const int ew = warp - kEpiWarp0;                     // TMEM lane quarter of this warp
+    const uint32_t lane_base = static_cast<uint32_t>(ew * 32) << 16;
+    const uint32_t stage = epi_smem + ew * kEpiWarpBytes;
+    const uint32_t o_empty_addr = mapa_shared(smem_u32(&ctrl->o_empty[0]), 0);   // the leader's barriers
+    uint32_t n_keyed = 0;
+    uint32_t lr_uses[kItemSlots] = {0, 0, 0, 0};
+    for (uint32_t n = 0;; ++n) {
+      const int islot = n & (kItemSlots - 1);
+      mbar_wait<11>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
+      const Item it = ctrl->items[islot];
+      if (!it.valid) break;
+      const int nt = (it.n_keys + kKeys - 1) / kKeys;
+      const int nh = cands_here(it);
+      const bool self_here = has_self && it.split == 0;
+      const uint32_t ob = n_keyed & 1;
+      if (nh > 0) {
+        mbar_wait<12>(smem_u32(&ctrl->l_ready[islot]), lr_uses[islot] & 1);
+        ++lr_uses[islot];
+      }
+      if (nt > 0) {
+        mbar_wait<13>(smem_u32(&ctrl->o_full[ob]), (n_keyed >> 1) & 1);
+        tc_fence_after();
+      }
+      if (nh > 0) {
+        const int row = ew * 32 + lane;                  // row of this thread within the tile
+        const int g_own = row / cpt, cl_own = row - g_own * cpt;
+        const float inv = ctrl->epi_inv[islot][row];
+        const float ws = ctrl->epi_wself[islot][row] * inv;
+        const float2 sc2 = make_float2(inv, inv);
+        const int cand0 = it.c0 + static_cast<int>(rank) * cpt;       // first candidate of this CTA's tile
+        const size_t lrow0 = static_cast<size_t>(it.layer) * args.total_q;
+        const size_t se0 = ((lrow0 + cand0 + cl_own) * args.H_q + it.hkv * G + g_own) * kD;   // own row, candidate side
+        const bool add_self = self_here && cl_own < nh;
+        const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD;
+        // the warp's 32 rows are 32 consecutive candidates of one query head when cpt >= 32
+        const int g_w = (ew * 32) / cpt, cl_w = (ew * 32) - g_w * cpt;
+        const bool warp_full = cpt >= 32 && cl_w + 32 <= nh;
+        if (args.out_tma && !partial && nt > 0 && warp_full) {
+          // all 32 rows valid: each 32 x 32 block leaves through one TMA store from a swizzled box
+          const int grow = static_cast<int>(lrow0) + cand0 + cl_w;
+          const int gcol = (it.hkv * G + g_w) * kD;
+          const uint32_t sw_row = stage + lane * 128;
+          uint32_t orr[32];
+          tmem_ld32(tm_o, orr);
+#pragma unroll 1
+          for (int c0 = 0; c0 < kD; c0 += 32) {
+            tmem_wait_ld_regs(orr);
+            if (c0 + 32 == kD) {
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive_cluster(o_empty_addr + ob * 8);
+            }
+            if (lane == 0) bulk_wait_read_all();
+            __syncwarp();
+            if (!self_here) {
+#pragma unroll
+              for (int c = 0; c < 32; c += 4) {
+                const float2 a = fmul2(make_float2(__uint_as_float(orr[c]), __uint_as_float(orr[c + 1])), sc2);
+                const float2 b2 = fmul2(make_float2(__uint_as_float(orr[c + 2]), __uint_as_float(orr[c + 3])), sc2);
+                sts128(sw_row + (((c >> 2) ^ (lane & 7)) << 4), __float_as_uint(a.x), __float_as_uint(a.y),
+                       __float_as_uint(b2.x), __float_as_uint(b2.y));
+              }
+            } else {
+#pragma unroll
+              for (int c = 0; c < 32; c += 8) {
+                const uint4 x = __ldg(reinterpret_cast<const uint4*>(
+                    static_cast<const __nv_bfloat16*>(args.v_self) + se0 + c0 + c));
+                const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+                float o[8];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                  o[2 * k + 0] = fmaf(ws, __uint_as_float(w[k] << 16), __uint_as_float(orr[c + 2 * k]) * inv);
+                  o[2 * k + 1] = fmaf(ws, __uint_as_float(w[k] & 0xffff0000u), __uint_as_float(orr[c + 2 * k + 1]) * inv);
+                }
+                sts128(sw_row + (((c >> 2) ^ (lane & 7)) << 4), __float_as_uint(o[0]), __float_as_uint(o[1]),
+                       __float_as_uint(o[2]), __float_as_uint(o[3]));
+                sts128(sw_row + ((((c >> 2) + 1) ^ (lane & 7)) << 4), __float_as_uint(o[4]), __float_as_uint(o[5]),
+                       __float_as_uint(o[6]), __float_as_uint(o[7]));
+              }
+            }
+            if (c0 + 32 < kD) tmem_ld32(tm_o + c0 + 32, orr);   // next block: overlaps the store hand-off
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_2d(&tmap_out, stage, gcol + c0, grow);
+              bulk_commit();
+            }
+          }
+        } else {
+          // general path: ragged rows, split-K partials, key-less items, G > 4
+          if (lane == 0) bulk_wait_read_all();   // a TMA store of an earlier item may still read the block
+          __syncwarp();
+          // transposed read-back: 8 lanes cover one row's 128-byte line, 4 rows per access
+          const int rr = lane >> 3, cq = lane & 7;
+          const uint32_t st_w = stage + lane * kEpiRowBytes;
+          const uint32_t st_r = stage + rr * kEpiRowBytes + cq * 16;
+#pragma unroll 1
+          for (int c0 = 0; c0 < kD; c0 += 32) {
+            uint32_t orr[32];
+            if (nt > 0) {
+              tmem_ld32(tm_o + c0, orr);
+              tmem_wait_ld_regs(orr);
+              if (c0 + 32 == kD) {
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(o_empty_addr + ob * 8);
+              }
+            } else {
+#pragma unroll
+              for (int c = 0; c < 32; ++c) orr[c] = 0u;
+            }
+#pragma unroll
+            for (int c = 0; c < 32; c += 8) {
+              float sv[8];
+#pragma unroll
+              for (int k = 0; k < 8; ++k) sv[k] = 0.f;
+              if (add_self) {
+                const uint4 x = __ldg(reinterpret_cast<const uint4*>(
+                    static_cast<const __nv_bfloat16*>(args.v_self) + se0 + c0 + c));
+                const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                  sv[2 * k + 0] = __uint_as_float(w[k] << 16);
+                  sv[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+                }
+              }
+              float o[8];
+#pragma unroll
+              for (int k = 0; k < 8; ++k) o[k] = fmaf(ws, sv[k], __uint_as_float(orr[c + k]) * inv);
+              sts128(st_w + c * 4, __float_as_uint(o[0]), __float_as_uint(o[1]), __float_as_uint(o[2]),
+                     __float_as_uint(o[3]));
+              sts128(st_w + c * 4 + 16, __float_as_uint(o[4]), __float_as_uint(o[5]), __float_as_uint(o[6]),
+                     __float_as_uint(o[7]));
+            }
+            __syncwarp();
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const int r2 = ew * 32 + 4 * k + rr;       // tile row this lane group stores
+              const int g2 = r2 / cpt, cl2 = r2 - g2 * cpt;
+              if (cl2 < nh) {
+                const size_t orow = (lrow0 + cand0 + cl2) * args.H_q + it.hkv * G + g2;
+                float* dst = partial ? args.part_o + (orow * args.num_splits + it.split) * kD
+                                     : args.out + orow * kD;
+                stg128_stream(dst + c0 + cq * 4, lds128(st_r + k * (4 * kEpiRowBytes)));
+              }
+            }
+            __syncwarp();
+          }
+        }
+      } else if (nt > 0) {
+        // no valid row in this CTA's tile: the accumulator is handed straight back
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(o_empty_addr + ob * 8);
+      }
+      if (nt > 0) ++n_keyed;
+      __syncwarp();
+      if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
+    }
+    if (lane == 0) bulk_wait_all();   // outstanding TMA stores must land before the CTA retires
+  }
+
+  // ------------------------------------------------------------------ teardown
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();      // the peer may still signal this CTA's barriers / read its shared memory
+  if (warp == kMmaWarp) {
+    tc_fence_after();
+    tmem_dealloc_pair(tmem_base, 512);
+  }
+}
+
+}  // namespace pair
+}  // namespace upr

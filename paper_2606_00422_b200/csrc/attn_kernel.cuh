@@ -79,6 +79,8 @@ struct AttnArgs {
   float* part_o;          // split-K partial O~  [n_layers][total_q][H][ns][D]
   float* part_ml;         // split-K partial (m, l) [n_layers][total_q][H][ns][2]
   unsigned int* counter;  // dynamic work counter (zeroed before launch) or nullptr = static
+  const int32_t* slot_ids;  // non-null: K/V are read in place from the pool [n_layers, pool_S, H, pool_n, D]
+  int pool_S, pool_n;
   int B, H, n_layers, num_splits;
   int q_is_f32;
   int q_tma;              // 1: tmap_q describes `q` as [n_layers*total_q, H*D] bf16: the producer loads Q tiles by TMA
@@ -433,7 +435,12 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           static_cast<int>((static_cast<long long>(split + 1) * nt_user) / args.num_splits);
       const int key0 = t0 * kTileN;
       const int n_keys = (t1 > t0) ? (min(Lb, t1 * kTileN) - key0) : 0;
-      const int kv_row0 = (layer * args.H + h) * R + row_off_b + key0;
+      // base row of the (layer, user, head) block in the 2-D [rows, d] view of the K/V storage:
+      // packed cache [n_layers, H, R, d], or the pool itself [n_layers, S, H, n, d] (zero copy)
+      const int kv_row0 =
+          (args.slot_ids != nullptr)
+              ? ((layer * args.pool_S + __ldg(args.slot_ids + b)) * args.H + h) * args.pool_n + key0
+              : (layer * args.H + h) * R + row_off_b + key0;
       if (elect_one()) {
         WorkItem& it = ctrl->items[islot];
         it.valid = 1;

@@ -10,8 +10,10 @@
 #include <atomic>
 
 #include "../../include/upr.h"
+#include "attn2_kernel.cuh"
 #include "attn_kernel.cuh"
 #include "pack_kernels.cuh"
+#include "sched_kernel.cuh"
 
 namespace {
 
@@ -57,15 +59,17 @@ EncodeTiledFn get_encode_fn() {
   return f;
 }
 
-// 2-D bf16 view [rows, d] of a packed cache; box = [128 rows x 64 cols], 128-byte swizzle.
-// The row extent is left unbounded (the layout contract guarantees UPR_TAIL_ROWS of slack),
-// because R depends on device-resident seq_lens the host never reads.
-upr_status make_kv_tmap(CUtensorMap* m, const void* base, int d) {
+// 2-D bf16 view [rows, d] of a packed cache or of the pool; box = [box_rows x 64 cols], 128-byte
+// swizzle.  rows = 0: the extent is left unbounded (a packed cache's R depends on device-resident
+// seq_lens the host never reads; the layout contract guarantees UPR_TAIL_ROWS of slack); rows > 0
+// (pool, or a caller-stated buffer size): boxes are clipped there, rows beyond it read as zeros.
+upr_status make_kv_tmap(CUtensorMap* m, const void* base, int d, long long rows, int box_rows = 128) {
   EncodeTiledFn enc = get_encode_fn();
   if (enc == nullptr) return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
-  cuuint64_t gdim[2] = {static_cast<cuuint64_t>(d), static_cast<cuuint64_t>(1) << 31};
+  cuuint64_t gdim[2] = {static_cast<cuuint64_t>(d),
+                        rows > 0 ? static_cast<cuuint64_t>(rows) : static_cast<cuuint64_t>(1) << 31};
   cuuint64_t gstride[1] = {static_cast<cuuint64_t>(d) * 2};
-  cuuint32_t box[2] = {64, 128};
+  cuuint32_t box[2] = {64, static_cast<cuuint32_t>(box_rows)};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim, gstride,
                    box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -94,21 +98,52 @@ upr_status check_device() {
 
 constexpr size_t kCounterBytes = 256;
 
-int pick_splits(const upr_attn_params* p) {
+int kv_heads(const upr_attn_params* p) { return p->H_kv > 0 ? p->H_kv : p->H; }
+
+// Which attention kernel runs these arguments.  The CTA-pair kernel (attn2_kernel.cuh) takes the
+// tensor-bound shapes: bf16 q and K/V, d = 128, a workspace (the extended entry point), query
+// groups of 1/2/4/8, and on average more than one 128-row tile of (candidate, head) rows per user
+// -- below that its second CTA would idle and the 1-CTA kernel streams K/V at the HBM rate.
+bool pair_capable(const upr_attn_params* p) {
+  const int hkv = kv_heads(p);
+  const int G = hkv > 0 ? p->H / hkv : 0;
+  return p->d == 128 && p->kv_dtype == UPR_BF16 && p->q_dtype == UPR_BF16 &&
+         (G == 1 || G == 2 || G == 4 || G == 8) &&
+         static_cast<long long>(p->n_layers) * p->total_q < (1LL << 31);
+}
+
+constexpr bool kPairInAuto = false;   // flipped once the pair kernel is parity-green on the GPU
+
+bool use_pair(const upr_attn_params* p, bool have_workspace) {
+  if (!have_workspace || p->kernel == UPR_KERNEL_SINGLE || !pair_capable(p)) return false;
+  if (p->kernel == UPR_KERNEL_PAIR) return true;
+  if (!kPairInAuto) return false;
+  const int G = p->H / kv_heads(p);
+  if (G > 1) return true;   // grouped queries exist only in the pair kernel
+  return p->B > 0 && static_cast<long long>(p->total_q) * G > 128LL * p->B;
+}
+
+int pick_splits(const upr_attn_params* p, bool pair) {
   if (p->num_splits >= 1) return p->num_splits;
   // heuristic: split the history when the (user, head, q-block) items cannot fill the SMs
   if (p->max_seq_len <= 0 || p->total_q <= 0 || p->B <= 0) return 1;
   const int sms = sm_count() > 0 ? sm_count() : 148;
-  const long long blocks = (p->total_q + upr::kQBlock - 1) / upr::kQBlock + p->B / 2;
-  const long long items = blocks * p->H * p->n_layers;
+  const int units = pair ? sms / 2 : sms;   // CTA pairs or CTAs
+  const int G = p->H / kv_heads(p);
+  const int rows_per_block = upr::kQBlock / (pair ? G : 1);   // candidates per 256-row block
+  const long long blocks = (p->total_q + rows_per_block - 1) / rows_per_block + p->B / 2;
+  const long long items = blocks * kv_heads(p) * p->n_layers;
   const int tiles = (p->max_seq_len + upr::kTileN - 1) / upr::kTileN;
-  if (items >= 2LL * sms || tiles < 4) return 1;
-  long long want = (2LL * sms + items - 1) / items;
+  if (items >= 2LL * units || tiles < 4) return 1;
+  long long want = (2LL * units + items - 1) / items;
   long long cap = tiles / 2;  // at least two tiles per split
   long long ns = want < cap ? want : cap;
   if (ns > 16) ns = 16;
   return ns < 1 ? 1 : static_cast<int>(ns);
 }
+
+// workspace: [scheduler counter block][work-list tables: iprefix[B+1], order[B], rowoff[B+1]][split-K partials]
+size_t tables_bytes(int B) { return (static_cast<size_t>(3) * (B + 1) * sizeof(int32_t) + 255) / 256 * 256; }
 
 upr_status validate(const upr_attn_params* p) {
   if (p == nullptr) return fail(UPR_ERR_INVALID_ARG, "params is NULL");
@@ -130,6 +165,34 @@ upr_status validate(const upr_attn_params* p) {
     return fail(UPR_ERR_INVALID_ARG, "sm_scale must be >= 0 (0 selects 1/sqrt(d))");
   if (p->num_splits < 0 || p->num_splits > 64)
     return fail(UPR_ERR_INVALID_ARG, "num_splits=%d out of range [0,64]", p->num_splits);
+  if (p->H_kv < 0 || (p->H_kv > 0 && p->H % p->H_kv != 0))
+    return fail(UPR_ERR_INVALID_ARG, "H_kv=%d must divide H=%d", p->H_kv, p->H);
+  const int hkv = p->H_kv > 0 ? p->H_kv : p->H;
+  if (p->kv_bytes < 0 || p->kv_rows < 0) return fail(UPR_ERR_INVALID_ARG, "negative kv_bytes / kv_rows");
+  const long long row_bytes = static_cast<long long>(p->d) * elem_bytes(p->kv_dtype);
+  if (p->kv_source == UPR_KV_POOL) {
+    if (p->kv_dtype != UPR_BF16)
+      return fail(UPR_ERR_UNSUPPORTED, "the pool is bf16 (PAPER.md:202): kv_source = UPR_KV_POOL needs kv_dtype = UPR_BF16");
+    if (p->pool_slots <= 0 || p->pool_n_max <= 0)
+      return fail(UPR_ERR_INVALID_ARG, "bad pool shape S=%d n=%d", p->pool_slots, p->pool_n_max);
+    if (p->B > 0 && p->slot_ids == nullptr) return fail(UPR_ERR_INVALID_ARG, "slot_ids is NULL");
+    const long long rows = static_cast<long long>(p->n_layers) * p->pool_slots * hkv * p->pool_n_max;
+    if (rows >= (1LL << 31))
+      return fail(UPR_ERR_UNSUPPORTED, "pool has too many rows for 32-bit TMA coordinates");
+    if (p->kv_bytes > 0 && p->kv_bytes < rows * row_bytes)
+      return fail(UPR_ERR_INVALID_ARG, "pool buffer too short: %lld bytes stated, %lld needed",
+                  (long long)p->kv_bytes, rows * row_bytes);
+  } else if (p->kv_source == UPR_KV_PACKED) {
+    if (p->kv_bytes > 0 && p->kv_rows > 0) {
+      const long long need =
+          (static_cast<long long>(p->n_layers) * hkv * p->kv_rows + UPR_TAIL_ROWS) * row_bytes;
+      if (p->kv_bytes < need)
+        return fail(UPR_ERR_INVALID_ARG, "cache buffer too short: %lld bytes stated, %lld needed",
+                    (long long)p->kv_bytes, need);
+    }
+  } else {
+    return fail(UPR_ERR_INVALID_ARG, "kv_source %d unknown", p->kv_source);
+  }
   return UPR_OK;
 }
 
@@ -156,6 +219,127 @@ upr_status launch_attn_d(int kv_dtype, const upr::AttnArgs& a, const CUtensorMap
   }
 }
 
+// 2-D tensor map [rows, cols] of a row-major candidate-side tensor (q: bf16, out: fp32)
+bool make_cand_tmap(CUtensorMap* m, CUtensorMapDataType dt, int elem, const void* base, long long rows,
+                    long long cols, int box_cols, int box_rows, CUtensorMapL2promotion promo) {
+  EncodeTiledFn enc = get_encode_fn();
+  if (enc == nullptr) return false;
+  cuuint64_t gdim[2] = {static_cast<cuuint64_t>(cols), static_cast<cuuint64_t>(rows)};
+  cuuint64_t gstride[1] = {static_cast<cuuint64_t>(cols) * elem};
+  cuuint32_t box[2] = {static_cast<cuuint32_t>(box_cols), static_cast<cuuint32_t>(box_rows)};
+  cuuint32_t estr[2] = {1, 1};
+  return enc(m, dt, 2, const_cast<void*>(base), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+upr_status launch_combine(const float* part_o, const float* part_ml, float* out, long long out_rows, int ns,
+                          int d, cudaStream_t st) {
+  long long blocks = (out_rows + 7) / 8;
+  int cgrid = static_cast<int>(blocks < sm_count() * 8LL ? blocks : sm_count() * 8LL);
+  if (d == 64)
+    upr::upr_combine_kernel<64><<<cgrid, 256, 0, st>>>(part_o, part_ml, out, out_rows, ns);
+  else
+    upr::upr_combine_kernel<128><<<cgrid, 256, 0, st>>>(part_o, part_ml, out, out_rows, ns);
+  UPR_CUDA_CHECK(cudaGetLastError());
+  return UPR_OK;
+}
+
+// rows of the 2-D [rows, d] view of the K / V storage the tensor maps may touch (0 = unbounded)
+long long kv_view_rows(const upr_attn_params* p) {
+  long long rows = 0;
+  if (p->kv_source == UPR_KV_POOL)
+    rows = static_cast<long long>(p->n_layers) * p->pool_slots * kv_heads(p) * p->pool_n_max;
+  else if (p->kv_bytes > 0)
+    rows = p->kv_bytes / (static_cast<long long>(p->d) * 2);
+  return rows >= (1LL << 31) ? 0 : rows;
+}
+
+// ---- the CTA-pair kernel (bf16, d = 128): schedule tables -> attention [-> combine]
+upr_status run_attn_pair(const upr_attn_params* p, int ns, cudaStream_t st) {
+  const int hkv = kv_heads(p), G = p->H / hkv;
+  uint8_t* ws = static_cast<uint8_t*>(p->workspace);
+  int32_t* tables = reinterpret_cast<int32_t*>(ws + kCounterBytes);
+  const long long out_rows = static_cast<long long>(p->n_layers) * p->total_q * p->H;
+
+  upr::SchedArgs sa;
+  sa.seq_lens = p->seq_lens;
+  sa.cand_offsets = p->cand_offsets;
+  sa.counter = reinterpret_cast<unsigned int*>(ws);
+  sa.iprefix = tables;
+  sa.order = tables + (p->B + 1);
+  sa.rowoff = tables + 2 * (p->B + 1);
+  sa.B = p->B;
+  sa.H_kv = hkv;
+  sa.num_splits = ns;
+  sa.cands_per_block = 2 * (128 / G);
+  upr::upr_schedule_kernel<<<1, upr::kSchedThreads, 0, st>>>(sa);
+  UPR_CUDA_CHECK(cudaGetLastError());
+
+  upr::pair::Args a;
+  memset(&a, 0, sizeof(a));
+  a.q = p->q;
+  a.k_self = p->k_self;
+  a.v_self = p->v_self;
+  a.out = p->out;
+  a.seq_lens = p->seq_lens;
+  a.cand_offsets = p->cand_offsets;
+  a.slot_ids = (p->kv_source == UPR_KV_POOL) ? p->slot_ids : nullptr;
+  a.iprefix = sa.iprefix;
+  a.order = sa.order;
+  a.rowoff = sa.rowoff;
+  a.counter = sa.counter;
+  a.B = p->B;
+  a.H_q = p->H;
+  a.H_kv = hkv;
+  a.G = G;
+  a.cpt = 128 / G;
+  a.n_layers = p->n_layers;
+  a.num_splits = ns;
+  a.pool_S = p->pool_slots;
+  a.pool_n = p->pool_n_max;
+  a.total_q = static_cast<int>(p->total_q);
+  const float sm = p->sm_scale > 0.f ? p->sm_scale : 1.0f / sqrtf(static_cast<float>(p->d));
+  a.scale_log2 = sm * 1.4426950408889634f;
+  if (ns > 1) {
+    a.part_o = reinterpret_cast<float*>(ws + kCounterBytes + tables_bytes(p->B));
+    a.part_ml = a.part_o + static_cast<size_t>(out_rows) * ns * p->d;
+  }
+
+  CUtensorMap tk, tv, tq, to;
+  memset(&to, 0, sizeof(to));
+  const long long rows = kv_view_rows(p);
+  upr_status s = make_kv_tmap(&tk, p->k_cache, p->d, rows, /*box_rows=*/64);    // K half: 64 keys x 64 d boxes
+  if (s != UPR_OK) return s;
+  s = make_kv_tmap(&tv, p->v_cache, p->d, rows, /*box_rows=*/128);              // V half: 128 keys x 64 d
+  if (s != UPR_OK) return s;
+  const long long cand_rows = static_cast<long long>(p->n_layers) * p->total_q;
+  const long long cand_cols = static_cast<long long>(p->H) * p->d;
+  if (!make_cand_tmap(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p->q, cand_rows, cand_cols, 64, a.cpt,
+                      CU_TENSOR_MAP_L2_PROMOTION_L2_256B))
+    return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for q");
+  if (ns == 1 && make_cand_tmap(&to, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p->out, cand_rows, cand_cols, 32, 32,
+                                CU_TENSOR_MAP_L2_PROMOTION_NONE))
+    a.out_tma = 1;
+
+  // persistent grid: one CTA pair per SM pair, never more pairs than an upper bound on the item count
+  const int cpb = 2 * a.cpt;
+  long long max_items = ((p->total_q + cpb - 1) / cpb + p->B) * static_cast<long long>(hkv) * p->n_layers * ns;
+  int pairs = sm_count() / 2;
+  if (pairs <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
+  if (max_items < pairs) pairs = static_cast<int>(max_items < 1 ? 1 : max_items);
+  UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::pair::upr_attn_pair_kernel,
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, upr::pair::kSmemTotal));
+  upr::pair::upr_attn_pair_kernel<<<2 * pairs, upr::pair::kThreads, upr::pair::kSmemTotal, st>>>(tk, tv, tq, to, a);
+  UPR_CUDA_CHECK(cudaGetLastError());
+  g_launches = 2;
+  if (ns > 1) {
+    s = launch_combine(a.part_o, a.part_ml, p->out, out_rows, ns, p->d, st);
+    if (s != UPR_OK) return s;
+    g_launches = 3;
+  }
+  return UPR_OK;
+}
+
 upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t st) {
   g_launches = 0;
   upr_status s = validate(p);
@@ -164,7 +348,24 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   s = check_device();
   if (s != UPR_OK) return s;
 
-  const int ns = have_workspace ? pick_splits(p) : 1;
+  const bool pair = use_pair(p, have_workspace);
+  if (p->kernel == UPR_KERNEL_PAIR && !pair)
+    return fail(UPR_ERR_UNSUPPORTED, "the CTA-pair kernel needs bf16 q and K/V, d = 128, H/H_kv in {1,2,4,8}");
+  const int hkv = kv_heads(p);
+  if (!pair && hkv != p->H)
+    return fail(UPR_ERR_UNSUPPORTED,
+                "grouped queries (H_kv=%d < H=%d) need bf16 q and K/V, d = 128, H/H_kv in {2,4,8}", hkv, p->H);
+  const int ns = have_workspace ? pick_splits(p, pair) : 1;
+  if (have_workspace) {
+    const size_t need = upr_cross_attn_workspace_bytes(p);
+    if (p->workspace == nullptr || p->workspace_bytes < need)
+      return fail(UPR_ERR_WORKSPACE, "workspace too small: need %zu bytes, got %zu", need,
+                  p->workspace ? p->workspace_bytes : (size_t)0);
+    if ((reinterpret_cast<uintptr_t>(p->workspace) & 255) != 0)
+      return fail(UPR_ERR_WORKSPACE, "workspace must be 256-byte aligned");
+  }
+  if (pair) return run_attn_pair(p, ns, st);
+
   upr::AttnArgs a;
   memset(&a, 0, sizeof(a));
   a.q = p->q;
@@ -180,21 +381,20 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   a.n_layers = p->n_layers;
   a.num_splits = ns;
   a.q_is_f32 = (p->q_dtype == UPR_F32);
+  if (p->kv_source == UPR_KV_POOL) {
+    a.slot_ids = p->slot_ids;
+    a.pool_S = p->pool_slots;
+    a.pool_n = p->pool_n_max;
+  }
   const float sm = p->sm_scale > 0.f ? p->sm_scale : 1.0f / sqrtf(static_cast<float>(p->d));
   a.scale_log2 = sm * 1.4426950408889634f;
 
   const long long out_rows = static_cast<long long>(p->n_layers) * p->total_q * p->H;
   if (have_workspace) {
-    const size_t need = upr_cross_attn_workspace_bytes(p);
-    if (p->workspace == nullptr || p->workspace_bytes < need)
-      return fail(UPR_ERR_WORKSPACE, "workspace too small: need %zu bytes, got %zu", need,
-                  p->workspace ? p->workspace_bytes : (size_t)0);
-    if ((reinterpret_cast<uintptr_t>(p->workspace) & 255) != 0)
-      return fail(UPR_ERR_WORKSPACE, "workspace must be 256-byte aligned");
     a.counter = static_cast<unsigned int*>(p->workspace);
     UPR_CUDA_CHECK(cudaMemsetAsync(a.counter, 0, sizeof(unsigned int), st));
     if (ns > 1) {
-      uint8_t* w = static_cast<uint8_t*>(p->workspace) + kCounterBytes;
+      uint8_t* w = static_cast<uint8_t*>(p->workspace) + kCounterBytes + tables_bytes(p->B);
       a.part_o = reinterpret_cast<float*>(w);
       a.part_ml = a.part_o + static_cast<size_t>(out_rows) * ns * p->d;
     }
@@ -205,9 +405,10 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   memset(&tk, 0, sizeof(tk));
   memset(&tv, 0, sizeof(tv));
   if (p->kv_dtype == UPR_BF16) {
-    s = make_kv_tmap(&tk, p->k_cache, p->d);
+    const long long rows = kv_view_rows(p);
+    s = make_kv_tmap(&tk, p->k_cache, p->d, rows);
     if (s != UPR_OK) return s;
-    s = make_kv_tmap(&tv, p->v_cache, p->d);
+    s = make_kv_tmap(&tv, p->v_cache, p->d, rows);
     if (s != UPR_OK) return s;
   } else {
     if ((reinterpret_cast<uintptr_t>(p->k_cache) & 15) || (reinterpret_cast<uintptr_t>(p->v_cache) & 15))
@@ -225,39 +426,20 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   // CTAs without an item leave at once)
   if (have_workspace && max_items < grid) grid = static_cast<int>(max_items < 1 ? 1 : max_items);
 
-  // `out` as a 2-D fp32 tensor [n_layers * total_q, H * d] for the TMA stores of full tiles
-  // (needs the host copy of total_q: the extended entry point only)
-  CUtensorMap to;
+  // `out` / `q` as 2-D tensors [n_layers * total_q, H * d] for the TMA stores of full tiles and the
+  // TMA loads of Q tiles (need the host copy of total_q: the extended entry point only)
+  CUtensorMap to, tq;
   memset(&to, 0, sizeof(to));
-  if (have_workspace && ns == 1 && p->total_q > 0 &&
-      static_cast<long long>(p->n_layers) * p->total_q < (1LL << 31)) {
-    EncodeTiledFn enc = get_encode_fn();
-    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(p->H) * p->d,
-                          static_cast<cuuint64_t>(p->n_layers) * static_cast<cuuint64_t>(p->total_q)};
-    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(p->H) * p->d * sizeof(float)};
-    cuuint32_t box[2] = {32, 32};
-    cuuint32_t estr[2] = {1, 1};
-    if (enc != nullptr &&
-        enc(&to, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, p->out, gdim, gstride, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS)
-      a.out_tma = 1;
-  }
-  // `q` as a 2-D bf16 tensor [n_layers * total_q, H * d]: Q tiles by TMA (bf16 q and cache only)
-  CUtensorMap tq;
   memset(&tq, 0, sizeof(tq));
-  if (have_workspace && p->total_q > 0 && p->q_dtype == UPR_BF16 && p->kv_dtype == UPR_BF16 &&
-      static_cast<long long>(p->n_layers) * p->total_q < (1LL << 31)) {
-    EncodeTiledFn enc = get_encode_fn();
-    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(p->H) * p->d,
-                          static_cast<cuuint64_t>(p->n_layers) * static_cast<cuuint64_t>(p->total_q)};
-    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(p->H) * p->d * 2};
-    cuuint32_t box[2] = {64, 128};
-    cuuint32_t estr[2] = {1, 1};
-    if (enc != nullptr &&
-        enc(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(p->q), gdim, gstride, box, estr,
-            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS)
+  const long long cand_rows = static_cast<long long>(p->n_layers) * p->total_q;
+  const long long cand_cols = static_cast<long long>(p->H) * p->d;
+  if (have_workspace && cand_rows < (1LL << 31)) {
+    if (ns == 1 && make_cand_tmap(&to, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p->out, cand_rows, cand_cols, 32, 32,
+                                  CU_TENSOR_MAP_L2_PROMOTION_NONE))
+      a.out_tma = 1;
+    if (p->q_dtype == UPR_BF16 && p->kv_dtype == UPR_BF16 &&
+        make_cand_tmap(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p->q, cand_rows, cand_cols, 64, 128,
+                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B))
       a.q_tma = 1;
   }
   s = (p->d == 64) ? launch_attn_d<64>(p->kv_dtype, a, tk, tv, to, tq, grid, st)
@@ -265,13 +447,8 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   if (s != UPR_OK) return s;
   g_launches = 1;
   if (ns > 1) {
-    long long blocks = (out_rows + 7) / 8;
-    int cgrid = static_cast<int>(blocks < sm_count() * 8LL ? blocks : sm_count() * 8LL);
-    if (p->d == 64)
-      upr::upr_combine_kernel<64><<<cgrid, 256, 0, st>>>(a.part_o, a.part_ml, p->out, out_rows, ns);
-    else
-      upr::upr_combine_kernel<128><<<cgrid, 256, 0, st>>>(a.part_o, a.part_ml, p->out, out_rows, ns);
-    UPR_CUDA_CHECK(cudaGetLastError());
+    s = launch_combine(a.part_o, a.part_ml, p->out, out_rows, ns, p->d, st);
+    if (s != UPR_OK) return s;
     g_launches = 2;
   }
   return UPR_OK;
@@ -408,16 +585,16 @@ upr_status upr_cross_attn_fwd(const void* q, const void* k_cache, const void* v_
 }
 
 int upr_cross_attn_num_splits(const upr_attn_params* p) {
-  if (p == nullptr) return 1;
-  return pick_splits(p);
+  if (p == nullptr || p->H <= 0 || (p->H_kv > 0 && p->H % p->H_kv != 0)) return 1;
+  return pick_splits(p, use_pair(p, true));
 }
 
 size_t upr_cross_attn_workspace_bytes(const upr_attn_params* p) {
   if (p == nullptr || p->B < 0 || p->H <= 0 || p->n_layers <= 0 || p->total_q < 0 ||
-      (p->d != 64 && p->d != 128))
+      (p->d != 64 && p->d != 128) || (p->H_kv > 0 && p->H % p->H_kv != 0))
     return 0;
-  const int ns = pick_splits(p);
-  size_t bytes = kCounterBytes;
+  const int ns = pick_splits(p, use_pair(p, true));
+  size_t bytes = kCounterBytes + tables_bytes(p->B);
   if (ns > 1) {
     const size_t rows = static_cast<size_t>(p->n_layers) * p->total_q * p->H;
     bytes += rows * ns * (static_cast<size_t>(p->d) + 2) * sizeof(float);

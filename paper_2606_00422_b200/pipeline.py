@@ -51,31 +51,66 @@ def pack_cache(cache: DecodeCache, k_pool: torch.Tensor, v_pool: torch.Tensor, s
     return cache
 
 
+@dataclasses.dataclass
+class PoolView:
+    """The retrieval stage's KV pool ([L,S,H_kv,n,D] bf16) addressed IN PLACE for one
+    batch of users: no slot copy (the copy PAPER.md:204 / 278 pays for)."""
+    k_pool: torch.Tensor           # bf16 [n_layers, S, H_kv, n_max, d]
+    v_pool: torch.Tensor
+    slot_ids: torch.Tensor         # device int32 [B]
+    seq_lens: torch.Tensor         # device int32 [B]
+    max_seq_len: int
+
+    @staticmethod
+    def of(k_pool, v_pool, slot_ids, seq_lens_host) -> "PoolView":
+        sl = torch.as_tensor(np.asarray(seq_lens_host, dtype=np.int32), device=k_pool.device)
+        mx = int(np.max(seq_lens_host)) if len(seq_lens_host) else 0
+        return PoolView(k_pool, v_pool, slot_ids, sl, mx)
+
+
 class CrossAttention:
     """a2-a8 for a fixed problem shape: owns the output and workspace buffers."""
 
-    def __init__(self, cache: DecodeCache, cand_offsets_host, q_dtype: int = B_.UPR_BF16, num_splits: int = 0,
-                 device=None):
-        lay = cache.layout
+    def __init__(self, cache, cand_offsets_host, q_dtype: int = B_.UPR_BF16, num_splits: int = 0,
+                 device=None, H_q: Optional[int] = None, kernel: int = B_.UPR_KERNEL_AUTO):
+        """cache: a DecodeCache (packed) or a PoolView (zero copy).  H_q: query heads when they are a
+        multiple of the KV heads (grouped queries); default = the KV head count."""
         self.cache = cache
-        self.B, self.H, self.d, self.n_layers = lay.B, lay.H, lay.d, lay.n_layers
+        self.pool = isinstance(cache, PoolView)
+        if self.pool:
+            self.n_layers, S, self.H_kv, n_max, self.d = (int(x) for x in cache.k_pool.shape)
+            self.B = int(cache.seq_lens.shape[0])
+            self.kv_dtype = B_.UPR_BF16
+            self.kv_kwargs = dict(kv_source=B_.UPR_KV_POOL, pool_slots=S, pool_n_max=n_max,
+                                  slot_ids=cache.slot_ids,
+                                  kv_bytes=cache.k_pool.numel() * cache.k_pool.element_size())
+        else:
+            lay = cache.layout
+            self.B, self.H_kv, self.d, self.n_layers = lay.B, lay.H, lay.d, lay.n_layers
+            self.kv_dtype = lay.dtype
+            self.kv_kwargs = dict(kv_bytes=int(lay.bytes_cache), kv_rows=int(lay.R))
+        self.H = H_q or self.H_kv
+        self.kv_kwargs["H_kv"] = self.H_kv
+        self.kv_kwargs["kernel"] = kernel
         self.q_dtype = q_dtype
         co = np.asarray(cand_offsets_host, dtype=np.int32)
         self.total_q = int(co[-1])
-        device = device or cache.k_cache.device
+        device = device or cache.seq_lens.device
         self.cand_offsets = torch.as_tensor(co, device=device)
         self.num_splits = num_splits
         self.splits = B_.upr_cross_attn_num_splits(self.B, self.H, self.d, self.n_layers, self.total_q, num_splits,
-                                                   cache.max_seq_len)
+                                                   cache.max_seq_len, self.H_kv, self.kv_dtype, q_dtype, kernel)
         nbytes = B_.upr_cross_attn_workspace_bytes(self.B, self.H, self.d, self.n_layers, self.total_q, num_splits,
-                                                   cache.max_seq_len)
+                                                   cache.max_seq_len, self.H_kv, self.kv_dtype, q_dtype, kernel)
         self.workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
         self.out = torch.empty((self.n_layers, self.total_q, self.H, self.d), dtype=torch.float32, device=device)
 
     def __call__(self, q, k_self=None, v_self=None, sm_scale: float = 0.0, stream=None) -> torch.Tensor:
         c = self.cache
-        B_.upr_cross_attn_fwd_ex(q, c.k_cache, c.v_cache, c.seq_lens, self.cand_offsets, self.out, self.B, self.H,
-                                 self.d, self.n_layers, c.layout.dtype, self.q_dtype, self.total_q, self.workspace,
-                                 k_self, v_self, c.k_scale, c.v_scale, sm_scale, self.num_splits, c.max_seq_len,
-                                 stream)
+        k, v = (c.k_pool, c.v_pool) if self.pool else (c.k_cache, c.v_cache)
+        ks, vs = (None, None) if self.pool else (c.k_scale, c.v_scale)
+        B_.upr_cross_attn_fwd_ex(q, k, v, c.seq_lens, self.cand_offsets, self.out, self.B, self.H,
+                                 self.d, self.n_layers, self.kv_dtype, self.q_dtype, self.total_q, self.workspace,
+                                 k_self, v_self, ks, vs, sm_scale, self.num_splits, c.max_seq_len,
+                                 stream, **self.kv_kwargs)
         return self.out

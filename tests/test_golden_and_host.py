@@ -69,14 +69,17 @@ def test_host_layout_call_matches_oracle_without_a_gpu(oracle):
 
 def test_workspace_and_split_policy_are_host_only():
     import paper_2606_00422_b200 as P
-    # plenty of items: no split, workspace is just the scheduler counter block
+    # plenty of items: no split, workspace = scheduler counter block + work-list tables (3 x (B+1) int32,
+    # rounded up to 256 bytes)
+    def tables(B):
+        return (3 * (B + 1) * 4 + 255) // 256 * 256
     assert P.upr_cross_attn_num_splits(256, 8, 128, 4, 131072, 0, 2048) == 1
-    assert P.upr_cross_attn_workspace_bytes(256, 8, 128, 4, 131072, 0, 2048) == 256
+    assert P.upr_cross_attn_workspace_bytes(256, 8, 128, 4, 131072, 0, 2048) == 256 + tables(256)
     # one user, few candidates, long history: the heuristic splits the history
     ns = P.upr_cross_attn_num_splits(1, 2, 128, 1, 16, 0, 8192)
     assert ns > 1
     need = P.upr_cross_attn_workspace_bytes(1, 2, 128, 1, 16, 0, 8192)
-    assert need == 256 + 16 * 2 * ns * (128 + 2) * 4
+    assert need == 256 + tables(1) + 16 * 2 * ns * (128 + 2) * 4
     assert P.upr_cross_attn_num_splits(1, 2, 128, 1, 16, 3, 8192) == 3   # explicit request wins
 
 

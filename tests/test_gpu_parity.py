@@ -37,6 +37,17 @@ def run_cuda(P, inp: Inputs, num_splits=1, sm_scale=0.0):
     return out.cpu().numpy(), cache, attn
 
 
+def run_cuda_pool(P, inp: Inputs, num_splits=1, sm_scale=0.0):
+    """Zero-copy: the attention reads the pool in place through slot_ids (no pack, no decode cache)."""
+    from paper_2606_00422_b200 import pipeline as pl
+    w = inp.w
+    view = pl.PoolView.of(inp.k_pool, inp.v_pool, inp.slot_ids, w.seq_lens)
+    attn = pl.CrossAttention(view, w.cand_offsets, pl.DTYPE_ID[w.q_dtype], num_splits=num_splits)
+    out = attn(inp.q, inp.k_self, inp.v_self, sm_scale=sm_scale)
+    torch.cuda.synchronize()
+    return out.cpu().numpy(), attn
+
+
 def check(got, want, tol=TOL_BF16, strict=TOL_STRICT):
     assert np.all(np.isfinite(got))
     mx, rel = error_stats(got, want)
@@ -124,6 +135,51 @@ def test_attention_matches_oracle(P, case):
     got, _, _ = run_cuda(P, inp)
     want = oracle_all(inp)
     check(got, want)
+
+
+POOL_CASES = [c for c in CASES if c[0] in ("key_tail_d128", "ragged_mix", "ragged_mix_d128", "self_term_d128",
+                                            "empty_history_self", "long_history")]
+
+
+@pytest.mark.parametrize("case", POOL_CASES, ids=[c[0] for c in POOL_CASES])
+@pytest.mark.parametrize("ns", [1, 3])
+def test_zero_copy_pool_matches_packed_and_oracle(P, case, ns):
+    """K/V read in place from the paper's pool [L,S,H,n,D] == pack-then-attend
+     == oracle.  The pool's rows beyond L_b hold other random values (the generator fills
+    every row), so a tail-masking slip would show."""
+    name, L, C, H, d, layers, self_on = case
+    w = S.custom_workload(name, 4242, L, C, H, d, layers, self_term=self_on, n_max=max(L) + 37)
+    inp = Inputs(w, "cuda")
+    got_pool, attn = run_cuda_pool(P, inp, num_splits=ns)
+    assert attn.splits == ns
+    got_packed, _, _ = run_cuda(P, inp, num_splits=ns)
+    check(got_pool, oracle_all(inp))
+    mx, _ = error_stats(got_pool, got_packed.astype(np.float64))
+    assert mx <= 1e-6, f"pool mode differs from packed mode by {mx}"
+
+
+def test_zero_copy_rejects_bad_arguments(P):
+    from paper_2606_00422_b200 import pipeline as pl
+    w = S.custom_workload("poolerr", 1, [64, 10], [4, 4], 2, 64, 1, n_max=64)
+    inp = Inputs(w, "cuda")
+    view = pl.PoolView.of(inp.k_pool, inp.v_pool, inp.slot_ids, w.seq_lens)
+    attn = pl.CrossAttention(view, w.cand_offsets, P.UPR_BF16)
+    attn.kv_kwargs["kv_bytes"] = inp.k_pool.numel() * 2 - 2          # buffer stated one element short
+    with pytest.raises(P.UprError) as e:
+        attn(inp.q)
+    assert e.value.status == 1
+    attn.kv_kwargs["kv_bytes"] = 0
+    attn.kv_dtype = P.UPR_FP8_E4M3                                     # the pool is bf16
+    with pytest.raises(P.UprError) as e:
+        attn(inp.q)
+    assert e.value.status == 2
+    # packed cache stated shorter than its layout
+    cache = pl.alloc_cache(w.seq_lens, w.H, w.d, 1, P.UPR_BF16, "cuda")
+    a2 = pl.CrossAttention(cache, w.cand_offsets, P.UPR_BF16)
+    a2.kv_kwargs["kv_bytes"] = int(cache.layout.bytes_cache) - 128
+    with pytest.raises(P.UprError) as e:
+        a2(inp.q)
+    assert e.value.status == 1
 
 
 @pytest.mark.parametrize("ns", [2, 3, 7])
