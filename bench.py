@@ -221,9 +221,10 @@ def run_ours(args):
     if zero_copy and w.kv_dtype != "bf16":
         raise SystemExit("--kv-source pool needs a bf16 workload (the pool is bf16)")
     cache = pl.alloc_cache(w.seq_lens, w.H, w.d, w.n_layers, kv_id, dev)
-    attn_packed = pl.CrossAttention(cache, w.cand_offsets, q_id, num_splits=0)
+    kern = {"auto": P.UPR_KERNEL_AUTO, "single": P.UPR_KERNEL_SINGLE, "pair": P.UPR_KERNEL_PAIR}[args.kernel]
+    attn_packed = pl.CrossAttention(cache, w.cand_offsets, q_id, num_splits=0, kernel=kern)
     view = pl.PoolView.of(k_pool, v_pool, slots, w.seq_lens)
-    attn = pl.CrossAttention(view, w.cand_offsets, q_id, num_splits=0) if zero_copy else attn_packed
+    attn = pl.CrossAttention(view, w.cand_offsets, q_id, num_splits=0, kernel=kern) if zero_copy else attn_packed
     stream = torch.cuda.current_stream()
     ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
 
@@ -271,6 +272,7 @@ def run_ours(args):
                 "attn_ms": float(np.mean([b.elapsed_time(c) for a, b, c in marks]))}
 
     main = timed(attn, not zero_copy, args.steps, True)
+    attn_kernel_name = P.upr_last_attn_kernel()
     clocks, total_ms, pack_ms, attn_ms = main["clocks"], main["total_ms"], main["pack_ms"], main["attn_ms"]
     launches = [main["launches"]]
     gpu_launches = launches[0]
@@ -308,7 +310,7 @@ def run_ours(args):
                               v_cache=cache.v_cache[l * lstride: l * lstride + lay1.bytes_cache],
                               k_scale=None if cache.k_scale is None else cache.k_scale[l * w.H:(l + 1) * w.H],
                               v_scale=None if cache.v_scale is None else cache.v_scale[l * w.H:(l + 1) * w.H])
-        layer_attn.append(pl.CrossAttention(sub, w.cand_offsets, q_id, num_splits=0))
+        layer_attn.append(pl.CrossAttention(sub, w.cand_offsets, q_id, num_splits=0, kernel=kern))
     seq_dev = view.seq_lens if zero_copy else cache.seq_lens
     ev_h = [ev() for _ in range(w.n_layers)]
     ev_c = [ev() for _ in range(w.n_layers)]
@@ -364,7 +366,7 @@ def run_ours(args):
     t_flop = flops / (peaks["bf16_tflops"] * 1e12)
     t_mem = w.kv_bytes / (peaks["hbm_gbs"] * 1e9)
     roof_ms = 1e3 * max(t_flop, t_mem)
-    roofline = {"bound": "tensor" if t_flop >= t_mem else "hbm", "kernel": "upr_attn_fwd_kernel",
+    roofline = {"bound": "tensor" if t_flop >= t_mem else "hbm", "kernel": attn_kernel_name,
                 "achieved": tflops, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": tflops / peaks["bf16_tflops"],
                 # ncu counters cannot be read from inside an unprofiled run: the DRAM bytes of the ncu
@@ -424,6 +426,8 @@ def main():
     ap.add_argument("--config", default="3")
     ap.add_argument("--kv-source", default="auto", choices=["auto", "pool", "packed"],
                     help="auto: bf16 workloads read the pool in place (zero copy), FP8/fp32 pack first")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "single", "pair"],
+                    help="attention kernel: the library's choice, or force the 1-CTA / CTA-pair kernel (A/B runs)")
     ap.add_argument("--skip-packed-variant", action="store_true",
                     help="leave out the secondary pack + attention leg of a zero-copy run")
     ap.add_argument("--skip-cpu-baseline", action="store_true",

@@ -194,6 +194,10 @@ upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream);
 /* Kernel launches the last successful call on this thread enqueued (for accounting). */
 int upr_last_launch_count(void);
 
+/* Name of the attention kernel the last successful forward call on this thread launched:
+ * "upr_attn_pair_kernel" (CTA pairs, tcgen05 cta_group::2) or "upr_attn_fwd_kernel" (one CTA per SM). */
+const char* upr_last_attn_kernel(void);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* upr_last_error(void);
 

@@ -15,7 +15,7 @@ UPR_ROW_ALIGN, UPR_TAIL_ROWS = 16, 128
 EXPORTED_SYMBOLS = [
     "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
     "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
-    "upr_last_error", "upr_version",
+    "upr_last_error", "upr_version", "upr_last_attn_kernel",
 ]
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -72,6 +72,7 @@ def _load() -> ctypes.CDLL:
         lib.upr_last_error.restype = ctypes.c_char_p
         lib.upr_version.restype = ctypes.c_char_p
         lib.upr_last_launch_count.restype = ctypes.c_int
+        lib.upr_last_attn_kernel.restype = ctypes.c_char_p
         lib.upr_cross_attn_workspace_bytes.restype = ctypes.c_size_t
         lib.upr_cross_attn_workspace_bytes.argtypes = [ctypes.POINTER(_AttnParams)]
         lib.upr_cross_attn_num_splits.restype = ctypes.c_int
@@ -111,6 +112,10 @@ def _stream(stream) -> Optional[int]:
 
 def upr_version() -> str:
     return _load().upr_version().decode()
+
+
+def upr_last_attn_kernel() -> str:
+    return _load().upr_last_attn_kernel().decode()
 
 
 def upr_last_launch_count() -> int:

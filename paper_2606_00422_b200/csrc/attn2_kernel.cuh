@@ -55,14 +55,14 @@ constexpr int kQBoxBytes = kRows * 128;   // one [128 rows x 64 d] box of the Q 
 constexpr int kQBytes = 2 * kQBoxBytes;
 constexpr int kEpiWarpBytes = 5120;   // 32 x 144 B rounded up to 1024 (see attn_kernel.cuh)
 constexpr int kEpiRowBytes = 144;
-constexpr int kSoftmaxRegs = 192;
+constexpr int kSoftmaxRegs = 168;
 constexpr int kOtherRegs = 56;
-constexpr int kEpilogueRegs = 72;
+constexpr int kEpilogueRegs = 88;
 static_assert(256 * kSoftmaxRegs + 128 * kOtherRegs + 128 * kEpilogueRegs <= kThreads * 128,
               "setmaxnreg budgets exceed the CTA's register allocation");
 constexpr int kProducerWarp = 8, kMmaWarp = 9, kHelpWarp0 = 10, kEpiWarp0 = 12;
 constexpr float kTau = 8.0f;          // lazy-rescale threshold, log2 units
-constexpr int kBarTurn0 = 1, kBarTurn1 = 2;   // named barriers: softmax group 0 / 1 may enter
+constexpr int kBarMax = 1;            // named barrier of the 256 softmax threads (row-maximum exchange)
 
 struct Args {
   const void* q;          // bf16 [n_layers, total_q, H_q, 128]
@@ -101,8 +101,9 @@ struct __align__(16) Ctrl {
   uint64_t idx_free[kItemSlots];   // leader: the peer has read idx_ring[slot] (remote arrive)
   uint64_t kv_full[kKvSlots], kv_empty[kKvSlots];
   uint64_t q_full[2], q_empty[2];
-  uint64_t s_full[2], p_full[2];
-  uint64_t pv_done;
+  uint64_t s_full[2];
+  uint64_t p_full[2][2];           // [S buffer][half]: leader's copy collects both CTAs' arrivals
+  uint64_t pv_done[4];            // PV half-step hs completes phase hs / 4 of pv_done[hs % 4]
   uint64_t o_full[2], o_empty[2];
   uint64_t l_ready[kItemSlots], self_full[kItemSlots];
   Item items[kItemSlots];
@@ -110,15 +111,15 @@ struct __align__(16) Ctrl {
   uint32_t tmem_base;
   uint32_t pad_[3];
   int mma_fifo[4][4];                      // MMA thread only: keyed items between its S and PV cursors
-  float m_sh[kRows], l_sh[kRows];          // running max (log2 units) / sum of the CTA's rows
   float s_self[kItemSlots][kRows];         // self logits, log2 units
-  float epi_inv[kItemSlots][kRows];        // 1/l (1 for split-K partials)
+  float mx_sh[2][2][kRows];                // [S buffer][softmax group][row]: maximum of the group's 64 columns
+  float epi_l[kItemSlots][2][kRows];       // the two groups' partial row sums
   float epi_wself[kItemSlots][kRows];      // weight of the candidate's own value row
 };
 constexpr int kSmemQ = 2 * kQBytes;                          //  65536
 constexpr int kSmemKV = kKvSlots * kHalfBytes;               // 131072
 constexpr int kSmemEpi = 4 * kEpiWarpBytes;                  //  20480
-constexpr int kSmemCtrl = 8192;
+constexpr int kSmemCtrl = 11264;
 constexpr int kSmemTotal = kSmemQ + kSmemKV + kSmemEpi + kSmemCtrl + 1024;
 static_assert(sizeof(Ctrl) <= kSmemCtrl, "control block too large");
 static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
@@ -163,7 +164,9 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
-  const uint32_t rank = cluster_ctarank();      // 0 = leader; this CTA owns tile `rank` of every item
+  // rank in the CTA pair (cluster dims (2,1,1): == %cluster_ctarank; written from blockIdx so that the
+  // compiler knows it is warp-uniform: 0 = leader; this CTA owns tile `rank` of every item
+  const uint32_t rank = blockIdx.x & 1u;
   const bool leader = rank == 0;
   const bool has_self = args.k_self != nullptr;
   const bool partial = args.num_splits > 1;
@@ -179,7 +182,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       mbar_init(smem_u32(&ctrl->item_empty[i]), readers);
       mbar_init(smem_u32(&ctrl->idx_full[i]), 1);
       mbar_init(smem_u32(&ctrl->idx_free[i]), 1);
-      mbar_init(smem_u32(&ctrl->l_ready[i]), 4);
+      mbar_init(smem_u32(&ctrl->l_ready[i]), 8);
       mbar_init(smem_u32(&ctrl->self_full[i]), 2);
     }
     for (int i = 0; i < kKvSlots; ++i) {
@@ -190,11 +193,12 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       mbar_init(smem_u32(&ctrl->q_full[i]), 1);
       mbar_init(smem_u32(&ctrl->q_empty[i]), 1);
       mbar_init(smem_u32(&ctrl->s_full[i]), 1);
-      mbar_init(smem_u32(&ctrl->p_full[i]), 8);     // 4 softmax warps of each CTA (leader's copy is used)
+      mbar_init(smem_u32(&ctrl->p_full[i][0]), 8);  // 4 softmax warps of a group in each CTA (leader's copy is used)
+      mbar_init(smem_u32(&ctrl->p_full[i][1]), 8);
       mbar_init(smem_u32(&ctrl->o_full[i]), 1);
       mbar_init(smem_u32(&ctrl->o_empty[i]), 8);    // 4 epilogue warps of each CTA (leader's copy)
     }
-    mbar_init(smem_u32(&ctrl->pv_done), 1);
+    for (int i = 0; i < 4; ++i) mbar_init(smem_u32(&ctrl->pv_done[i]), 1);
     fence_mbar_init();
   }
   if (warp == kProducerWarp && lane == 0) {
@@ -294,7 +298,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
           (args.slot_ids != nullptr)
               ? ((layer * args.pool_S + __ldg(args.slot_ids + b)) * args.H_kv + hkv) * args.pool_n + key0
               : (layer * args.H_kv + hkv) * __ldg(args.rowoff + args.B) + __ldg(args.rowoff + b) + key0;
-      if (lane == 0) {
+      if (elect_one()) {   // (elect.sync: the compiler then issues the TMA instructions without a per-lane loop)
         Item& it = ctrl->items[islot];
         it.valid = 1;
         it.layer = layer;
@@ -351,7 +355,8 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
     // buffer g & 1, later O += P(g) V_g.  S runs up to two tiles ahead of PV, across item
     // boundaries, so the tensor pipe never waits for an item's epilogue or first loads.
     setmaxnreg_dec<kOtherRegs>();
-    if (leader && elect_one()) {
+    if (leader) {
+    if (elect_one()) {
       constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);   // SBO 1024, version 1, SWIZZLE_128B
       constexpr uint32_t kLoK = (16u >> 4) << 16;                               // K-major operands (Q, K)
       constexpr uint32_t kLoMN = (1024u >> 4) << 16;                            // MN-major V half (one atom wide)
@@ -447,20 +452,24 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
           if (p_j == 0 && p_keyed >= 2)   // the epilogue must have drained this O buffer (item p_keyed - 2)
             mbar_wait_cluster(smem_u32(&ctrl->o_empty[ob]), ((p_keyed >> 1) - 1) & 1);
           const uint32_t sb = gp & 1;
-          mbar_wait_cluster(smem_u32(&ctrl->p_full[sb]), (gp >> 1) & 1);
           const uint32_t vpos = p_kv + 2 * p_j + 1;
           const uint32_t vslot = vpos % kKvSlots;
-          mbar_wait_cluster(smem_u32(&ctrl->kv_full[vslot]), (vpos / kKvSlots) & 1);
-          tc_fence_after();
           const int ksteps = (min(kKeys, n_keys - p_j * kKeys) + 15) >> 4;
           const uint32_t v_lo = kv_lo + kLoMN + ((vslot * kHalfBytes) >> 4);
-          const uint32_t tp = tmem_base + sb * kKeys;          // P(g): packed bf16 pairs over S(g)
+          const uint32_t tp = tmem_base + sb * kKeys;          // P(g, h): packed bf16 pairs at columns 64 h + [0, 32)
           const uint32_t to = tmem_base + 256 + ob * kD;
 #pragma unroll
-          for (int k = 0; k < kKeys / 16; ++k)
-            if (k < ksteps)
-              umma_ts_pair(to, tp + k * 8, mk_desc(v_lo + k * (2048 >> 4)), kIdescO, (p_j > 0 || k > 0) ? 1u : 0u);
-          umma_commit_pair(smem_u32(&ctrl->pv_done));
+          for (int h = 0; h < 2; ++h) {
+            mbar_wait_cluster(smem_u32(&ctrl->p_full[sb][h]), (gp >> 1) & 1);
+            if (h == 0) mbar_wait_cluster(smem_u32(&ctrl->kv_full[vslot]), (vpos / kKvSlots) & 1);
+            tc_fence_after();
+#pragma unroll
+            for (int k = 4 * h; k < 4 * h + 4; ++k)
+              if (k < ksteps)
+                umma_ts_pair(to, tp + h * 64 + (k & 3) * 8, mk_desc(v_lo + k * (2048 >> 4)), kIdescO,
+                             (p_j > 0 || k > 0) ? 1u : 0u);
+            umma_commit_pair(smem_u32(&ctrl->pv_done[(2 * gp + h) & 3]));
+          }
           umma_commit_pair(smem_u32(&ctrl->kv_empty[vslot]));
           ++gp;
           ++p_j;
@@ -473,6 +482,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
           }
         }
       }
+    }
     }
     __syncwarp();
   } else if (warp == kHelpWarp0 || warp == kHelpWarp0 + 1) {
@@ -509,19 +519,25 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
     }
   } else if (warp < 8) {
     // ================================================================= softmax groups
+    // Both groups work on EVERY key tile of the CTA's 128 rows, two threads per row: group wg owns
+    // the tile's columns [64 wg, 64 wg + 64) -- 64 exponentials per thread and tile.  The row
+    // maximum is the one quantity the two threads of a row must share: each publishes the maximum
+    // of its half and reads its partner's after a 256-thread named barrier; both then take the same
+    // rescale decision, so the running maximum needs no further exchange.  Each thread keeps the
+    // row sum of its own columns (the epilogue adds the two) and rescales its own half of O's
+    // columns.  P(g, wg) is written over the group's OWN S columns (packed bf16 at columns
+    // 64 wg + [0, 32)), so neither group touches TMEM the other still reads.
+    // The two groups' exponential phases run CONCURRENTLY: the two warps that share an SM
+    // sub-partition are the two groups' warps of the same 32 rows, one warp alone reaches only half
+    // of the MUFU rate (measured: 64 ex2 in ~950 cycles against 512), two together saturate it.
     setmaxnreg_inc<kSoftmaxRegs>();
-    const int wg = warp >> 2;                // this group takes the key tiles with (global index & 1) == wg
+    const int wg = warp >> 2;
     const int row = threadIdx.x & 127;       // row of the CTA's tile == TMEM lane
     const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
-    const uint32_t tm_s = tmem_base + lane_base + wg * kKeys;     // S buffer wg
-    const uint32_t p_full_addr = mapa_shared(smem_u32(&ctrl->p_full[wg]), 0);   // the leader's barrier
-    const int turn_mine = wg == 0 ? kBarTurn0 : kBarTurn1;
-    const int turn_other = wg == 0 ? kBarTurn1 : kBarTurn0;
+    const uint32_t p_full_addr = mapa_shared(smem_u32(&ctrl->p_full[0][wg]), 0);   // the leader's barriers
     uint32_t g0 = 0;          // global key tiles before the current item
-    uint32_t my_tiles = 0;    // tiles this group has processed (phase of s_full[wg])
     uint32_t n_keyed = 0;     // keyed items before the current one (O buffer)
-    uint32_t self_uses[kItemSlots] = {0, 0, 0, 0};
-    if (wg == 1) named_bar_arrive(kBarTurn0, 256);   // group 0 holds the first turn
+    uint32_t self_par = 0;    // bit s: parity of the next self_full[s] phase to wait for
     for (uint32_t n = 0;; ++n) {
       const int islot = n & (kItemSlots - 1);
       mbar_wait<7>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
@@ -533,143 +549,146 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       const bool row_valid = cl < nh;
       const bool self_here = has_self && it.split == 0;
       const uint32_t ob = n_keyed & 1;
-      const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD;
+      const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD + wg * (kD / 2);   // own half of O's columns
       float s_self = 0.f;
       if (self_here) {
-        mbar_wait<8>(smem_u32(&ctrl->self_full[islot]), self_uses[islot] & 1);
-        ++self_uses[islot];
+        mbar_wait<8>(smem_u32(&ctrl->self_full[islot]), (self_par >> islot) & 1);
+        self_par ^= 1u << islot;
         s_self = ctrl->s_self[islot][row];
       }
-      const size_t prow = ((static_cast<size_t>(it.layer) * args.total_q + it.c0 + rank * cpt + cl) * args.H_q +
-                           it.hkv * G + g) * args.num_splits + it.split;
-      // hand the row's final state to the epilogue (called by the group that closes the item)
-      auto finish = [&](float m_fin, float l_fin) {
-        ctrl->epi_inv[islot][row] = partial ? 1.0f : (l_fin > 0.f ? 1.0f / l_fin : 0.f);
-        ctrl->epi_wself[islot][row] = self_here ? ex2_approx(s_self - m_fin) : 0.f;
-        if (partial && row_valid) {
-          args.part_ml[prow * 2 + 0] = m_fin;
-          args.part_ml[prow * 2 + 1] = l_fin;
+      // running state, log2 units; the self key (first split only) seeds it (its weight 1 is
+      // carried by group 0's partial sum)
+      float m_used = self_here ? s_self : -INFINITY;
+      float l = (self_here && wg == 0) ? 1.f : 0.f;
+      if (nh > 0) {
+        // One 128-key tile.  The last tile of an item (tail masking) is a separate instantiation so
+        // that the steady-state loop body stays small.
+        auto step = [&](const int j, auto last_tag) {
+          constexpr bool kLast = decltype(last_tag)::value;
+          const uint32_t gidx = g0 + j;
+          const uint32_t sb = gidx & 1;
+          const uint32_t tm_s = tmem_base + lane_base + sb * kKeys + wg * 64;   // own columns of S(g)
+          mbar_wait<9>(smem_u32(&ctrl->s_full[sb]), (gidx >> 1) & 1);
+          tc_fence_after();
+          uint32_t sr[64];
+          tmem_ld32(tm_s, &sr[0]);
+          tmem_ld32(tm_s + 32, &sr[32]);
+          tmem_wait_ld_regs(sr);
+          if (kLast) {
+            const int keys_mine = it.n_keys - j * kKeys - wg * 64;   // valid keys among this thread's columns
+#pragma unroll
+            for (int c = 0; c < 64; ++c)
+              if (c >= keys_mine) sr[c] = 0xff800000u;  // -inf
+          }
+          float mxa = fmax3(__uint_as_float(sr[0]), __uint_as_float(sr[1]), __uint_as_float(sr[2]));
+          float mxb = fmax3(__uint_as_float(sr[3]), __uint_as_float(sr[4]), __uint_as_float(sr[5]));
+          float mxc = fmaxf(__uint_as_float(sr[6]), __uint_as_float(sr[7]));
+          float mxd = -INFINITY;
+#pragma unroll
+          for (int c = 8; c < 64; c += 8) {
+            mxa = fmax3(mxa, __uint_as_float(sr[c + 0]), __uint_as_float(sr[c + 1]));
+            mxb = fmax3(mxb, __uint_as_float(sr[c + 2]), __uint_as_float(sr[c + 3]));
+            mxc = fmax3(mxc, __uint_as_float(sr[c + 4]), __uint_as_float(sr[c + 5]));
+            mxd = fmax3(mxd, __uint_as_float(sr[c + 6]), __uint_as_float(sr[c + 7]));
+          }
+          const float mx_mine = fmaxf(fmaxf(mxa, mxb), fmaxf(mxc, mxd));
+          ctrl->mx_sh[sb][wg][row] = mx_mine;
+          named_bar_sync(kBarMax, 256);
+          const float mx = fmaxf(mx_mine, ctrl->mx_sh[sb][wg ^ 1][row]) * args.scale_log2;
+          const float m_new = fmaxf(m_used, mx);
+          const bool need = m_new > m_used + kTau;
+          if (j == 0) {
+            // nothing accumulated in O yet (the first PV overwrites); only l may hold the self weight
+            if (need) {
+              l *= ex2_approx(m_used - m_new);
+              m_used = m_new;
+            }
+          } else if (__any_sync(0xffffffffu, need)) {
+            // the PV half-steps of the earlier tiles (hs < 2 g) may still be accumulating into O.
+            // Steps <= 2 g - 4 are complete (they were issued before S(g), which has been read); a
+            // ring of four barriers keeps the parity wait on step 2 g - 1 unambiguous even though
+            // this path is taken rarely.
+            const uint32_t hp = 2 * gidx - 1;
+            mbar_wait<10>(smem_u32(&ctrl->pv_done[hp & 3]), (hp >> 2) & 1);
+            tc_fence_after();
+            const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
+#pragma unroll
+            for (int c0 = 0; c0 < kD / 2; c0 += 16) {
+              uint32_t orr[16];
+              tmem_ld16(tm_o + c0, orr);
+              tmem_wait_ld_regs(orr);
+#pragma unroll
+              for (int c = 0; c < 16; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
+              tmem_st16(tm_o + c0, orr);
+            }
+            l *= alpha;
+            if (need) m_used = m_new;
+          }
+          float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
+          const float2 c2 = make_float2(args.scale_log2, args.scale_log2), nm2 = make_float2(-m_used, -m_used);
+#pragma unroll
+          for (int c0 = 0; c0 < 64; c0 += 32) {
+            uint32_t pr[16];
+#pragma unroll
+            for (int c = 0; c < 32; c += 4) {
+              const float2 x01 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 0]),
+                                                   __uint_as_float(sr[c0 + c + 1])), c2, nm2);
+              const float2 x23 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 2]),
+                                                   __uint_as_float(sr[c0 + c + 3])), c2, nm2);
+              const float p0 = ex2_approx(x01.x), p1 = ex2_approx(x01.y);
+              const float p2 = ex2_approx(x23.x), p3 = ex2_approx(x23.y);
+              const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
+              pr[(c >> 1) + 0] = w01;
+              pr[(c >> 1) + 1] = w23;
+              // the row sum adds the bf16-ROUNDED weights: out stays a convex combination of V rows
+              sumA = fadd2(sumA, make_float2(__uint_as_float(w01 << 16), __uint_as_float(w01 & 0xffff0000u)));
+              sumB = fadd2(sumB, make_float2(__uint_as_float(w23 << 16), __uint_as_float(w23 & 0xffff0000u)));
+            }
+            // P(g, wg): packed bf16 pairs over the group's own S columns
+            tmem_st16(tm_s + (c0 >> 1), pr);
+          }
+          l += (sumA.x + sumA.y) + (sumB.x + sumB.y);
+          tmem_wait_st();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(p_full_addr + sb * 16);
+        };
+        for (int j = 0; j + 1 < nt; ++j) step(j, cuda::std::false_type{});
+        if (nt > 0) step(nt - 1, cuda::std::true_type{});
+        // hand the row's final state to the epilogue: the two partial sums (added there), and from
+        // group 0 the weight of the candidate's own value row; split-K partial state by group 0
+        // once both sums are in shared memory
+        ctrl->epi_l[islot][wg][row] = l;
+        if (wg == 0) ctrl->epi_wself[islot][row] = self_here ? ex2_approx(s_self - m_used) : 0.f;
+        if (partial) {
+          named_bar_sync(kBarMax, 256);
+          if (wg == 0 && row_valid) {
+            const size_t prow = ((static_cast<size_t>(it.layer) * args.total_q + it.c0 + rank * cpt + cl) * args.H_q +
+                                 it.hkv * G + g) * args.num_splits + it.split;
+            args.part_ml[prow * 2 + 0] = m_used;
+            args.part_ml[prow * 2 + 1] = l + ctrl->epi_l[islot][1][row];
+          }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&ctrl->l_ready[islot]));
-      };
-      if (nt == 0) {
-        if (wg == 0 && nh > 0) finish(self_here ? s_self : -INFINITY, self_here ? 1.f : 0.f);
       } else {
+        // this CTA's tile has no valid row for this item: keep the pair's barriers moving
         for (int j = 0; j < nt; ++j) {
-          if (static_cast<int>((g0 + j) & 1) != wg) continue;
-          const bool first = (j == 0), last = (j == nt - 1);
-          mbar_wait<9>(smem_u32(&ctrl->s_full[wg]), my_tiles & 1);
-          ++my_tiles;
-          tc_fence_after();
-          if (nh > 0) {
-            uint32_t sr[kKeys];
-#pragma unroll
-            for (int c0 = 0; c0 < kKeys; c0 += 32) tmem_ld32(tm_s + c0, &sr[c0]);
-            tmem_wait_ld_regs(sr);
-            const int keys_here = it.n_keys - j * kKeys;
-            if (last && keys_here < kKeys) {
-#pragma unroll
-              for (int c = 0; c < kKeys; ++c)
-                if (c >= keys_here) sr[c] = 0xff800000u;  // -inf
-            }
-            float mx0 = __uint_as_float(sr[0]), mx1 = __uint_as_float(sr[1]);
-            float mx2 = __uint_as_float(sr[2]), mx3 = __uint_as_float(sr[3]);
-#pragma unroll
-            for (int c = 4; c < kKeys; c += 4) {
-              mx0 = fmaxf(mx0, __uint_as_float(sr[c + 0]));
-              mx1 = fmaxf(mx1, __uint_as_float(sr[c + 1]));
-              mx2 = fmaxf(mx2, __uint_as_float(sr[c + 2]));
-              mx3 = fmaxf(mx3, __uint_as_float(sr[c + 3]));
-            }
-            const float mx = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * args.scale_log2;
-            // ---- exclusive section: this group owns the rows' running state and the MUFU phase
-            named_bar_sync(turn_mine, 256);
-            float m_used, l;
-            if (first) {
-              m_used = self_here ? s_self : -INFINITY;
-              l = self_here ? 1.f : 0.f;
-            } else {
-              m_used = ctrl->m_sh[row];
-              l = ctrl->l_sh[row];
-            }
-            const float m_new = fmaxf(m_used, mx);
-            const bool need = m_new > m_used + kTau;
-            if (first) {
-              // nothing accumulated in O yet (the first PV overwrites); only l may hold the self weight
-              if (need) {
-                l *= ex2_approx(m_used - m_new);
-                m_used = m_new;
-              }
-            } else if (__any_sync(0xffffffffu, need)) {
-              // PV(g-1) may still be accumulating into O: it is complete once pv_done has seen g tiles
-              const uint32_t gidx = g0 + j;
-              mbar_wait<10>(smem_u32(&ctrl->pv_done), (gidx - 1) & 1);
-              tc_fence_after();
-              const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
-#pragma unroll
-              for (int c0 = 0; c0 < kD; c0 += 16) {
-                uint32_t orr[16];
-                tmem_ld16(tm_o + c0, orr);
-                tmem_wait_ld_regs(orr);
-#pragma unroll
-                for (int c = 0; c < 16; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
-                tmem_st16(tm_o + c0, orr);
-              }
-              l *= alpha;
-              if (need) m_used = m_new;
-            }
-            float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
-            const float2 c2 = make_float2(args.scale_log2, args.scale_log2), nm2 = make_float2(-m_used, -m_used);
-#pragma unroll
-            for (int c0 = 0; c0 < kKeys; c0 += 32) {
-              uint32_t pr[16];
-#pragma unroll
-              for (int c = 0; c < 32; c += 4) {
-                const float2 x01 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 0]),
-                                                     __uint_as_float(sr[c0 + c + 1])), c2, nm2);
-                const float2 x23 = ffma2(make_float2(__uint_as_float(sr[c0 + c + 2]),
-                                                     __uint_as_float(sr[c0 + c + 3])), c2, nm2);
-                const float p0 = ex2_approx(x01.x), p1 = ex2_approx(x01.y);
-                const float p2 = ex2_approx(x23.x), p3 = ex2_approx(x23.y);
-                const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
-                pr[(c >> 1) + 0] = w01;
-                pr[(c >> 1) + 1] = w23;
-                // the row sum adds the bf16-ROUNDED weights: out stays a convex combination of V rows
-                sumA = fadd2(sumA, make_float2(__uint_as_float(w01 << 16), __uint_as_float(w01 & 0xffff0000u)));
-                sumB = fadd2(sumB, make_float2(__uint_as_float(w23 << 16), __uint_as_float(w23 & 0xffff0000u)));
-              }
-              tmem_st16(tm_s + (c0 >> 1), pr);
-            }
-            l += (sumA.x + sumA.y) + (sumB.x + sumB.y);
-            if (!last) {
-              ctrl->m_sh[row] = m_used;
-              ctrl->l_sh[row] = l;
-            }
-            named_bar_arrive(turn_other, 256);
-            // ---- end of the exclusive section
-            tmem_wait_st();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(p_full_addr);
-            if (last) finish(m_used, l);
-          } else {
-            // this CTA's tile has no valid row for this item: keep the barriers moving
-            named_bar_sync(turn_mine, 256);
-            named_bar_arrive(turn_other, 256);
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(p_full_addr);
-          }
+          const uint32_t gidx = g0 + j;
+          const uint32_t sb = gidx & 1;
+          mbar_wait<9>(smem_u32(&ctrl->s_full[sb]), (gidx >> 1) & 1);
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(p_full_addr + sb * 16);
         }
+      }
+      if (nt > 0) {
         g0 += nt;
         ++n_keyed;
       }
       __syncwarp();
       if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
     }
-    // consume the last, unmatched turn hand-over so that no barrier is left half-arrived
-    if (static_cast<int>(g0 & 1) == wg) named_bar_sync(turn_mine, 256);
   } else {
     // ================================================================= epilogue group (a7)
     setmaxnreg_dec<kEpilogueRegs>();
@@ -678,7 +697,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
     const uint32_t stage = epi_smem + ew * kEpiWarpBytes;
     const uint32_t o_empty_addr = mapa_shared(smem_u32(&ctrl->o_empty[0]), 0);   // the leader's barriers
     uint32_t n_keyed = 0;
-    uint32_t lr_uses[kItemSlots] = {0, 0, 0, 0};
+    uint32_t lr_par = 0;      // bit s: parity of the next l_ready[s] phase to wait for
     for (uint32_t n = 0;; ++n) {
       const int islot = n & (kItemSlots - 1);
       mbar_wait<11>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
@@ -689,8 +708,8 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       const bool self_here = has_self && it.split == 0;
       const uint32_t ob = n_keyed & 1;
       if (nh > 0) {
-        mbar_wait<12>(smem_u32(&ctrl->l_ready[islot]), lr_uses[islot] & 1);
-        ++lr_uses[islot];
+        mbar_wait<12>(smem_u32(&ctrl->l_ready[islot]), (lr_par >> islot) & 1);
+        lr_par ^= 1u << islot;
       }
       if (nt > 0) {
         mbar_wait<13>(smem_u32(&ctrl->o_full[ob]), (n_keyed >> 1) & 1);
@@ -699,7 +718,8 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       if (nh > 0) {
         const int row = ew * 32 + lane;                  // row of this thread within the tile
         const int g_own = row / cpt, cl_own = row - g_own * cpt;
-        const float inv = ctrl->epi_inv[islot][row];
+        const float lsum = ctrl->epi_l[islot][0][row] + ctrl->epi_l[islot][1][row];
+        const float inv = partial ? 1.0f : (lsum > 0.f ? 1.0f / lsum : 0.f);
         const float ws = ctrl->epi_wself[islot][row] * inv;
         const float2 sc2 = make_float2(inv, inv);
         const int cand0 = it.c0 + static_cast<int>(rank) * cpt;       // first candidate of this CTA's tile

@@ -267,25 +267,15 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t rank) {
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
   return r;
 }
-// arrive on a barrier of any CTA of the cluster (address from mapa_shared); release at cluster scope
+// arrive on a barrier of any CTA of the cluster (address from mapa_shared).  Plain form: what it
+// orders here are tcgen05 accesses, which tcgen05.fence::before_thread_sync already handles; the
+// .release.cluster form compiles to MEMBAR.ALL.GPU in front of every arrive.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr)
-               : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(bar_cluster_addr) : "memory");
 }
-// wait on a local barrier whose arrivals may come from the peer CTA: acquire at cluster scope
-__device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred P;\n\t"
-      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2;\n\t"
-      "selp.b32 %0, 1, 0, P;\n\t}\n"
-      : "=r"(ok)
-      : "r"(bar), "r"(parity)
-      : "memory");
-  return ok != 0;
-}
+// wait on a local barrier whose arrivals may come from the peer CTA
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
-  while (!mbar_try_wait_cluster(bar, parity)) {
+  while (!mbar_try_wait<0>(bar, parity)) {
   }
 }
 // one 32-bit word into the peer's shared memory, completing 4 bytes on the peer's mbarrier
@@ -449,6 +439,12 @@ __device__ __forceinline__ float2 ex2_poly2(float2 x) {
 }
 
 // ------------------------------------------------------------------------------ misc
+// three-input maximum (FMNMX3 on sm_100)
+__device__ __forceinline__ float fmax3(float a, float b, float c) {
+  float r;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+  return r;
+}
 __device__ __forceinline__ float ex2_approx(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));

@@ -19,6 +19,7 @@ namespace {
 
 thread_local char g_err[512] = "";
 thread_local int g_launches = 0;
+thread_local const char* g_kernel = "";
 
 upr_status fail(upr_status s, const char* fmt, ...) {
   va_list ap;
@@ -112,7 +113,7 @@ bool pair_capable(const upr_attn_params* p) {
          static_cast<long long>(p->n_layers) * p->total_q < (1LL << 31);
 }
 
-constexpr bool kPairInAuto = false;   // flipped once the pair kernel is parity-green on the GPU
+constexpr bool kPairInAuto = true;
 
 bool use_pair(const upr_attn_params* p, bool have_workspace) {
   if (!have_workspace || p->kernel == UPR_KERNEL_SINGLE || !pair_capable(p)) return false;
@@ -332,6 +333,7 @@ upr_status run_attn_pair(const upr_attn_params* p, int ns, cudaStream_t st) {
   upr::pair::upr_attn_pair_kernel<<<2 * pairs, upr::pair::kThreads, upr::pair::kSmemTotal, st>>>(tk, tv, tq, to, a);
   UPR_CUDA_CHECK(cudaGetLastError());
   g_launches = 2;
+  g_kernel = "upr_attn_pair_kernel";
   if (ns > 1) {
     s = launch_combine(a.part_o, a.part_ml, p->out, out_rows, ns, p->d, st);
     if (s != UPR_OK) return s;
@@ -446,6 +448,7 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
                    : launch_attn_d<128>(p->kv_dtype, a, tk, tv, to, tq, grid, st);
   if (s != UPR_OK) return s;
   g_launches = 1;
+  g_kernel = "upr_attn_fwd_kernel";
   if (ns > 1) {
     s = launch_combine(a.part_o, a.part_ml, p->out, out_rows, ns, p->d, st);
     if (s != UPR_OK) return s;
@@ -462,6 +465,7 @@ extern "C" {
 const char* upr_last_error(void) { return g_err; }
 const char* upr_version(void) { return "upr 0.1 sm_100a"; }
 int upr_last_launch_count(void) { return g_launches; }
+const char* upr_last_attn_kernel(void) { return g_kernel; }
 
 upr_status upr_kv_cache_layout(const int32_t* seq_lens, int B, int H, int d, int n_layers,
                                upr_dtype dtype, upr_kv_layout* out, int64_t* row_off) {

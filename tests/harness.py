@@ -24,14 +24,20 @@ def to_f64(t: torch.Tensor) -> np.ndarray:
 
 
 class Inputs:
-    def __init__(self, w: S.Workload, device, q_scale: float = 1.0):
+    def __init__(self, w: S.Workload, device, q_scale: float = 1.0, H_kv=None):
+        """w.H is the number of QUERY heads; H_kv (default w.H) the number of KV heads of the pool
+        (grouped queries: query head hq reads KV head hq // (w.H // H_kv), PAPER.md:202 "KV heads")."""
         self.w = w
         self.device = device
+        self.H_kv = H_kv or w.H
+        self.G = w.H // self.H_kv
+        assert self.G * self.H_kv == w.H
         self.q = S.gen_queries(w, "q", device, q_scale)
         self.k_self = S.gen_queries(w, "k_self", device) if w.self_term else None
         self.v_self = S.gen_queries(w, "v_self", device) if w.self_term else None
-        self.k_pool = S.gen_pool(w, "k_pool", device)
-        self.v_pool = S.gen_pool(w, "v_pool", device)
+        pool_shape = (w.n_layers, w.B, self.H_kv, w.n_max, w.d)
+        self.k_pool = S.normal_bf16(w.seed, "k_pool", pool_shape, device)   # == S.gen_pool when H_kv == w.H
+        self.v_pool = S.normal_bf16(w.seed, "v_pool", pool_shape, device)
         self.slot_ids_host = S.slot_ids(w)
         self.slot_ids = torch.as_tensor(self.slot_ids_host, device=device)
 
@@ -40,7 +46,8 @@ class Inputs:
         (bf16 values widened exactly) -- for bf16/f32 caches this IS what the cache stores."""
         Lb = int(self.w.seq_lens[b])
         s = int(self.slot_ids_host[b])
-        return to_f64(self.k_pool[l, s, h, :Lb]), to_f64(self.v_pool[l, s, h, :Lb])
+        hk = h // self.G
+        return to_f64(self.k_pool[l, s, hk, :Lb]), to_f64(self.v_pool[l, s, hk, :Lb])
 
     def oracle_fp8_cache(self):
         """(k_bytes, k_scale, v_bytes, v_scale, row_off, R): the ORACLE's E4M3 pack of the whole pools

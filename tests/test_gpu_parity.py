@@ -26,23 +26,25 @@ def P():
     return pkg
 
 
-def run_cuda(P, inp: Inputs, num_splits=1, sm_scale=0.0):
+def run_cuda(P, inp: Inputs, num_splits=1, sm_scale=0.0, kernel=0):
     from paper_2606_00422_b200 import pipeline as pl
     w = inp.w
-    cache = pl.alloc_cache(w.seq_lens, w.H, w.d, w.n_layers, pl.DTYPE_ID[w.kv_dtype], inp.device)
+    cache = pl.alloc_cache(w.seq_lens, inp.H_kv, w.d, w.n_layers, pl.DTYPE_ID[w.kv_dtype], inp.device)
     pl.pack_cache(cache, inp.k_pool, inp.v_pool, inp.slot_ids)
-    attn = pl.CrossAttention(cache, w.cand_offsets, pl.DTYPE_ID[w.q_dtype], num_splits=num_splits)
+    attn = pl.CrossAttention(cache, w.cand_offsets, pl.DTYPE_ID[w.q_dtype], num_splits=num_splits, H_q=w.H,
+                             kernel=kernel)
     out = attn(inp.q, inp.k_self, inp.v_self, sm_scale=sm_scale)
     torch.cuda.synchronize()
     return out.cpu().numpy(), cache, attn
 
 
-def run_cuda_pool(P, inp: Inputs, num_splits=1, sm_scale=0.0):
+def run_cuda_pool(P, inp: Inputs, num_splits=1, sm_scale=0.0, kernel=0):
     """Zero-copy: the attention reads the pool in place through slot_ids (no pack, no decode cache)."""
     from paper_2606_00422_b200 import pipeline as pl
     w = inp.w
     view = pl.PoolView.of(inp.k_pool, inp.v_pool, inp.slot_ids, w.seq_lens)
-    attn = pl.CrossAttention(view, w.cand_offsets, pl.DTYPE_ID[w.q_dtype], num_splits=num_splits)
+    attn = pl.CrossAttention(view, w.cand_offsets, pl.DTYPE_ID[w.q_dtype], num_splits=num_splits, H_q=w.H,
+                             kernel=kernel)
     out = attn(inp.q, inp.k_self, inp.v_self, sm_scale=sm_scale)
     torch.cuda.synchronize()
     return out.cpu().numpy(), attn
@@ -156,6 +158,107 @@ def test_zero_copy_pool_matches_packed_and_oracle(P, case, ns):
     check(got_pool, oracle_all(inp))
     mx, _ = error_stats(got_pool, got_packed.astype(np.float64))
     assert mx <= 1e-6, f"pool mode differs from packed mode by {mx}"
+
+
+D128_CASES = [c for c in CASES if c[4] == 128]
+
+
+@pytest.mark.parametrize("case", D128_CASES, ids=[c[0] for c in D128_CASES])
+@pytest.mark.parametrize("kernel", ["single", "pair"])
+@pytest.mark.parametrize("source", ["packed", "pool"])
+def test_both_kernels_match_oracle(P, case, kernel, source):
+    """The 1-CTA kernel and the CTA-pair kernel (tcgen05 cta_group::2, two S buffers of 128 keys, O
+    double-buffered across items, longest-first work list) on the same d = 128 cases, from the packed
+    cache and from the pool in place; ns in {1, 2}."""
+    name, L, C, H, d, layers, self_on = case
+    w = S.custom_workload(name, 4242, L, C, H, d, layers, self_term=self_on, n_max=max(L) + 37)
+    inp = Inputs(w, "cuda")
+    kid = {"single": P.UPR_KERNEL_SINGLE, "pair": P.UPR_KERNEL_PAIR}[kernel]
+    want = oracle_all(inp)
+    for ns in (1, 2):
+        if source == "pool":
+            got, attn = run_cuda_pool(P, inp, num_splits=ns, kernel=kid)
+        else:
+            got, _, attn = run_cuda(P, inp, num_splits=ns, kernel=kid)
+        assert P.upr_last_attn_kernel() == ("upr_attn_pair_kernel" if kernel == "pair" else "upr_attn_fwd_kernel")
+        check(got, want)
+
+
+GQA_CASES = [
+    # name, seq_lens, cand_counts, H_q, H_kv, layers, self, splits
+    ("gqa2", [300, 77, 640], [200, 64, 129], 4, 2, 1, False, 1),
+    ("gqa2_full_tiles", [256, 512], [128, 256], 2, 1, 2, True, 1),
+    ("gqa4_self", [300, 77, 640, 0], [200, 31, 129, 70], 8, 2, 2, True, 1),
+    ("gqa4_split", [1300, 77, 0, 2048], [100, 33, 5, 17], 4, 1, 1, True, 3),
+    ("gqa8", [1300, 77, 15], [100, 33, 1], 8, 1, 1, False, 1),
+    ("gqa8_self_split", [1300, 77, 15], [16, 33, 40], 16, 2, 1, True, 2),
+]
+
+
+@pytest.mark.parametrize("case", GQA_CASES, ids=[c[0] for c in GQA_CASES])
+@pytest.mark.parametrize("source", ["packed", "pool"])
+def test_grouped_queries_match_oracle(P, case, source):
+    """SURVEY 8(f)3 / PAPER.md:202 "KV heads": H_kv < H_q, the query group folded into M (a tile holds
+    128/G candidates x G heads).  Oracle: the plain definition with KV head hq // G."""
+    name, L, C, Hq, Hkv, layers, self_on, ns = case
+    w = S.custom_workload(name, 777, L, C, Hq, 128, layers, self_term=self_on, n_max=max(L) + 5)
+    inp = Inputs(w, "cuda", H_kv=Hkv)
+    if source == "pool":
+        got, attn = run_cuda_pool(P, inp, num_splits=ns)
+    else:
+        got, _, attn = run_cuda(P, inp, num_splits=ns)
+    assert attn.splits == ns and P.upr_last_attn_kernel() == "upr_attn_pair_kernel"
+    check(got, oracle_all(inp))
+    # the same through the oracle's own pool-addressed, grouped-query driver (plain indexing)
+    kw = dict(kself=bits(inp.k_self), vself=bits(inp.v_self)) if self_on else {}
+    want2 = oracle.cross_attn_pool(bits(inp.q), oracle.BF16, bits(inp.k_pool), bits(inp.v_pool), inp.slot_ids_host,
+                                   w.seq_lens, w.cand_offsets, Hq, **kw)
+    check(got, want2)
+
+
+def test_grouped_queries_unsupported_combinations_are_refused(P):
+    from paper_2606_00422_b200 import pipeline as pl
+    w = S.custom_workload("gqa_err", 1, [64], [4], 4, 64, 1)
+    inp = Inputs(w, "cuda", H_kv=2)
+    view = pl.PoolView.of(inp.k_pool, inp.v_pool, inp.slot_ids, w.seq_lens)
+    attn = pl.CrossAttention(view, w.cand_offsets, P.UPR_BF16, H_q=4)          # d = 64: no grouped-query kernel
+    with pytest.raises(P.UprError) as e:
+        attn(inp.q)
+    assert e.value.status == 2
+    with pytest.raises(P.UprError) as e:                                        # H_kv does not divide H
+        P.upr_cross_attn_fwd_ex(inp.q, inp.k_pool, inp.v_pool, view.seq_lens, attn.cand_offsets, attn.out, 1, 4, 64, 1,
+                                P.UPR_BF16, P.UPR_BF16, 4, attn.workspace, H_kv=3)
+    assert e.value.status == 1
+
+
+@pytest.mark.parametrize("kernel", ["single", "pair"])
+def test_longest_first_schedule_on_very_ragged_batch(P, kernel):
+    """Histories from 0 to 8192 keys and candidate counts 1 .. 1000 in one batch:
+    the pair kernel hands items out longest-first from the tables of upr_schedule_kernel (bitonic sort of
+    the users by L_b, ties by index), every row is checked."""
+    L = [0, 8192, 64, 700, 8192, 1, 129, 2049, 0, 4096, 333, 16]
+    C = [1, 129, 257, 1000, 3, 512, 50, 256, 128, 255, 130, 64]
+    w = S.custom_workload("very_ragged", 2025, L, C, 2, 128, 1, self_term=True)
+    inp = Inputs(w, "cuda")
+    kid = {"single": P.UPR_KERNEL_SINGLE, "pair": P.UPR_KERNEL_PAIR}[kernel]
+    got, attn = run_cuda_pool(P, inp, num_splits=0, kernel=kid)
+    check(got, oracle_all(inp))
+
+
+@pytest.mark.parametrize("B", [4097, 1000])
+def test_many_users(P, B):
+    """More users than the schedule kernel sorts (B > 4096 keeps the user order) and a batch that is not a
+    power of two: the work-list tables (prefix sums over a chunk per thread) must cover every user."""
+    rng = np.random.default_rng(B)
+    L = [int(x) for x in rng.choice([0, 3, 16, 40, 130], size=B)]
+    C = [int(x) for x in rng.choice([0, 1, 2, 5], size=B)]
+    w = S.custom_workload(f"many_users_{B}", 99, L, C, 1, 128, 1)
+    inp = Inputs(w, "cuda")
+    got, attn = run_cuda_pool(P, inp, num_splits=1, kernel=P.UPR_KERNEL_PAIR)
+    kw = {}
+    want = oracle.cross_attn_pool(bits(inp.q), oracle.BF16, bits(inp.k_pool), bits(inp.v_pool), inp.slot_ids_host,
+                                  w.seq_lens, w.cand_offsets, 1, **kw)
+    check(got, want)
 
 
 def test_zero_copy_rejects_bad_arguments(P):
