@@ -236,3 +236,44 @@ def cross_attn_pool(q, q_dtype: int, k_pool_bits, v_pool_bits, slot_ids, seq_len
     if rc:
         raise ValueError("upro_cross_attn_pool: invalid argument")
     return out
+
+
+# ---------------------------------------------------------------------------- decode-layer tail, consumer
+ACT_NONE, ACT_SILU, ACT_RELU = 0, 1, 2
+
+
+def linear(x, w, b=None, act: int = ACT_NONE):
+    """y = act(x W^T + b) in fp64; x [M,K], w [N,K] (nn.Linear convention), b [N] or None."""
+    x, w = _c64(x), _c64(w)
+    M, K = x.shape
+    N = w.shape[0]
+    assert w.shape[1] == K
+    bb = _c64(b) if b is not None else None
+    y = np.zeros((M, N), dtype=np.float64)
+    lib().upro_linear(_p(x), _p(w), _p(bb), ctypes.c_int64(M), N, K, act, _p(y))
+    return y
+
+
+def action_utility(z, w1, b1, w2, b2, wc, act: int = ACT_SILU):
+    """Per-action MLP heads -> probabilities -> weighted utility.
+    z [M,D]; w1 [C,Dh,D]; b1 [C,Dh]; w2 [C,Dh]; b2 [C]; wc [C].  Returns (probs [M,C], util [M])."""
+    z, w1, b1, w2, b2, wc = (_c64(a) for a in (z, w1, b1, w2, b2, wc))
+    M, D = z.shape
+    C, Dh, _ = w1.shape
+    probs = np.zeros((M, C), dtype=np.float64)
+    util = np.zeros(M, dtype=np.float64)
+    lib().upro_action_utility(_p(z), _p(w1), _p(b1), _p(w2), _p(b2), _p(wc), ctypes.c_int64(M), D, C, Dh, act,
+                              _p(probs), _p(util))
+    return probs, util
+
+
+def topk_per_user(util, cand_offsets, K: int):
+    """Top-K candidates per user by utility (fp32 compare), ties by ascending index.
+    Returns (idx [B,K] int32 global candidate indices, -1 padded; cnt [B] int32)."""
+    util = np.ascontiguousarray(util, dtype=np.float32)
+    cand_offsets = np.ascontiguousarray(cand_offsets, dtype=np.int32)
+    B = int(cand_offsets.shape[0]) - 1
+    idx = np.zeros((B, K), dtype=np.int32)
+    cnt = np.zeros(B, dtype=np.int32)
+    lib().upro_topk_per_user(_p(util), _p(cand_offsets), B, K, _p(idx), _p(cnt))
+    return idx, cnt

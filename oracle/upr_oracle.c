@@ -554,3 +554,93 @@ int upro_cross_attn_pool(const void* q, int q_dtype, const uint16_t* k_pool,
   }
   return 0;
 }
+
+/* ====================================================================================
+ * The rest of the ranking decode layer and its consumer.
+ * ==================================================================================== */
+
+/* ------------------------------------------------------------------------------------
+ * upro_linear -- one linear layer of the ranking pass over candidate tokens only
+ * ("only the candidate tokens are processed"): y = act(x W^T + b), the plain
+ * definition, fp64.  W is [N, K] row-major (one output feature per row, the nn.Linear
+ * convention); act: 0 = identity, 1 = SiLU x*sigmoid(x), 2 = ReLU.  The paper names no
+ * activation for its MLPs (reading Q15): SiLU is this build's default.
+ *   x [M, K], w [N, K], b [N] or NULL, y [M, N]
+ * ---------------------------------------------------------------------------------- */
+void upro_linear(const double* x, const double* w, const double* b, int64_t M, int N, int K,
+                 int act, double* y) {
+#pragma omp parallel for schedule(static)
+  for (int64_t m = 0; m < M; ++m)
+    for (int n = 0; n < N; ++n) {
+      double acc = 0.0;
+      for (int k = 0; k < K; ++k) acc += x[m * K + k] * w[(int64_t)n * K + k];
+      if (b) acc += b[n];
+      if (act == 1) acc = acc / (1.0 + exp(-acc));
+      else if (act == 2) acc = acc > 0.0 ? acc : 0.0;
+      y[m * N + n] = acc;
+    }
+}
+
+/* ------------------------------------------------------------------------------------
+ * upro_action_utility -- the ranking head's consumer (PAPER.md:146-152, Eq. 4; :321).
+ * For every candidate hidden state z and action type c = 0..C-1 a dedicated two-layer MLP
+ * head h_c produces a scalar logit,
+ *     hid_c = act(W1_c z + b1_c)   (W1_c [Dh, D], act as in upro_linear)
+ *     logit_c = <w2_c, hid_c> + b2_c
+ * p_c = sigmoid(logit_c) is the action probability (the BCE of Eq. 4 trains exactly this),
+ * and the candidate's utility is the weighted sum  u = sum_c w_c p_c  ("head utility
+ * functions"; the weights are the per-head w_c of Eq. 4 -- reading Q16).
+ *   z [M, D]; w1 [C, Dh, D]; b1 [C, Dh]; w2 [C, Dh]; b2 [C]; wc [C]
+ *   probs [M, C] (may be NULL), util [M]
+ * ---------------------------------------------------------------------------------- */
+void upro_action_utility(const double* z, const double* w1, const double* b1, const double* w2,
+                         const double* b2, const double* wc, int64_t M, int D, int C, int Dh,
+                         int act, double* probs, double* util) {
+#pragma omp parallel for schedule(static)
+  for (int64_t m = 0; m < M; ++m) {
+    double u = 0.0;
+    for (int c = 0; c < C; ++c) {
+      double logit = b2[c];
+      for (int j = 0; j < Dh; ++j) {
+        double h = b1[(int64_t)c * Dh + j];
+        for (int t = 0; t < D; ++t) h += w1[((int64_t)c * Dh + j) * D + t] * z[m * D + t];
+        if (act == 1) h = h / (1.0 + exp(-h));
+        else if (act == 2) h = h > 0.0 ? h : 0.0;
+        logit += w2[(int64_t)c * Dh + j] * h;
+      }
+      double p = 1.0 / (1.0 + exp(-logit));
+      if (probs) probs[m * C + c] = p;
+      u += wc[c] * p;
+    }
+    util[m] = u;
+  }
+}
+
+/* ------------------------------------------------------------------------------------
+ * upro_topk_per_user -- "returns the top K ranked candidates": for user b
+ * the min(K, C_b) candidates of [cand_offsets[b], cand_offsets[b+1]) with the largest
+ * utility, in descending order of utility; equal utilities in ascending order of index
+ * (the order is then unique, so the comparison with the GPU is exact).  Utilities are
+ * compared as the fp32 values the GPU holds.  out_idx [B, K] global candidate indices,
+ * -1 past the user's count; out_cnt [B].
+ * ---------------------------------------------------------------------------------- */
+void upro_topk_per_user(const float* util, const int32_t* cand_offsets, int B, int K,
+                        int32_t* out_idx, int32_t* out_cnt) {
+  for (int b = 0; b < B; ++b) {
+    int c0 = cand_offsets[b], n = cand_offsets[b + 1] - c0;
+    int kk = n < K ? n : K;
+    out_cnt[b] = kk;
+    char* used = (char*)calloc((size_t)(n > 0 ? n : 1), 1);
+    for (int r = 0; r < K; ++r) {
+      int best = -1;
+      if (r < kk)
+        for (int i = 0; i < n; ++i) {   /* selection by repeated maximum: first index wins ties */
+          if (used[i]) continue;
+          if (best < 0 || util[c0 + i] > util[c0 + best]) best = i;
+        }
+      if (best >= 0) used[best] = 1;
+      out_idx[(int64_t)b * K + r] = best >= 0 ? c0 + best : -1;
+    }
+    free(used);
+  }
+}
