@@ -191,6 +191,76 @@ int upr_cross_attn_num_splits(const upr_attn_params* p);
  */
 upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream);
 
+/* ====================================================================================
+ * Around the attention: the rest of one ranking decode layer and the consumer
+ * of the ranking pass (8(f)4).  Candidate tokens only; synthetic weights.
+ * ==================================================================================== */
+
+typedef enum { UPR_ACT_NONE = 0, UPR_ACT_SILU = 1, UPR_ACT_RELU = 2 } upr_activation;
+
+/*
+ * y = act(x W^T + bias): out-projection, MLP and projection layers of the candidate-only pass
+ * (PAPER.md:192), the stacked first layers of the per-action heads.  tcgen05 GEMM,
+ * bf16 operands, fp32 accumulation.
+ *   x     device  [M, K] row-major, x_dtype UPR_BF16 or UPR_F32 (fp32 rows -- e.g. the attention output --
+ *                 are rounded to bf16 inside the kernel on their way into the MMA, no cast pass)
+ *   w     device  bf16 [N, K] row-major (one output feature per row)
+ *   bias  device  fp32 [N] or NULL
+ *   y     device  [M, N] row-major, y_dtype UPR_BF16 or UPR_F32
+ * K % 64 == 0 and N % 8 == 0 (else UPR_ERR_UNSUPPORTED); M >= 0 (0: no launch); x, w 16-byte aligned.
+ */
+upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
+                          upr_dtype y_dtype, int64_t M, int N, int K, upr_activation act, void* stream);
+
+/*
+ * Per-action heads, second half: hid = act(W1_c z + b1_c) for the C heads side by
+ * side comes from upr_linear_fwd (N = C * Dh); this call finishes them:
+ *     logit_c = <w2_c, hid_c> + b2_c,  p_c = sigmoid(logit_c),  util = sum_c wc_c * p_c
+ * ("head utility functions"; wc = the per-head weights of Eq. 4).
+ *   hid   device bf16 [M, C * Dh]; w2 device fp32 [C, Dh]; b2, wc device fp32 [C]
+ *   probs device fp32 [M, C] or NULL; util device fp32 [M]
+ * Dh % 8 == 0.
+ */
+upr_status upr_action_utility(const void* hid, const float* w2, const float* b2, const float* wc, int64_t M,
+                              int C, int Dh, float* probs, float* util, void* stream);
+
+/*
+ * "returns the top K ranked candidates": for every user b the min(K, C_b) candidates of
+ * [cand_offsets[b], cand_offsets[b+1]) with the largest utility, descending; equal utilities in
+ * ascending order of candidate index (the result is unique).
+ *   util device fp32 [total_q]; cand_offsets device int32 [B+1]
+ *   max_cands  host upper bound on any user's candidate count (<= 16384, else UPR_ERR_UNSUPPORTED)
+ *   out_idx device int32 [B, K]: global candidate indices, -1 past the user's count; out_cnt device int32 [B]
+ */
+upr_status upr_topk_per_user(const float* util, const int32_t* cand_offsets, int B, int K, int max_cands,
+                             int32_t* out_idx, int32_t* out_cnt, void* stream);
+
+/* ====================================================================================
+ * The KV pool across processes: the retrieval replica allocates the
+ * pool [L, S, H, n, D], exports a CUDA IPC handle "to a per-instance file", the ranking process opens it
+ * and reads the same physical allocation in place (with UPR_KV_POOL: no copy at all); slots are reused
+ * round-robin.
+ * ==================================================================================== */
+
+#define UPR_IPC_HANDLE_BYTES 80
+typedef struct upr_ipc_handle { unsigned char bytes[UPR_IPC_HANDLE_BYTES]; } upr_ipc_handle;
+
+/* Export a handle for device memory allocated in THIS process (cudaMalloc-class).  pool_dev may point
+ * anywhere inside its allocation (a framework's caching allocator sub-allocates): the handle carries the
+ * CUDA IPC handle of the allocation and the pointer's offset in it.  The handle is plain bytes: write it
+ * to a file, a pipe, shared memory. */
+upr_status upr_pool_export(const void* pool_dev, upr_ipc_handle* out);
+/* Map the exporter's allocation into this (other) process; *pool_dev (the exporter's pointer, translated)
+ * is valid until upr_pool_close(*pool_dev).  One open mapping per allocation and process (a CUDA rule). */
+upr_status upr_pool_open(const upr_ipc_handle* handle, void** pool_dev);
+upr_status upr_pool_close(void* pool_dev);
+
+/* Round-robin slot assignment ("slots are reused round-robin"): host-only, no device work.
+ * state: {S, next}; upr_slot_ring_acquire writes n consecutive slot ids (mod S) and advances. */
+typedef struct upr_slot_ring { int32_t S; int32_t next; } upr_slot_ring;
+upr_status upr_slot_ring_init(upr_slot_ring* ring, int32_t S);
+upr_status upr_slot_ring_acquire(upr_slot_ring* ring, int32_t n, int32_t* slot_ids_host);
+
 /* Kernel launches the last successful call on this thread enqueued (for accounting). */
 int upr_last_launch_count(void);
 

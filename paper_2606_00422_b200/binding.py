@@ -16,7 +16,11 @@ EXPORTED_SYMBOLS = [
     "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
     "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
     "upr_last_error", "upr_version", "upr_last_attn_kernel",
+    "upr_linear_fwd", "upr_action_utility", "upr_topk_per_user",
+    "upr_pool_export", "upr_pool_open", "upr_pool_close", "upr_slot_ring_init", "upr_slot_ring_acquire",
 ]
+UPR_ACT_NONE, UPR_ACT_SILU, UPR_ACT_RELU = 0, 1, 2
+UPR_IPC_HANDLE_BYTES = 80
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -88,6 +92,26 @@ def _load() -> ctypes.CDLL:
         lib.upr_cross_attn_fwd.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_int] * 4 + [ctypes.c_void_p]
         lib.upr_cross_attn_fwd_ex.restype = ctypes.c_int
         lib.upr_cross_attn_fwd_ex.argtypes = [ctypes.POINTER(_AttnParams), ctypes.c_void_p]
+        lib.upr_linear_fwd.restype = ctypes.c_int
+        lib.upr_linear_fwd.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
+                                       ctypes.c_int, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                       ctypes.c_void_p]
+        lib.upr_action_utility.restype = ctypes.c_int
+        lib.upr_action_utility.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_int64, ctypes.c_int, ctypes.c_int,
+                                                                   ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.upr_topk_per_user.restype = ctypes.c_int
+        lib.upr_topk_per_user.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                          ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
+        lib.upr_pool_export.restype = ctypes.c_int
+        lib.upr_pool_export.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.upr_pool_open.restype = ctypes.c_int
+        lib.upr_pool_open.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_void_p)]
+        lib.upr_pool_close.restype = ctypes.c_int
+        lib.upr_pool_close.argtypes = [ctypes.c_void_p]
+        lib.upr_slot_ring_init.restype = ctypes.c_int
+        lib.upr_slot_ring_init.argtypes = [ctypes.c_void_p, ctypes.c_int32]
+        lib.upr_slot_ring_acquire.restype = ctypes.c_int
+        lib.upr_slot_ring_acquire.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -191,3 +215,62 @@ def upr_cross_attn_fwd_ex(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H
                 k_self, v_self, k_scale, v_scale, sm_scale, num_splits, max_seq_len, workspace, kv_source,
                 pool_slots, pool_n_max, H_kv, slot_ids, kv_bytes, kv_rows, kernel)
     _check(_load().upr_cross_attn_fwd_ex(ctypes.byref(p), _stream(stream)))
+
+
+# ---------------------------------------------------------------------------- decode-layer tail, consumer, pool
+_DT = {torch.float32: UPR_F32, torch.bfloat16: UPR_BF16}
+
+
+def upr_linear_fwd(x, w, bias, y, act: int = UPR_ACT_NONE, stream=None) -> None:
+    """y = act(x W^T + bias): x [M,K] bf16/fp32, w [N,K] bf16, bias fp32 [N] or None, y [M,N] bf16/fp32."""
+    M, K = int(x.shape[0]), int(x.shape[1])
+    N = int(w.shape[0])
+    _check(_load().upr_linear_fwd(_ptr(x), _DT[x.dtype], _ptr(w), _ptr(bias), _ptr(y), _DT[y.dtype], M, N, K, act,
+                                  _stream(stream)))
+
+
+def upr_action_utility(hid, w2, b2, wc, probs, util, stream=None) -> None:
+    """hid bf16 [M, C*Dh]; w2 fp32 [C,Dh]; b2, wc fp32 [C]; probs fp32 [M,C] or None; util fp32 [M]."""
+    C, Dh = int(w2.shape[0]), int(w2.shape[1])
+    M = int(hid.shape[0])
+    _check(_load().upr_action_utility(_ptr(hid), _ptr(w2), _ptr(b2), _ptr(wc), M, C, Dh, _ptr(probs), _ptr(util),
+                                      _stream(stream)))
+
+
+def upr_topk_per_user(util, cand_offsets, K: int, max_cands: int, out_idx, out_cnt, stream=None) -> None:
+    B = int(cand_offsets.shape[0]) - 1
+    _check(_load().upr_topk_per_user(_ptr(util), _ptr(cand_offsets), B, K, max_cands, _ptr(out_idx), _ptr(out_cnt),
+                                     _stream(stream)))
+
+
+def upr_pool_export(pool: torch.Tensor) -> bytes:
+    """Opaque handle bytes for the device memory of `pool`: CUDA IPC handle + offset."""
+    buf = (ctypes.c_ubyte * UPR_IPC_HANDLE_BYTES)()
+    _check(_load().upr_pool_export(pool.data_ptr(), ctypes.byref(buf)))
+    return bytes(buf)
+
+
+def upr_pool_open(handle: bytes) -> int:
+    """Map the exporter's allocation into this process; returns the device pointer."""
+    buf = (ctypes.c_ubyte * UPR_IPC_HANDLE_BYTES).from_buffer_copy(handle)
+    out = ctypes.c_void_p()
+    _check(_load().upr_pool_open(ctypes.byref(buf), ctypes.byref(out)))
+    return int(out.value)
+
+
+def upr_pool_close(ptr: int) -> None:
+    _check(_load().upr_pool_close(ctypes.c_void_p(ptr)))
+
+
+class SlotRing(ctypes.Structure):
+    """Round-robin slot assignment."""
+    _fields_ = [("S", ctypes.c_int32), ("next", ctypes.c_int32)]
+
+    def __init__(self, S: int):
+        super().__init__()
+        _check(_load().upr_slot_ring_init(ctypes.byref(self), S))
+
+    def acquire(self, n: int) -> np.ndarray:
+        out = np.zeros(n, dtype=np.int32)
+        _check(_load().upr_slot_ring_acquire(ctypes.byref(self), n, out.ctypes.data))
+        return out

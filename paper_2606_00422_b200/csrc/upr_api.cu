@@ -12,8 +12,10 @@
 #include "../../include/upr.h"
 #include "attn2_kernel.cuh"
 #include "attn_kernel.cuh"
+#include "linear_kernel.cuh"
 #include "pack_kernels.cuh"
 #include "sched_kernel.cuh"
+#include "tail_kernels.cuh"
 
 namespace {
 
@@ -608,6 +610,185 @@ size_t upr_cross_attn_workspace_bytes(const upr_attn_params* p) {
 
 upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream) {
   return run_attn(p, /*have_workspace=*/true, static_cast<cudaStream_t>(stream));
+}
+
+// ------------------------------------------------------------------ decode-layer tail, consumer, pool
+upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
+                          upr_dtype y_dtype, int64_t M, int N, int K, upr_activation act, void* stream) {
+  g_launches = 0;
+  if (M < 0 || N <= 0 || K <= 0) return fail(UPR_ERR_INVALID_ARG, "bad sizes M=%lld N=%d K=%d", (long long)M, N, K);
+  if (x_dtype != UPR_BF16 && x_dtype != UPR_F32) return fail(UPR_ERR_UNSUPPORTED, "x_dtype %d (bf16 or f32)", (int)x_dtype);
+  if (y_dtype != UPR_BF16 && y_dtype != UPR_F32) return fail(UPR_ERR_UNSUPPORTED, "y_dtype %d (bf16 or f32)", (int)y_dtype);
+  if (act != UPR_ACT_NONE && act != UPR_ACT_SILU && act != UPR_ACT_RELU)
+    return fail(UPR_ERR_INVALID_ARG, "activation %d unknown", (int)act);
+  if (K % 64 != 0 || N % 8 != 0) return fail(UPR_ERR_UNSUPPORTED, "K=%d must be a multiple of 64, N=%d of 8", K, N);
+  if (M == 0) return UPR_OK;
+  if (!x || !w || !y) return fail(UPR_ERR_INVALID_ARG, "NULL tensor pointer");
+  if ((reinterpret_cast<uintptr_t>(x) & 15) || (reinterpret_cast<uintptr_t>(w) & 15) || (reinterpret_cast<uintptr_t>(y) & 15))
+    return fail(UPR_ERR_INVALID_ARG, "x, w, y must be 16-byte aligned");
+  if (M >= (1LL << 31)) return fail(UPR_ERR_UNSUPPORTED, "M too large for 32-bit TMA coordinates");
+  upr_status s = check_device();
+  if (s != UPR_OK) return s;
+  EncodeTiledFn enc = get_encode_fn();
+  if (enc == nullptr) return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
+  CUtensorMap tx, tw;
+  cuuint32_t box[2] = {64, 128}, estr[2] = {1, 1};
+  {
+    const bool f32 = x_dtype == UPR_F32;
+    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(M)};
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(K) * (f32 ? 4 : 2)};
+    if (enc(&tx, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(x),
+            gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+            f32 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for x");
+  }
+  {
+    cuuint64_t gdim[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N)};
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(K) * 2};
+    if (enc(&tw, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(w), gdim, gstride, box, estr,
+            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for w");
+  }
+  upr::lin::Args a;
+  a.bias = bias;
+  a.y = y;
+  a.M = M;
+  a.N = N;
+  a.K = K;
+  a.act = static_cast<int>(act);
+  a.y_is_f32 = y_dtype == UPR_F32;
+  const long long tiles = ((M + 127) / 128) * ((N + 127) / 128);
+  int grid = sm_count();
+  if (grid <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
+  if (tiles < grid) grid = static_cast<int>(tiles);
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (x_dtype == UPR_F32) {
+    UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin::upr_linear_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        upr::lin::kSmemTotal));
+    upr::lin::upr_linear_kernel<true><<<grid, upr::lin::kThreads, upr::lin::kSmemTotal, st>>>(tx, tw, a);
+  } else {
+    UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin::upr_linear_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        upr::lin::kSmemTotal));
+    upr::lin::upr_linear_kernel<false><<<grid, upr::lin::kThreads, upr::lin::kSmemTotal, st>>>(tx, tw, a);
+  }
+  UPR_CUDA_CHECK(cudaGetLastError());
+  g_launches = 1;
+  return UPR_OK;
+}
+
+upr_status upr_action_utility(const void* hid, const float* w2, const float* b2, const float* wc, int64_t M,
+                              int C, int Dh, float* probs, float* util, void* stream) {
+  g_launches = 0;
+  if (M < 0 || C <= 0 || Dh <= 0) return fail(UPR_ERR_INVALID_ARG, "bad sizes M=%lld C=%d Dh=%d", (long long)M, C, Dh);
+  if (Dh % 8 != 0) return fail(UPR_ERR_UNSUPPORTED, "Dh=%d must be a multiple of 8", Dh);
+  if (M == 0) return UPR_OK;
+  if (!hid || !w2 || !b2 || !wc || !util) return fail(UPR_ERR_INVALID_ARG, "NULL tensor pointer");
+  upr_status s = check_device();
+  if (s != UPR_OK) return s;
+  const long long blocks = (M + 7) / 8;
+  const int grid = static_cast<int>(blocks < sm_count() * 8LL ? blocks : sm_count() * 8LL);
+  upr::upr_head_utility_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(
+      static_cast<const __nv_bfloat16*>(hid), w2, b2, wc, M, C, Dh, probs, util);
+  UPR_CUDA_CHECK(cudaGetLastError());
+  g_launches = 1;
+  return UPR_OK;
+}
+
+upr_status upr_topk_per_user(const float* util, const int32_t* cand_offsets, int B, int K, int max_cands,
+                             int32_t* out_idx, int32_t* out_cnt, void* stream) {
+  g_launches = 0;
+  if (B < 0 || K <= 0 || max_cands < 0) return fail(UPR_ERR_INVALID_ARG, "bad sizes B=%d K=%d max_cands=%d", B, K, max_cands);
+  if (max_cands > 16384) return fail(UPR_ERR_UNSUPPORTED, "max_cands=%d > 16384 candidates per user", max_cands);
+  if (B == 0) return UPR_OK;
+  if (!util || !cand_offsets || !out_idx || !out_cnt) return fail(UPR_ERR_INVALID_ARG, "NULL tensor pointer");
+  upr_status s = check_device();
+  if (s != UPR_OK) return s;
+  int n_pad = 2;
+  while (n_pad < max_cands) n_pad <<= 1;
+  const size_t smem = static_cast<size_t>(n_pad) * sizeof(unsigned long long);
+  UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::upr_topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      static_cast<int>(smem)));
+  upr::upr_topk_kernel<<<B, upr::kTopkThreads, smem, static_cast<cudaStream_t>(stream)>>>(util, cand_offsets, K, n_pad,
+                                                                                            out_idx, out_cnt);
+  UPR_CUDA_CHECK(cudaGetLastError());
+  g_launches = 1;
+  return UPR_OK;
+}
+
+static_assert(sizeof(cudaIpcMemHandle_t) + 8 <= UPR_IPC_HANDLE_BYTES, "IPC handle does not fit");
+
+typedef CUresult (*GetAddressRangeFn)(CUdeviceptr*, size_t*, CUdeviceptr);
+
+upr_status upr_pool_export(const void* pool_dev, upr_ipc_handle* out) {
+  if (!pool_dev || !out) return fail(UPR_ERR_INVALID_ARG, "NULL argument");
+  void* fnp = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  UPR_CUDA_CHECK(cudaGetDriverEntryPoint("cuMemGetAddressRange", &fnp, cudaEnableDefault, &qres));
+  if (fnp == nullptr || qres != cudaDriverEntryPointSuccess)
+    return fail(UPR_ERR_CUDA, "cuMemGetAddressRange entry point not found");
+  CUdeviceptr base = 0;
+  size_t size = 0;
+  if (reinterpret_cast<GetAddressRangeFn>(fnp)(&base, &size, reinterpret_cast<CUdeviceptr>(pool_dev)) != CUDA_SUCCESS)
+    return fail(UPR_ERR_INVALID_ARG, "pool_dev is not inside a device allocation of this process");
+  cudaIpcMemHandle_t h;
+  UPR_CUDA_CHECK(cudaIpcGetMemHandle(&h, reinterpret_cast<void*>(base)));
+  const uint64_t offset = reinterpret_cast<CUdeviceptr>(pool_dev) - base;
+  memset(out->bytes, 0, sizeof(out->bytes));
+  memcpy(out->bytes, &h, sizeof(h));
+  memcpy(out->bytes + sizeof(h), &offset, sizeof(offset));
+  return UPR_OK;
+}
+
+namespace {
+// open mappings of this process: translated pointer -> mapped base (upr_pool_close needs the base)
+struct OpenPool { void* ptr; void* base; };
+OpenPool g_open[64];
+int g_n_open = 0;
+}  // namespace
+
+upr_status upr_pool_open(const upr_ipc_handle* handle, void** pool_dev) {
+  if (!handle || !pool_dev) return fail(UPR_ERR_INVALID_ARG, "NULL argument");
+  if (g_n_open >= 64) return fail(UPR_ERR_UNSUPPORTED, "too many open pools");
+  cudaIpcMemHandle_t h;
+  uint64_t offset = 0;
+  memcpy(&h, handle->bytes, sizeof(h));
+  memcpy(&offset, handle->bytes + sizeof(h), sizeof(offset));
+  void* base = nullptr;
+  UPR_CUDA_CHECK(cudaIpcOpenMemHandle(&base, h, cudaIpcMemLazyEnablePeerAccess));
+  *pool_dev = static_cast<uint8_t*>(base) + offset;
+  g_open[g_n_open++] = OpenPool{*pool_dev, base};
+  return UPR_OK;
+}
+
+upr_status upr_pool_close(void* pool_dev) {
+  if (!pool_dev) return fail(UPR_ERR_INVALID_ARG, "NULL argument");
+  for (int i = 0; i < g_n_open; ++i)
+    if (g_open[i].ptr == pool_dev) {
+      void* base = g_open[i].base;
+      g_open[i] = g_open[--g_n_open];
+      UPR_CUDA_CHECK(cudaIpcCloseMemHandle(base));
+      return UPR_OK;
+    }
+  return fail(UPR_ERR_INVALID_ARG, "pointer was not returned by upr_pool_open");
+}
+
+upr_status upr_slot_ring_init(upr_slot_ring* ring, int32_t S) {
+  if (!ring || S <= 0) return fail(UPR_ERR_INVALID_ARG, "bad slot ring (S=%d)", S);
+  ring->S = S;
+  ring->next = 0;
+  return UPR_OK;
+}
+
+upr_status upr_slot_ring_acquire(upr_slot_ring* ring, int32_t n, int32_t* slot_ids_host) {
+  if (!ring || ring->S <= 0 || n < 0 || (n > 0 && !slot_ids_host)) return fail(UPR_ERR_INVALID_ARG, "bad slot ring request");
+  if (n > ring->S) return fail(UPR_ERR_INVALID_ARG, "%d slots requested from a pool of %d: a batch would overwrite itself", n, ring->S);
+  for (int32_t i = 0; i < n; ++i) {
+    slot_ids_host[i] = ring->next;
+    ring->next = (ring->next + 1) % ring->S;
+  }
+  return UPR_OK;
 }
 
 }  // extern "C"

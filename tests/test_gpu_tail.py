@@ -1,0 +1,171 @@
+"""GPU parity for the decode-layer tail and the ranking consumer: the tcgen05
+linear layer, the per-action head utility, the per-user top-K, and the cross-process pool (CUDA IPC).
+Oracle: oracle.linear / action_utility / topk_per_user (plain fp64 definitions, pinned in
+tests/test_oracle_tail_pins.py) on the same seeded inputs.
+
+Tolerances (T3): operands are bf16 values (exact in fp64), products are accumulated in
+fp32 over K terms of magnitude ~|x||w|: relative error ~ sqrt(K) 2^-24 -- negligible; a bf16 OUTPUT adds one
+rounding, 2^-9 relative; fp32 x rows are rounded to bf16 on the way into the MMA (2^-9 relative per element,
+independent: ~2^-9 |y| / sqrt(K) ... bounded here by 2^-8 max|y|)."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import upr_synth as S
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2606_00422_b200 as pkg
+    assert torch.cuda.is_available()
+    return pkg
+
+
+def f64(t):
+    return t.detach().cpu().to(torch.float64).numpy()
+
+
+def weights(seed, tag, N, K, dev):
+    """bf16 weights ~ N(0, 1/K) (unit-variance outputs for unit-variance inputs)."""
+    return (S.normal_bf16(seed, tag, (N, K), dev).float() / np.sqrt(K)).to(torch.bfloat16)
+
+
+LINEAR_CASES = [
+    # M, N, K, x dtype, y dtype, act, bias
+    (128, 128, 64, "bf16", "f32", 0, False),
+    (1, 8, 64, "bf16", "f32", 0, True),
+    (300, 136, 192, "bf16", "bf16", 1, True),      # ragged M, N not a multiple of the tile, SiLU
+    (517, 1024, 1024, "bf16", "bf16", 0, False),   # the out-projection shape (H d = D_model = 1024)
+    (517, 1024, 1024, "f32", "bf16", 0, True),     # fp32 activations (the attention output) converted in-kernel
+    (130, 264, 128, "f32", "f32", 2, True),
+    (4099, 384, 256, "bf16", "f32", 1, False),     # more tiles than SMs
+]
+
+
+@pytest.mark.parametrize("case", LINEAR_CASES, ids=[f"M{c[0]}_N{c[1]}_K{c[2]}_{c[3]}_{c[4]}_act{c[5]}" for c in LINEAR_CASES])
+def test_linear_matches_oracle(P, case):
+    M, N, K, xdt, ydt, act, has_bias = case
+    dev = "cuda"
+    x = S.normal_bf16(11, "x", (M, K), dev)
+    if xdt == "f32":
+        x = S.normal_f32(11, "x32", (M, K)).to(dev)
+    w = weights(12, "w", N, K, dev)
+    b = (S.normal_bf16(13, "b", (N,), dev).float() * 0.5) if has_bias else None
+    y = torch.full((M, N), float("nan"), dtype=torch.float32 if ydt == "f32" else torch.bfloat16, device=dev)
+    P.upr_linear_fwd(x, w, b, y, act)
+    torch.cuda.synchronize()
+    assert P.upr_last_launch_count() == 1
+    want = oracle.linear(f64(x), f64(w), None if b is None else f64(b), act=act)
+    got = f64(y)
+    assert np.isfinite(got).all()
+    tol = 2e-4 * max(1.0, np.abs(want).max())
+    if xdt == "f32":
+        tol += 2.0 ** -8 * np.abs(want).max()
+    if ydt == "bf16":
+        tol += 2.0 ** -8 * np.abs(want).max()
+    err = np.abs(got - want).max()
+    print(f"max-abs {err:.2e} (tol {tol:.2e}, max|y| {np.abs(want).max():.2f})")
+    assert err <= tol
+
+
+def test_linear_rejects_unsupported(P):
+    x = torch.zeros((4, 96), dtype=torch.bfloat16, device="cuda")
+    w = torch.zeros((8, 96), dtype=torch.bfloat16, device="cuda")
+    y = torch.zeros((4, 8), dtype=torch.float32, device="cuda")
+    with pytest.raises(P.UprError) as e:     # K not a multiple of 64
+        P.upr_linear_fwd(x, w, None, y)
+    assert e.value.status == 2
+
+
+def test_action_heads_and_utility_match_oracle(P):
+    """z -> [stacked first layers of the C heads, SiLU] (tcgen05 GEMM) -> logits -> sigmoid -> utility."""
+    dev = "cuda"
+    M, D, C, Dh = 777, 256, 5, 64
+    z = S.normal_bf16(21, "z", (M, D), dev)
+    w1 = weights(22, "w1", C * Dh, D, dev)
+    b1 = S.normal_bf16(23, "b1", (C * Dh,), dev).float() * 0.1
+    w2 = (S.normal_bf16(24, "w2", (C, Dh), dev).float() / np.sqrt(Dh)).contiguous()
+    b2 = S.normal_bf16(25, "b2", (C,), dev).float() * 0.1
+    wc = torch.tensor([1.0, 0.5, 2.0, 0.25, 1.5], device=dev)
+    hid = torch.empty((M, C * Dh), dtype=torch.bfloat16, device=dev)
+    probs = torch.empty((M, C), dtype=torch.float32, device=dev)
+    util = torch.empty(M, dtype=torch.float32, device=dev)
+    P.upr_linear_fwd(z, w1, b1, hid, P.UPR_ACT_SILU)
+    P.upr_action_utility(hid, w2, b2, wc, probs, util)
+    torch.cuda.synchronize()
+    want_p, want_u = oracle.action_utility(f64(z), f64(w1).reshape(C, Dh, D), f64(b1).reshape(C, Dh), f64(w2), f64(b2),
+                                           f64(wc))
+    ep, eu = np.abs(f64(probs) - want_p).max(), np.abs(f64(util) - want_u).max()
+    print(f"probs max-abs {ep:.2e}, utility max-abs {eu:.2e}")
+    # hid is rounded to bf16 (2^-9 relative, Dh independent terms): logit error ~ 2^-9 |logit| -> prob error <= 1/4 of it
+    assert ep <= 2e-3 and eu <= 2e-3 * float(wc.sum())
+
+
+def test_topk_matches_oracle_bit_for_bit(P):
+    dev = "cuda"
+    rng = np.random.default_rng(5)
+    counts = np.array([0, 1, 5, 1000, 37, 4096, 129, 0, 2], dtype=np.int64)
+    co = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    util_h = (rng.integers(-50, 50, size=co[-1]) / 16.0).astype(np.float32)     # many exact ties
+    util_h[7] = -0.0
+    util = torch.from_numpy(util_h).to(dev)
+    for K in (1, 10, 300):
+        idx = torch.full((len(counts), K), -7, dtype=torch.int32, device=dev)
+        cnt = torch.full((len(counts),), -7, dtype=torch.int32, device=dev)
+        P.upr_topk_per_user(util, torch.from_numpy(co).to(dev), K, int(counts.max()), idx, cnt)
+        torch.cuda.synchronize()
+        want_idx, want_cnt = oracle.topk_per_user(util_h, co, K)
+        assert np.array_equal(cnt.cpu().numpy(), want_cnt)
+        assert np.array_equal(idx.cpu().numpy(), want_idx)
+    with pytest.raises(P.UprError) as e:
+        P.upr_topk_per_user(util, torch.from_numpy(co).to(dev), 4, 20000, idx, cnt)
+    assert e.value.status == 2
+
+
+_CHILD = r"""
+import sys, numpy as np, torch
+sys.path.insert(0, {root!r})
+import paper_2606_00422_b200 as P
+handle = bytes.fromhex(sys.argv[1]); n = int(sys.argv[2])
+ptr = P.upr_pool_open(handle)
+# wrap the mapped allocation (no copy) and read it; then run the attention on it in place
+import ctypes
+class _Arr:  # minimal __cuda_array_interface__ holder
+    def __init__(self, ptr, n): self.__cuda_array_interface__ = dict(shape=(n,), typestr='<i2', data=(ptr, False), version=3)
+t = torch.as_tensor(_Arr(ptr, n), device='cuda')
+print('SUM', int(t.to(torch.int64).sum().item()))
+del t
+P.upr_pool_close(ptr)
+"""
+
+
+def test_pool_crosses_process_boundary_through_cuda_ipc(P, tmp_path):
+    """the retrieval process allocates the pool and exports an IPC handle 'to a per-instance
+    file'; the ranking process opens it and reads the same physical allocation.  Parent = retrieval replica,
+    child = ranking consumer."""
+    pool = (torch.arange(0, 50000, device="cuda") % 30011).to(torch.int16)     # stands in for the bf16 pool's bits
+    torch.cuda.synchronize()
+    handle = P.upr_pool_export(pool)
+    (tmp_path / "pool.handle").write_bytes(handle)                             # the per-instance file
+    script = tmp_path / "child.py"
+    script.write_text(_CHILD.format(root=ROOT))
+    r = subprocess.run([sys.executable, str(script), (tmp_path / "pool.handle").read_bytes().hex(), str(pool.numel())],
+                       capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    assert f"SUM {int(pool.to(torch.int64).sum().item())}" in r.stdout
+
+
+def test_slot_ring_round_robin(P):
+    ring = P.SlotRing(5)
+    assert ring.acquire(3).tolist() == [0, 1, 2]
+    assert ring.acquire(4).tolist() == [3, 4, 0, 1]
+    with pytest.raises(P.UprError):
+        ring.acquire(6)
