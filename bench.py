@@ -191,6 +191,84 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ----------------------------------------------------------------------------- ranking tail
+def ranking_tail(P, w, attn, q, k_self, v_self, q_host, stream, dev, ev, n_heads=4, d_head_hidden=128, top_k=100,
+                 iters=5):
+    """Synthetic-weight tail of the ranking pass on the last layer's attention output.
+    Returns per-kernel times, GEMM TFLOP/s and an end-to-end figure where only the top-K indices return to the host."""
+    import math
+    D = w.H * w.d
+    M = w.total_q
+
+    def wgt(tag, n, k):
+        return (S.normal_bf16(w.seed, tag, (n, k), dev).float() / math.sqrt(k)).to(torch.bfloat16)
+    w_o, w_1 = wgt("w_o", D, D), wgt("w_head1", n_heads * d_head_hidden, D)
+    b_1 = torch.zeros(n_heads * d_head_hidden, dtype=torch.float32, device=dev)
+    w_2 = S.normal_bf16(w.seed, "w_head2", (n_heads, d_head_hidden), dev).float() / math.sqrt(d_head_hidden)
+    b_2 = torch.zeros(n_heads, dtype=torch.float32, device=dev)
+    w_c = torch.ones(n_heads, dtype=torch.float32, device=dev)
+    z = torch.empty((M, D), dtype=torch.bfloat16, device=dev)
+    hid = torch.empty((M, n_heads * d_head_hidden), dtype=torch.bfloat16, device=dev)
+    util = torch.empty(M, dtype=torch.float32, device=dev)
+    idx = torch.empty((w.B, top_k), dtype=torch.int32, device=dev)
+    cnt = torch.empty(w.B, dtype=torch.int32, device=dev)
+    idx_host = torch.empty((w.B, top_k), dtype=torch.int32).pin_memory()
+    max_c = int(w.cand_counts.max())
+    marks = [ev() for _ in range(5)]
+
+    def tail_once(out_last, record=False):
+        x = out_last.view(M, D)
+        if record:
+            marks[0].record(stream)
+        P.upr_linear_fwd(x, w_o, None, z, P.UPR_ACT_NONE, stream)                 # out-projection
+        if record:
+            marks[1].record(stream)
+        P.upr_linear_fwd(z, w_1, b_1, hid, P.UPR_ACT_SILU, stream)                # heads, first layers
+        if record:
+            marks[2].record(stream)
+        P.upr_action_utility(hid, w_2, b_2, w_c, None, util, stream)              # logits -> probabilities -> utility
+        if record:
+            marks[3].record(stream)
+        P.upr_topk_per_user(util, attn.cand_offsets, top_k, max_c, idx, cnt, stream)
+        if record:
+            marks[4].record(stream)
+    out = attn(q, k_self, v_self, stream=stream)
+    for _ in range(2):
+        tail_once(out[-1])
+    torch.cuda.synchronize()
+    ts = np.zeros(4)
+    for _ in range(iters):
+        tail_once(out[-1], record=True)
+        torch.cuda.synchronize()
+        ts += np.array([marks[i].elapsed_time(marks[i + 1]) for i in range(4)])
+    ts /= iters
+    # end to end, ranked: queries up, attention + tail on the device, K indices per user back
+    q_dev = torch.empty_like(q)
+    e0, e1 = ev(), ev()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(iters):
+        q_dev.copy_(q_host, non_blocking=True)
+        o = attn(q_dev, k_self, v_self, stream=stream)
+        tail_once(o[-1])
+        idx_host.copy_(idx, non_blocking=True)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / iters
+    assert int(idx_host.max()) < M and int(cnt.min()) >= 0
+    fl_o, fl_h = 2.0 * M * D * D, 2.0 * M * D * n_heads * d_head_hidden
+    return {"shapes": {"M": M, "D_model": D, "action_heads": n_heads, "head_hidden": d_head_hidden, "top_k": top_k},
+            "out_proj_ms": float(ts[0]), "out_proj_tflops": fl_o / (ts[0] * 1e-3) / 1e12,
+            "heads_gemm_ms": float(ts[1]), "heads_gemm_tflops": fl_h / (ts[1] * 1e-3) / 1e12,
+            "utility_ms": float(ts[2]), "utility_gbs": (hid.numel() * 2 + M * 4) / (ts[2] * 1e-3) / 1e9,
+            "topk_ms": float(ts[3]),
+            "e2e_ranked": {"value": M / (ms * 1e-3), "unit": "candidates/s", "ms_per_step": ms,
+                           "h2d_bytes_per_step": q_host.numel() * q_host.element_size(),
+                           "d2h_bytes_per_step": idx_host.numel() * 4,
+                           "what": "q up, all layers' attention + out-projection + action heads + utility + top-K on the "
+                                   "device, K indices per user back"}}
+
+
 # ----------------------------------------------------------------------------- CUDA arm
 def run_ours(args):
     import paper_2606_00422_b200 as P
@@ -354,6 +432,14 @@ def run_ours(args):
     torch.cuda.synchronize()
     assert torch.equal(out_host[0, :64], layer_attn[0].out[0, :64].cpu()), "e2e result did not reach the host"
 
+    # ---- the rest of the ranking pass on the device, reported beside the hot path: the
+    # last layer's attention output -> out-projection (tcgen05 GEMM, fp32 rows converted in-kernel) -> stacked
+    # first layers of the per-action heads (GEMM + SiLU) -> probabilities -> utility -> per-user top-K.  With it
+    # the attention output never leaves the chip: only K indices per user go back to the host.
+    tail = None
+    if not args.skip_tail and w.q_dtype == "bf16":
+        tail = ranking_tail(P, w, attn, q, k_self, v_self, q_host, stream, dev, ev)
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -386,7 +472,8 @@ def run_ours(args):
              "attn_candidates_per_s": w.total_q / (attn_ms * 1e-3), "splits": attn.splits,
              "kv_source": "pool (zero copy)" if zero_copy else "packed decode cache",
              "packed_variant": None if other is None else dict(
-                 other, pack_gbs=pack_bytes / (other["pack_ms"] * 1e-3) / 1e9)}
+                 other, pack_gbs=pack_bytes / (other["pack_ms"] * 1e-3) / 1e9),
+             "ranking_tail": tail}
 
     # ---- CPU baseline: the oracle as it stands, bounded sample, host cores of this box
     cpu_baseline = None
@@ -430,6 +517,7 @@ def main():
                     help="attention kernel: the library's choice, or force the 1-CTA / CTA-pair kernel (A/B runs)")
     ap.add_argument("--skip-packed-variant", action="store_true",
                     help="leave out the secondary pack + attention leg of a zero-copy run")
+    ap.add_argument("--skip-tail", action="store_true", help="leave out the ranking-tail legs (detail.ranking_tail)")
     ap.add_argument("--skip-cpu-baseline", action="store_true",
                     help="leave out the oracle timing leg (used for the ncu captures under profiles/)")
     args = ap.parse_args()
