@@ -18,7 +18,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "upr_oracle.c")
 _LIB = os.path.join(_HERE, "libupr_oracle.so")
 
-F32, BF16, FP8_E4M3 = 0, 1, 2
+F32, BF16, FP8_E4M3, FP8_E4M3_USER = 0, 1, 2, 3
 ROW_ALIGN = 16  # DESIGN.md reading Q14
 
 
@@ -112,7 +112,8 @@ def pack(pool_bits: np.ndarray, slot_ids, seq_lens, dtype: int, align: int = ROW
     B = int(seq_lens.shape[0])
     lay = layout(seq_lens, H, d, n_layers, dtype, align, tail_rows)
     cache = np.zeros(lay["bytes_cache"], dtype=np.uint8)
-    scales = np.zeros(n_layers * H, dtype=np.float32) if dtype == FP8_E4M3 else None
+    scales = (np.zeros(n_layers * H, dtype=np.float32) if dtype == FP8_E4M3 else
+              np.zeros(n_layers * B * H, dtype=np.float32) if dtype == FP8_E4M3_USER else None)
     rc = lib().upro_pack(_p(pool_bits), n_layers, S, H, n_max, d, _p(slot_ids), _p(seq_lens), B, dtype, align,
                          tail_rows, _p(cache), _p(scales))
     if rc:
@@ -188,7 +189,7 @@ def cross_attn_packed(q, q_dtype: int, k_cache, v_cache, kv_dtype: int, seq_lens
     if sm_scale is None:
         sm_scale = 1.0 / np.sqrt(d)
     qdt = np.float32 if q_dtype == F32 else np.uint16
-    kdt = {F32: np.float32, BF16: np.uint16, FP8_E4M3: np.uint8}[kv_dtype]
+    kdt = {F32: np.float32, BF16: np.uint16, FP8_E4M3: np.uint8, FP8_E4M3_USER: np.uint8}[kv_dtype]
     q = np.ascontiguousarray(q, dtype=qdt)
     assert q.size == n_layers * total_q * H * d
     k_cache = np.ascontiguousarray(k_cache).view(kdt)

@@ -37,6 +37,8 @@
 #define UPRO_F32 0
 #define UPRO_BF16 1
 #define UPRO_FP8_E4M3 2
+#define UPRO_FP8_E4M3_USER 3 /* E4M3 bytes, one scale per (layer, USER, head): SURVEY.md 8(f)3, reading Q18 */
+#define UPRO_IS_FP8(dt) ((dt) == UPRO_FP8_E4M3 || (dt) == UPRO_FP8_E4M3_USER)
 
 int upro_num_threads(void) {
 #ifdef _OPENMP
@@ -147,7 +149,8 @@ int upro_layout(const int32_t* seq_lens, int B, int H, int d, int n_layers, int 
   out7[3] = acc * eb * d;
   out7[4] = (int64_t)H * acc * eb * d;
   out7[5] = ((int64_t)n_layers * H * acc + tail_rows) * eb * d;
-  out7[6] = (dtype == UPRO_FP8_E4M3) ? (int64_t)n_layers * H * 4 : 0;
+  out7[6] = (dtype == UPRO_FP8_E4M3) ? (int64_t)n_layers * H * 4
+            : (dtype == UPRO_FP8_E4M3_USER) ? (int64_t)n_layers * B * H * 4 : 0;
   return 0;
 }
 
@@ -204,9 +207,21 @@ int upro_pack(const uint16_t* pool, int n_layers, int S, int H, int n_max, int d
             pool + ((((int64_t)l * S + slot_ids[b]) * H + h) * n_max) * (int64_t)d;
         int64_t dst0 = (((int64_t)l * H + h) * R + row_off[b]) * (int64_t)d;
         int64_t n = (int64_t)seq_lens[b] * d;
+        if (dtype == UPRO_FP8_E4M3_USER) {
+          /* the same rule as above, amax over THIS user's valid rows of the (layer, head) only:
+             a cache that is written user by user (incrementally) never needs another user's rows */
+          float amax = 0.0f;
+          for (int64_t i = 0; i < n; ++i) {
+            float v = fabsf((float)upro_bf16_to_f64(src[i]));
+            if (v > amax) amax = v;
+          }
+          int64_t si = ((int64_t)l * B + b) * H + h;
+          scales[si] = amax > 0.0f ? amax / 448.0f : 1.0f;
+          mult = amax > 0.0f ? 448.0f / amax : 1.0f;
+        }
         if (dtype == UPRO_BF16) {
           memcpy((uint16_t*)cache + dst0, src, (size_t)n * 2);
-        } else if (dtype == UPRO_FP8_E4M3) {
+        } else if (UPRO_IS_FP8(dtype)) {
           uint8_t* dst = (uint8_t*)cache + dst0;
           for (int64_t i = 0; i < n; ++i) {
             float x = (float)upro_bf16_to_f64(src[i]);
@@ -446,8 +461,9 @@ int upro_cross_attn_packed(const void* q, int q_dtype, const void* k_cache, cons
     int C = cand_offsets[b + 1] - cand_offsets[b];
     int L = seq_lens[b];
     if (C <= 0) continue;
-    double ks = (kv_dtype == UPRO_FP8_E4M3 && k_scale) ? (double)k_scale[l * H + h] : 1.0;
-    double vs = (kv_dtype == UPRO_FP8_E4M3 && v_scale) ? (double)v_scale[l * H + h] : 1.0;
+    int64_t si = (kv_dtype == UPRO_FP8_E4M3_USER) ? ((int64_t)l * B + b) * H + h : (int64_t)l * H + h;
+    double ks = (UPRO_IS_FP8(kv_dtype) && k_scale) ? (double)k_scale[si] : 1.0;
+    double vs = (UPRO_IS_FP8(kv_dtype) && v_scale) ? (double)v_scale[si] : 1.0;
     double* qb = (double*)malloc(sizeof(double) * (size_t)C * d);
     double* ob = (double*)malloc(sizeof(double) * (size_t)C * d);
     double* Kb = (double*)malloc(sizeof(double) * (size_t)(L > 0 ? L : 1) * d);

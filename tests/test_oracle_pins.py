@@ -363,6 +363,54 @@ def test_pack_fp8_scales_and_bytes_against_torch(oracle):
             assert (np.abs(oracle.e4m3_decode(c[l, h])) == 448.0).any()
 
 
+def test_pack_fp8_per_user_scales_against_torch_and_single_user_packs(oracle):
+    """FP8_E4M3_USER (reading Q18): one scale per (layer, USER, head), amax over that user's valid
+    rows only.  Pinned (i) against torch's float8 cast of the same fp32 products and (ii) against the already
+    pinned per-(layer, head) pack of each user ALONE (a batch of one has exactly that user's amax)."""
+    r = rng(18)
+    n_layers, S, H, n_max, d = 2, 4, 2, 24, 16
+    pool_t, pool_bits = _pool(r, n_layers, S, H, n_max, d)
+    slot = np.array([2, 1, 3, 0], np.int32)
+    L = np.array([24, 5, 0, 17], np.int32)
+    B = len(L)
+    cache, scales = oracle.pack(pool_bits, slot, L, oracle.FP8_E4M3_USER, tail_rows=0)
+    lay = oracle.layout(L, H, d, n_layers, oracle.FP8_E4M3_USER, tail_rows=0)
+    assert lay["bytes_scales"] == n_layers * B * H * 4 and scales.shape == (n_layers * B * H,)
+    R, ro = lay["R"], lay["row_off"]
+    c = cache.reshape(n_layers, H, R, d)
+    sc = scales.reshape(n_layers, B, H)
+    pf = pool_t.to(torch.float32)
+    for b in range(B):
+        alone, s_alone = oracle.pack(pool_bits, slot[b:b + 1], L[b:b + 1], oracle.FP8_E4M3, tail_rows=0)
+        Rb = oracle.layout(L[b:b + 1], H, d, n_layers, oracle.FP8_E4M3, tail_rows=0)["R"]
+        alone = alone.reshape(n_layers, H, Rb, d)
+        for l in range(n_layers):
+            for h in range(H):
+                assert sc[l, b, h] == s_alone[l * H + h]
+                assert np.array_equal(c[l, h, ro[b]: ro[b] + L[b]], alone[l, h, : L[b]])
+                if L[b] == 0:
+                    assert sc[l, b, h] == 1.0
+                    continue
+                amax = float(pf[l, slot[b], h, : L[b]].abs().max())
+                assert sc[l, b, h] == np.float32(amax) / np.float32(448.0)
+                y = pf[l, slot[b], h, : L[b]] * torch.tensor(np.float32(448.0) / np.float32(amax))
+                assert np.array_equal(c[l, h, ro[b]: ro[b] + L[b]], y.to(torch.float8_e4m3fn).view(torch.uint8).numpy())
+    # the whole-batch driver indexes the scales per user: equal to per-block calls on the dequantised values
+    C = np.array([3, 2, 4, 1])
+    co = np.concatenate([[0], np.cumsum(C)]).astype(np.int32)
+    q = r.standard_normal((n_layers, co[-1], H, d)).astype(np.float32)
+    vc, vs = oracle.pack(pool_bits[:, ::-1].copy(), slot, L, oracle.FP8_E4M3_USER, tail_rows=0)
+    out = oracle.cross_attn_packed(q, oracle.F32, cache, vc, oracle.FP8_E4M3_USER, L, co, H, d, n_layers, scales, vs)
+    vcr, vsr = vc.reshape(n_layers, H, R, d), vs.reshape(n_layers, B, H)
+    for l in range(n_layers):
+        for b in range(B):
+            for h in range(H):
+                K = oracle.e4m3_decode(c[l, h, ro[b]: ro[b] + L[b]]) * float(sc[l, b, h])
+                V = oracle.e4m3_decode(vcr[l, h, ro[b]: ro[b] + L[b]]) * float(vsr[l, b, h])
+                want = oracle.attn_block(q[l, co[b]:co[b + 1], h].astype(np.float64), K, V)
+                np.testing.assert_allclose(out[l, co[b]:co[b + 1], h], want, rtol=0, atol=1e-13)
+
+
 def test_pack_fp8_zero_head_has_unit_scale(oracle):
     pool = np.zeros((1, 1, 1, 4, 8), np.uint16)
     cache, scales = oracle.pack(pool, [0], [4], oracle.FP8_E4M3, tail_rows=0)
