@@ -52,7 +52,10 @@ typedef enum {
   UPR_ERR_CUDA = 4         /* a CUDA runtime/driver call failed (message in upr_last_error) */
 } upr_status;
 
-typedef enum { UPR_F32 = 0, UPR_BF16 = 1, UPR_FP8_E4M3 = 2 } upr_dtype;
+/* UPR_FP8_E4M3: E4M3 bytes with one fp32 scale per (layer, head); UPR_FP8_E4M3_USER: the same bytes format with
+ * one scale per (layer, USER, head) -- amax over that user's valid rows only, for caches written user by user
+ * (SURVEY.md 8(f)3).  Scale tables: fp32 [n_layers, H] resp. [n_layers, B, H]. */
+typedef enum { UPR_F32 = 0, UPR_BF16 = 1, UPR_FP8_E4M3 = 2, UPR_FP8_E4M3_USER = 3 } upr_dtype;
 typedef enum { UPR_KV_PACKED = 0, UPR_KV_POOL = 1 } upr_kv_source;
 typedef enum { UPR_KERNEL_AUTO = 0, UPR_KERNEL_SINGLE = 1, UPR_KERNEL_PAIR = 2 } upr_kernel_choice;
 
@@ -71,7 +74,7 @@ typedef struct upr_kv_layout {
   int64_t head_stride_bytes;
   int64_t layer_stride_bytes;
   int64_t bytes_cache;  /* bytes of ONE cache (K or V), tail rows included */
-  int64_t bytes_scales; /* bytes of ONE scale table: n_layers*H*4 for FP8, else 0 */
+  int64_t bytes_scales; /* bytes of ONE scale table: n_layers*H*4 (FP8), n_layers*B*H*4 (FP8 per user), else 0 */
 } upr_kv_layout;
 
 /*
@@ -136,7 +139,7 @@ typedef struct upr_attn_params {
   float* out;                  /* device fp32 [n_layers, total_q, H, d] */
   const void* k_self;          /* device, same shape/dtype as q, or NULL: the candidate's own */
   const void* v_self;          /*   key/value joins its softmax (PAPER.md:198 identity mask) */
-  const float* k_scale;        /* device fp32 [n_layers*H] or NULL (=1): FP8 dequant scales */
+  const float* k_scale;        /* device fp32 [n_layers*H] ([n_layers*B*H] for UPR_FP8_E4M3_USER) or NULL (=1) */
   const float* v_scale;
   int32_t B, H, d, n_layers;
   int32_t kv_dtype;            /* upr_dtype of the caches */

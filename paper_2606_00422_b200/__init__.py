@@ -6,7 +6,7 @@ argument marshalling only; every step of the path runs in the CUDA kernels under
 There is no CPU fallback: importing the binding fails loudly when the library is missing.
 """
 from .binding import (  # noqa: F401
-    UPR_BF16, UPR_F32, UPR_FP8_E4M3, UPR_KV_PACKED, UPR_KV_POOL, UPR_KERNEL_AUTO,
+    UPR_BF16, UPR_F32, UPR_FP8_E4M3, UPR_FP8_E4M3_USER, UPR_KV_PACKED, UPR_KV_POOL, UPR_KERNEL_AUTO,
     UPR_KERNEL_SINGLE, UPR_KERNEL_PAIR, UPR_ROW_ALIGN, UPR_TAIL_ROWS, KvLayout, UprError, lib_path,
     upr_cross_attn_fwd, upr_cross_attn_fwd_ex, upr_cross_attn_num_splits, upr_cross_attn_workspace_bytes,
     upr_kv_cache_layout, upr_kv_pack, upr_last_attn_kernel, upr_linear_fwd, upr_action_utility,

@@ -8,7 +8,7 @@ from typing import Optional
 import numpy as np
 import torch
 
-UPR_F32, UPR_BF16, UPR_FP8_E4M3 = 0, 1, 2
+UPR_F32, UPR_BF16, UPR_FP8_E4M3, UPR_FP8_E4M3_USER = 0, 1, 2, 3
 UPR_KV_PACKED, UPR_KV_POOL = 0, 1
 UPR_KERNEL_AUTO, UPR_KERNEL_SINGLE, UPR_KERNEL_PAIR = 0, 1, 2
 UPR_ROW_ALIGN, UPR_TAIL_ROWS = 16, 128

@@ -83,6 +83,7 @@ struct AttnArgs {
   int pool_S, pool_n;
   int B, H, n_layers, num_splits;
   int q_is_f32;
+  int scale_per_user;     // FP8 scales indexed [layer, user, head] instead of [layer, head]
   int q_tma;              // 1: tmap_q describes `q` as [n_layers*total_q, H*D] bf16: the producer loads Q tiles by TMA
   int out_tma;            // 1: tmap_out describes `out` as [n_layers*total_q, H*D] fp32 (full tiles use TMA stores)
   float scale_log2;       // sm_scale * log2(e)
@@ -97,6 +98,7 @@ struct WorkItem {
   int key0;      // first key index (within the user) of this split
   int n_keys;    // valid keys in this split's range (>= 0)
   int total_q;   // cand_offsets[B]
+  int b;         // user
 };
 
 template <int D, int KV>
@@ -453,6 +455,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
         it.key0 = key0;
         it.n_keys = n_keys;
         it.total_q = total_q;
+        it.b = b;
         mbar_arrive(smem_u32(&ctrl->item_full[islot]));
         // stream this item's K/V tiles: K0 V0 K1 V1 ...
         const int nt = (n_keys + kTileN - 1) / kTileN;
@@ -770,7 +773,7 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
           if (lane == 0) mbar_arrive(smem_u32(&ctrl->q_full[t]));
           q_prefetched = false;
         }
-        const int sidx = it.layer * args.H + it.h;
+        const int sidx = args.scale_per_user ? (it.layer * args.B + it.b) * args.H + it.h : it.layer * args.H + it.h;
         const float ks = args.k_scale ? __ldg(args.k_scale + sidx) : 1.0f;
         const float c_log2 = args.scale_log2 * ks;  // multiplies raw S
 
@@ -936,7 +939,9 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
       if (!it.valid) break;
       const int nt = (it.n_keys + kTileN - 1) / kTileN;
       const bool self_here = has_self && it.split == 0;
-      const float vs = args.v_scale ? __ldg(args.v_scale + it.layer * args.H + it.h) : 1.0f;
+      const float vs = args.v_scale ? __ldg(args.v_scale + (args.scale_per_user ? (it.layer * args.B + it.b) * args.H + it.h
+                                                                                 : it.layer * args.H + it.h))
+                                    : 1.0f;
 #pragma unroll 1
       for (int t = 0; t < 2; ++t) {
         const int rows_here = min(kTileM, it.n_rows - t * kTileM);

@@ -62,6 +62,7 @@ struct PackArgs {
   const int32_t* slot_ids;
   const int32_t* seq_lens;
   int B, H, d, n_layers, S, n_max, tail_rows;
+  int per_user;               // FP8: one scale per (layer, user, head) instead of per (layer, head)
 };
 
 // MODE 0: bf16 copy, 1: fp8 quantise, 2: fp32 widen, 3: amax pass (no cache write)
@@ -113,11 +114,12 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
         const int slot = __ldg(a.slot_ids + b);
         const __nv_bfloat16* src =
             a.pool + ((((static_cast<size_t>(l) * a.S + slot) * a.H + h) * a.n_max) + j0) * D;
-        lh_u[u] = lh;
+        // index of the scale (and, in the amax pass, of the running maximum) this block belongs to
+        lh_u[u] = a.per_user ? (l * a.B + b) * a.H + h : lh;
         dst_elem[u] = (static_cast<size_t>(lh) * R + row) * D;
         const int valid_chunks = valid_rows * CPR;
         if (MODE == 1) {
-          const float amax = a.scale[lh];
+          const float amax = a.scale[lh_u[u]];
           mult[u] = amax > 0.f ? __fdiv_rn(448.0f, amax) : 1.0f;
         }
 #pragma unroll

@@ -155,7 +155,8 @@ upr_status validate(const upr_attn_params* p) {
                 p->B, p->H, p->n_layers, (long long)p->total_q);
   if (p->d != 64 && p->d != 128)
     return fail(UPR_ERR_UNSUPPORTED, "head dim d=%d unsupported (64 or 128)", p->d);
-  if (p->kv_dtype != UPR_BF16 && p->kv_dtype != UPR_FP8_E4M3 && p->kv_dtype != UPR_F32)
+  if (p->kv_dtype != UPR_BF16 && p->kv_dtype != UPR_FP8_E4M3 && p->kv_dtype != UPR_F32 &&
+      p->kv_dtype != UPR_FP8_E4M3_USER)
     return fail(UPR_ERR_UNSUPPORTED, "kv_dtype %d unsupported (f32, bf16 or fp8 e4m3)", p->kv_dtype);
   if (p->q_dtype != UPR_BF16 && p->q_dtype != UPR_F32)
     return fail(UPR_ERR_UNSUPPORTED, "q_dtype %d unsupported (bf16 or f32)", p->q_dtype);
@@ -217,7 +218,8 @@ upr_status launch_attn_d(int kv_dtype, const upr::AttnArgs& a, const CUtensorMap
                          cudaStream_t st) {
   switch (kv_dtype) {
     case UPR_BF16: return launch_attn<D, upr::KV_BF16>(a, tk, tv, to, tq, grid, st);
-    case UPR_FP8_E4M3: return launch_attn<D, upr::KV_FP8>(a, tk, tv, to, tq, grid, st);
+    case UPR_FP8_E4M3:
+    case UPR_FP8_E4M3_USER: return launch_attn<D, upr::KV_FP8>(a, tk, tv, to, tq, grid, st);
     default: return launch_attn<D, upr::KV_F32>(a, tk, tv, to, tq, grid, st);
   }
 }
@@ -385,6 +387,7 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   a.n_layers = p->n_layers;
   a.num_splits = ns;
   a.q_is_f32 = (p->q_dtype == UPR_F32);
+  a.scale_per_user = (p->kv_dtype == UPR_FP8_E4M3_USER);
   if (p->kv_source == UPR_KV_POOL) {
     a.slot_ids = p->slot_ids;
     a.pool_S = p->pool_slots;
@@ -475,7 +478,7 @@ upr_status upr_kv_cache_layout(const int32_t* seq_lens, int B, int H, int d, int
   if (B < 0 || H <= 0 || n_layers <= 0 || d <= 0 || (B > 0 && seq_lens == nullptr))
     return fail(UPR_ERR_INVALID_ARG, "bad sizes (B=%d H=%d d=%d n_layers=%d)", B, H, d, n_layers);
   if (d != 64 && d != 128) return fail(UPR_ERR_UNSUPPORTED, "head dim d=%d unsupported", d);
-  if (dtype != UPR_F32 && dtype != UPR_BF16 && dtype != UPR_FP8_E4M3)
+  if (dtype != UPR_F32 && dtype != UPR_BF16 && dtype != UPR_FP8_E4M3 && dtype != UPR_FP8_E4M3_USER)
     return fail(UPR_ERR_UNSUPPORTED, "dtype %d unsupported", (int)dtype);
   int64_t acc = 0;
   if (row_off) row_off[0] = 0;
@@ -500,7 +503,9 @@ upr_status upr_kv_cache_layout(const int32_t* seq_lens, int B, int H, int d, int
   out->head_stride_bytes = acc * eb * d;
   out->layer_stride_bytes = static_cast<int64_t>(H) * acc * eb * d;
   out->bytes_cache = (static_cast<int64_t>(n_layers) * H * acc + UPR_TAIL_ROWS) * eb * d;
-  out->bytes_scales = (dtype == UPR_FP8_E4M3) ? static_cast<int64_t>(n_layers) * H * 4 : 0;
+  out->bytes_scales = (dtype == UPR_FP8_E4M3)        ? static_cast<int64_t>(n_layers) * H * 4
+                      : (dtype == UPR_FP8_E4M3_USER) ? static_cast<int64_t>(n_layers) * B * H * 4
+                                                      : 0;
   return UPR_OK;
 }
 
@@ -517,7 +522,8 @@ upr_status upr_kv_pack(const void* k_pool, const void* v_pool, int S, int n_max,
   if (lay->B == 0) return UPR_OK;  // nothing to gather; tail untouched
   if (slot_ids == nullptr || seq_lens == nullptr)
     return fail(UPR_ERR_INVALID_ARG, "slot_ids / seq_lens is NULL");
-  const bool fp8 = lay->dtype == UPR_FP8_E4M3;
+  const bool per_user = lay->dtype == UPR_FP8_E4M3_USER;
+  const bool fp8 = lay->dtype == UPR_FP8_E4M3 || per_user;
   if (fp8 && ((k_pool && !k_scale) || (v_pool && !v_scale)))
     return fail(UPR_ERR_INVALID_ARG, "FP8 pack needs scale outputs");
   upr_status s = check_device();
@@ -526,7 +532,7 @@ upr_status upr_kv_pack(const void* k_pool, const void* v_pool, int S, int n_max,
   const size_t smem = (static_cast<size_t>(lay->B) + 1) * sizeof(int);
   if (smem > 40 * 1024) return fail(UPR_ERR_UNSUPPORTED, "B=%d too large for the pack kernel", lay->B);
   const int grid = sm_count() * 8;
-  const int n_scale = lay->n_layers * lay->H;
+  const int n_scale = lay->n_layers * lay->H * (per_user ? lay->B : 1);
   for (int which = 0; which < 2; ++which) {
     const void* pool = which == 0 ? k_pool : v_pool;
     if (pool == nullptr) continue;
@@ -543,6 +549,7 @@ upr_status upr_kv_pack(const void* k_pool, const void* v_pool, int S, int n_max,
     a.S = S;
     a.n_max = n_max;
     a.tail_rows = lay->tail_rows;
+    a.per_user = per_user ? 1 : 0;
     const bool d64 = lay->d == 64;
 #define UPR_PACK_LAUNCH(MODE)                                                              \
   do {                                                                                     \

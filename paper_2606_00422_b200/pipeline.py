@@ -14,7 +14,7 @@ import torch
 from . import binding as B_
 
 _TORCH_DT = {B_.UPR_F32: torch.float32, B_.UPR_BF16: torch.bfloat16}
-DTYPE_ID = {"f32": B_.UPR_F32, "bf16": B_.UPR_BF16, "fp8": B_.UPR_FP8_E4M3}
+DTYPE_ID = {"f32": B_.UPR_F32, "bf16": B_.UPR_BF16, "fp8": B_.UPR_FP8_E4M3, "fp8_user": B_.UPR_FP8_E4M3_USER}
 
 
 @dataclasses.dataclass
@@ -35,9 +35,9 @@ def alloc_cache(seq_lens_host, H: int, d: int, n_layers: int, kv_dtype: int, dev
     k = torch.empty(lay.bytes_cache, dtype=torch.uint8, device=device)
     v = torch.empty(lay.bytes_cache, dtype=torch.uint8, device=device)
     ks = vs = None
-    if kv_dtype == B_.UPR_FP8_E4M3:
-        ks = torch.empty(n_layers * H, dtype=torch.float32, device=device)
-        vs = torch.empty(n_layers * H, dtype=torch.float32, device=device)
+    if lay.bytes_scales:
+        ks = torch.empty(lay.bytes_scales // 4, dtype=torch.float32, device=device)
+        vs = torch.empty(lay.bytes_scales // 4, dtype=torch.float32, device=device)
     sl = torch.as_tensor(np.asarray(seq_lens_host, dtype=np.int32), device=device)
     mx = int(np.max(seq_lens_host)) if len(seq_lens_host) else 0
     return DecodeCache(lay, row_off, k, v, ks, vs, sl, mx)

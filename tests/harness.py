@@ -8,7 +8,7 @@ import torch
 import oracle
 import upr_synth as S
 
-ORACLE_DT = {"f32": oracle.F32, "bf16": oracle.BF16, "fp8": oracle.FP8_E4M3}
+ORACLE_DT = {"f32": oracle.F32, "bf16": oracle.BF16, "fp8": oracle.FP8_E4M3, "fp8_user": oracle.FP8_E4M3_USER}
 
 
 def bits(t: torch.Tensor) -> np.ndarray:

@@ -336,6 +336,39 @@ def test_attention_fp8_cache_matches_oracle(P, case):
         print("no history of >= 300 keys in this case: pre-quantisation bar not applicable (DESIGN.md 6, T2)")
 
 
+@pytest.mark.parametrize("d", [64, 128])
+def test_fp8_per_user_scales_pack_and_attention(P, d):
+    """FP8 E4M3 cache with one scale per (layer, USER, head).  Pack: bytes and scales bit for bit
+    against the oracle; attention: against the oracle's whole-batch driver fed the same bytes and scales (the
+    kernel's bf16 MMA sees the dequantised values exactly), and 5e-2 against the pre-quantisation inputs for the
+    long histories.  One user has a 16x larger amplitude: with per-(layer, head) scales it would set everyone's
+    step; here every user keeps its own."""
+    L, C = [1000, 37, 0, 1300, 129], [130, 5, 3, 64, 257]
+    w = S.custom_workload("fp8_user", 4545, L, C, 2, d, 2, kv_dtype="fp8_user", self_term=True)
+    inp = Inputs(w, "cuda")
+    s3 = int(inp.slot_ids_host[3])
+    inp.k_pool[:, s3] *= 16.0
+    inp.v_pool[:, s3] *= 16.0
+    got, cache, attn = run_cuda(P, inp, num_splits=1)
+    kc, ks = oracle.pack(bits(inp.k_pool), inp.slot_ids_host, w.seq_lens, oracle.FP8_E4M3_USER)
+    vc, vs = oracle.pack(bits(inp.v_pool), inp.slot_ids_host, w.seq_lens, oracle.FP8_E4M3_USER)
+    assert np.array_equal(cache.k_scale.cpu().numpy().view(np.uint32), ks.view(np.uint32))
+    assert np.array_equal(cache.v_scale.cpu().numpy().view(np.uint32), vs.view(np.uint32))
+    assert np.array_equal(cache.k_cache.cpu().numpy(), kc) and np.array_equal(cache.v_cache.cpu().numpy(), vc)
+    want = oracle.cross_attn_packed(bits(inp.q), oracle.BF16, kc, vc, oracle.FP8_E4M3_USER, w.seq_lens, w.cand_offsets,
+                                    w.H, w.d, w.n_layers, ks, vs, bits(inp.k_self), bits(inp.v_self))
+    for ns in (1, 3):
+        if ns != 1:
+            got, _, _ = run_cuda(P, inp, num_splits=ns)
+        mx, rel = error_stats(got, want)
+        # user 3's values are 16x larger: scale the strict gate by the largest |v| of the batch
+        assert mx <= TOL_STRICT * 16 and rel <= TOL_RMS, (mx, rel)
+        rows = np.arange(w.cand_offsets[0], w.cand_offsets[1])                     # user 0: L = 1000, unit variance
+        assert error_stats(got[:, rows], want[:, rows])[0] <= TOL_STRICT
+        pre = oracle_all(inp)
+        assert error_stats(got[:, rows], pre[:, rows])[0] <= TOL_FP8
+
+
 def test_fp8_decode_is_exact_for_every_code(P):
     """L = 1: out = V[0] exactly, so a V row holding all 254 finite E4M3 codes reads the kernel's
     in-register dequantisation back bit for bit (decode(byte) * v_scale in fp32)."""

@@ -162,7 +162,7 @@ class Workload:
         return f
 
     def kv_elem_bytes(self) -> int:
-        return {"f32": 4, "bf16": 2, "fp8": 1}[self.kv_dtype]
+        return {"f32": 4, "bf16": 2, "fp8": 1, "fp8_user": 1}[self.kv_dtype]
 
     @property
     def kv_bytes(self) -> int:
