@@ -7,7 +7,7 @@
 //   warp 0      TMA producer: x tile [128 rows, 64 k] and W tile [128 outputs, 64 k] per stage
 //   warp 1      tcgen05.mma issuer (one elected thread), fp32 accumulators in TMEM, two of them so
 //               that the epilogue of tile i overlaps the MMAs of tile i + 1
-//   warps 2-3   converters (fp32 x only, e.g. the attention output): raw fp32 rows -> bf16 swizzled
+//   warps 2-3, 8-9  converters (fp32 x only, e.g. the attention output): raw fp32 rows -> bf16 swizzled
 //               MMA tile, so the activation never takes a separate cast pass through HBM
 //   warps 4-7   epilogue: TMEM -> registers, + bias, activation, store as bf16 or fp32
 // x: [M, K] bf16 or fp32 row-major; W: [N, K] bf16 row-major (one output feature per row);
@@ -19,18 +19,20 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cuda/std/type_traits>
+
 #include "ptx.cuh"
 
 namespace upr {
 namespace lin {
 
-constexpr int kThreads = 256;
+constexpr int kThreads = 320;
 constexpr int kBM = 128, kBN = 128, kBK = 64;
 constexpr int kTileBytes = kBM * kBK * 2;      // 16 KB: one bf16 operand tile
 constexpr int kRawBytes = kBM * kBK * 4;       // 32 KB: one fp32 x tile as loaded
 constexpr int kStages = 5;                     // (x, W) tile pairs
 constexpr int kRawStages = 2;
-constexpr int kConvThreads = 64;
+constexpr int kConvThreads = 128;          // warps 2, 3, 8, 9
 constexpr int kSmemCtrl = 1024;
 constexpr int kSmemTotal = kStages * 2 * kTileBytes + kRawStages * kRawBytes + kSmemCtrl + 1024;
 static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
@@ -75,13 +77,13 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < kStages; ++i) {
-      // fp32 x: the W bytes (producer's arrive.expect_tx) and the two converter warps complete a stage
-      mbar_init(smem_u32(&ctrl->full[i]), X_F32 ? 3 : 1);
+      // fp32 x: the W bytes (producer's arrive.expect_tx) and the four converter warps complete a stage
+      mbar_init(smem_u32(&ctrl->full[i]), X_F32 ? 5 : 1);
       mbar_init(smem_u32(&ctrl->empty[i]), 1);
     }
     for (int i = 0; i < kRawStages; ++i) {
       mbar_init(smem_u32(&ctrl->raw_full[i]), 1);
-      mbar_init(smem_u32(&ctrl->raw_empty[i]), 2);
+      mbar_init(smem_u32(&ctrl->raw_empty[i]), 4);
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(smem_u32(&ctrl->acc_full[i]), 1);
@@ -160,10 +162,10 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
       }
     }
     __syncwarp();
-  } else if (warp == 2 || warp == 3) {
+  } else if (warp == 2 || warp == 3 || warp >= 8) {
     // ================================================================= converters (fp32 x)
     if constexpr (X_F32) {
-      const int ctid = threadIdx.x - 64;   // 0..63
+      const int ctid = (warp < 4 ? warp - 2 : warp - 6) * 32 + lane;   // 0..127
       uint32_t it = 0, raw_it = 0;
       for (long long t = blockIdx.x; t < total_tiles; t += gridDim.x) {
         for (int ks = 0; ks < k_steps; ++ks, ++it, ++raw_it) {
@@ -192,8 +194,8 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
         }
       }
     }
-  } else if (warp >= 4) {
-    // ================================================================= epilogue
+  } else {
+    // ================================================================= epilogue (warps 4-7)
     const int ew = warp - 4;                                   // TMEM lane quarter
     const uint32_t lane_base = static_cast<uint32_t>(ew * 32) << 16;
     uint32_t n_acc = 0;
@@ -204,8 +206,10 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
       tc_fence_after();
       const long long row = static_cast<long long>(mb) * kBM + ew * 32 + lane;
       const bool row_ok = row < args.M;
-#pragma unroll 1
-      for (int c0 = 0; c0 < kBN; c0 += 32) {
+      // one 32-column chunk: + bias, activation, store.  The activation is a compile-time branch (the
+      // per-element form with run-time tests made the epilogue, not the MMAs, the bound of the kernel)
+      auto chunk = [&](auto act_tag, const int c0) {
+        constexpr int kAct = decltype(act_tag)::value;
         uint32_t r[32];
         tmem_ld32(tmem_base + lane_base + ab * kBN + c0, r);
         tmem_wait_ld_regs(r);
@@ -215,33 +219,43 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
           if (lane == 0) mbar_arrive(smem_u32(&ctrl->acc_empty[ab]));
         }
         const int col0 = nb * kBN + c0;
-        if (col0 >= args.N) continue;
-        float v[32];
-#pragma unroll
-        for (int c = 0; c < 32; ++c) {
-          float x = __uint_as_float(r[c]);
-          if (args.bias != nullptr && col0 + c < args.N) x += __ldg(args.bias + col0 + c);
-          if (args.act == ACT_SILU) x = x / (1.0f + __expf(-x));
-          else if (args.act == ACT_RELU) x = fmaxf(x, 0.f);
-          v[c] = x;
-        }
-        if (!row_ok) continue;
+        if (col0 >= args.N || !row_ok) return;
         // N % 8 == 0: 8-column groups are either whole or absent
-        if (args.y_is_f32) {
-          float* dst = static_cast<float*>(args.y) + row * args.N + col0;
 #pragma unroll
-          for (int c = 0; c < 32; c += 4)
-            if (col0 + c < args.N)
-              *reinterpret_cast<float4*>(dst + c) = make_float4(v[c], v[c + 1], v[c + 2], v[c + 3]);
-        } else {
-          __nv_bfloat16* dst = static_cast<__nv_bfloat16*>(args.y) + row * args.N + col0;
+        for (int c = 0; c < 32; c += 8) {
+          if (col0 + c >= args.N) break;
+          float v[8];
 #pragma unroll
-          for (int c = 0; c < 32; c += 8)
-            if (col0 + c < args.N)
-              *reinterpret_cast<uint4*>(dst + c) =
-                  make_uint4(pack_bf16x2(v[c], v[c + 1]), pack_bf16x2(v[c + 2], v[c + 3]),
-                             pack_bf16x2(v[c + 4], v[c + 5]), pack_bf16x2(v[c + 6], v[c + 7]));
+          for (int k = 0; k < 8; ++k) v[k] = __uint_as_float(r[c + k]);
+          if (args.bias != nullptr) {
+            const float4 b0 = __ldg(reinterpret_cast<const float4*>(args.bias + col0 + c));
+            const float4 b1 = __ldg(reinterpret_cast<const float4*>(args.bias + col0 + c + 4));
+            v[0] += b0.x; v[1] += b0.y; v[2] += b0.z; v[3] += b0.w;
+            v[4] += b1.x; v[5] += b1.y; v[6] += b1.z; v[7] += b1.w;
+          }
+          if (kAct == ACT_SILU) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = __fdividef(v[k], 1.0f + __expf(-v[k]));
+          } else if (kAct == ACT_RELU) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] = fmaxf(v[k], 0.f);
+          }
+          if (args.y_is_f32) {
+            float* dst = static_cast<float*>(args.y) + row * args.N + col0 + c;
+            *reinterpret_cast<float4*>(dst) = make_float4(v[0], v[1], v[2], v[3]);
+            *reinterpret_cast<float4*>(dst + 4) = make_float4(v[4], v[5], v[6], v[7]);
+          } else {
+            __nv_bfloat16* dst = static_cast<__nv_bfloat16*>(args.y) + row * args.N + col0 + c;
+            *reinterpret_cast<uint4*>(dst) = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]),
+                                                        pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+          }
         }
+      };
+#pragma unroll 1
+      for (int c0 = 0; c0 < kBN; c0 += 32) {
+        if (args.act == ACT_SILU) chunk(cuda::std::integral_constant<int, ACT_SILU>{}, c0);
+        else if (args.act == ACT_RELU) chunk(cuda::std::integral_constant<int, ACT_RELU>{}, c0);
+        else chunk(cuda::std::integral_constant<int, ACT_NONE>{}, c0);
       }
     }
   }
