@@ -168,6 +168,11 @@ typedef struct upr_attn_params {
                                   refused with UPR_ERR_INVALID_ARG, and the bf16 K/V tensor maps are clipped
                                   to it, so no TMA read ever leaves the allocation (rows beyond it read 0). */
   int64_t kv_rows;             /* packed cache: layout.R of the cache (host copy), or 0 = unknown */
+  int32_t causal;              /* 1: candidate c of user b (local index cl in [0, C_b)) sees only the keys
+                                  j <= cl + (L_b - C_b) -- with C_b = L_b and q = the history tokens' queries this is the
+                                  causal O(n^2) self-attention of the history prefill over K/V that
+                                  already sit in the pool / cache layout.  CTA-pair kernel only (bf16, d = 128), no
+                                  split-K; a candidate that sees no key gets zeros (or its self term). */
   int32_t kernel;              /* UPR_KERNEL_AUTO (0): the library picks.  UPR_KERNEL_SINGLE (1) / UPR_KERNEL_PAIR
                                   (2) force the 1-CTA kernel / the CTA-pair kernel (bf16 q and K/V, d = 128,
                                   H / H_kv in {1,2,4,8}); a forced kernel that cannot run the arguments

@@ -57,7 +57,7 @@ class _AttnParams(ctypes.Structure):
         ("max_seq_len", ctypes.c_int32), ("workspace", ctypes.c_void_p), ("workspace_bytes", ctypes.c_size_t),
         ("kv_source", ctypes.c_int32), ("pool_slots", ctypes.c_int32), ("pool_n_max", ctypes.c_int32),
         ("H_kv", ctypes.c_int32), ("slot_ids", ctypes.c_void_p), ("kv_bytes", ctypes.c_int64),
-        ("kv_rows", ctypes.c_int64), ("kernel", ctypes.c_int32),
+        ("kv_rows", ctypes.c_int64), ("causal", ctypes.c_int32), ("kernel", ctypes.c_int32),
     ]
 
 
@@ -176,7 +176,7 @@ def upr_cross_attn_fwd(q, k_cache, v_cache, seq_lens, cand_offsets, out, B: int,
 def _params(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers, kv_dtype, q_dtype, total_q,
             k_self=None, v_self=None, k_scale=None, v_scale=None, sm_scale=0.0, num_splits=0, max_seq_len=0,
             workspace=None, kv_source=UPR_KV_PACKED, pool_slots=0, pool_n_max=0, H_kv=0, slot_ids=None,
-            kv_bytes=0, kv_rows=0, kernel=UPR_KERNEL_AUTO) -> _AttnParams:
+            kv_bytes=0, kv_rows=0, kernel=UPR_KERNEL_AUTO, causal=0) -> _AttnParams:
     p = _AttnParams()
     p.q, p.k_cache, p.v_cache = _ptr(q), _ptr(k_cache), _ptr(v_cache)
     p.seq_lens, p.cand_offsets, p.out = _ptr(seq_lens), _ptr(cand_offsets), _ptr(out)
@@ -186,21 +186,21 @@ def _params(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers,
     p.workspace = _ptr(workspace)
     p.workspace_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     p.kv_source, p.pool_slots, p.pool_n_max, p.H_kv = kv_source, pool_slots, pool_n_max, H_kv
-    p.slot_ids, p.kv_bytes, p.kv_rows, p.kernel = _ptr(slot_ids), kv_bytes, kv_rows, kernel
+    p.slot_ids, p.kv_bytes, p.kv_rows, p.kernel, p.causal = _ptr(slot_ids), kv_bytes, kv_rows, kernel, int(causal)
     return p
 
 
 def upr_cross_attn_workspace_bytes(B, H, d, n_layers, total_q, num_splits=0, max_seq_len=0, H_kv=0,
-                                   kv_dtype=UPR_BF16, q_dtype=UPR_BF16, kernel=UPR_KERNEL_AUTO) -> int:
+                                   kv_dtype=UPR_BF16, q_dtype=UPR_BF16, kernel=UPR_KERNEL_AUTO, causal=0) -> int:
     p = _params(None, None, None, None, None, None, B, H, d, n_layers, kv_dtype, q_dtype, total_q,
-                num_splits=num_splits, max_seq_len=max_seq_len, H_kv=H_kv, kernel=kernel)
+                num_splits=num_splits, max_seq_len=max_seq_len, H_kv=H_kv, kernel=kernel, causal=causal)
     return int(_load().upr_cross_attn_workspace_bytes(ctypes.byref(p)))
 
 
 def upr_cross_attn_num_splits(B, H, d, n_layers, total_q, num_splits=0, max_seq_len=0, H_kv=0,
-                              kv_dtype=UPR_BF16, q_dtype=UPR_BF16, kernel=UPR_KERNEL_AUTO) -> int:
+                              kv_dtype=UPR_BF16, q_dtype=UPR_BF16, kernel=UPR_KERNEL_AUTO, causal=0) -> int:
     p = _params(None, None, None, None, None, None, B, H, d, n_layers, kv_dtype, q_dtype, total_q,
-                num_splits=num_splits, max_seq_len=max_seq_len, H_kv=H_kv, kernel=kernel)
+                num_splits=num_splits, max_seq_len=max_seq_len, H_kv=H_kv, kernel=kernel, causal=causal)
     return int(_load().upr_cross_attn_num_splits(ctypes.byref(p)))
 
 
@@ -208,12 +208,12 @@ def upr_cross_attn_fwd_ex(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H
                           total_q, workspace, k_self=None, v_self=None, k_scale=None, v_scale=None, sm_scale=0.0,
                           num_splits=0, max_seq_len=0, stream=None, kv_source=UPR_KV_PACKED, pool_slots=0,
                           pool_n_max=0, H_kv=0, slot_ids=None, kv_bytes=0, kv_rows=0,
-                          kernel=UPR_KERNEL_AUTO) -> None:
+                          kernel=UPR_KERNEL_AUTO, causal=0) -> None:
     """k_cache / v_cache are packed decode caches, or (kv_source=UPR_KV_POOL) the bf16 pools
     [n_layers, pool_slots, H_kv, pool_n_max, d] read in place through slot_ids."""
     p = _params(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers, kv_dtype, q_dtype, total_q,
                 k_self, v_self, k_scale, v_scale, sm_scale, num_splits, max_seq_len, workspace, kv_source,
-                pool_slots, pool_n_max, H_kv, slot_ids, kv_bytes, kv_rows, kernel)
+                pool_slots, pool_n_max, H_kv, slot_ids, kv_bytes, kv_rows, kernel, causal)
     _check(_load().upr_cross_attn_fwd_ex(ctypes.byref(p), _stream(stream)))
 
 

@@ -83,6 +83,7 @@ struct Args {
   int pool_S, pool_n;
   int total_q;
   int out_tma;
+  int causal;             // candidate c of user b (local index cl) sees keys j <= cl + (L_b - C_b): history prefill
   float scale_log2;
 };
 
@@ -93,6 +94,8 @@ struct Item {
   int cands;     // candidates in the block, 1 .. 2 * cpt
   int kv_row0;   // row of the split's first key in the [rows, d] view of K / V
   int n_keys;    // keys of the split's range (>= 0)
+  int lim0;      // causal mode: keys visible to the block's first candidate (row r of the block sees lim0 + r);
+                 // otherwise 1 << 30
 };
 
 struct __align__(16) Ctrl {
@@ -293,7 +296,11 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       const int t0 = static_cast<int>((static_cast<long long>(split) * nt_user) / args.num_splits);
       const int t1 = static_cast<int>((static_cast<long long>(split + 1) * nt_user) / args.num_splits);
       const int key0 = t0 * kKeys;
-      const int n_keys = (t1 > t0) ? (min(Lb, t1 * kKeys) - key0) : 0;
+      // causal (prefill, one split): row r of the block sees keys [0, lim0 + r); the block needs the keys its
+      // last row sees
+      const int lim0 = args.causal ? (Lb - Cb) + qblk * cpb + 1 : (1 << 30);
+      const int n_keys = args.causal ? max(0, min(Lb, lim0 + min(cpb, Cb - qblk * cpb) - 1))
+                                     : ((t1 > t0) ? (min(Lb, t1 * kKeys) - key0) : 0);
       const int kv_row0 =
           (args.slot_ids != nullptr)
               ? ((layer * args.pool_S + __ldg(args.slot_ids + b)) * args.H_kv + hkv) * args.pool_n + key0
@@ -308,6 +315,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
         it.cands = min(cpb, Cb - qblk * cpb);
         it.kv_row0 = kv_row0;
         it.n_keys = n_keys;
+        it.lim0 = lim0;
         mbar_arrive(smem_u32(&ctrl->item_full[islot]));
         const int nt = (n_keys + kKeys - 1) / kKeys;
         if (nt > 0) {
@@ -561,8 +569,12 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       float m_used = self_here ? s_self : -INFINITY;
       float l = (self_here && wg == 0) ? 1.f : 0.f;
       if (nh > 0) {
-        // One 128-key tile.  The last tile of an item (tail masking) is a separate instantiation so
-        // that the steady-state loop body stays small.
+        // keys this thread's row may see (causal mode; otherwise all of the item's)
+        const int lim_row = min(it.n_keys, it.lim0 + static_cast<int>(rank) * cpt + cl);
+        const int lim_cta = it.lim0 + static_cast<int>(rank) * cpt;      // ... and the CTA tile's first row
+        // One 128-key tile.  Tiles that need masking (the item's last tile: history tail; causal mode: the
+        // tiles that reach past the diagonal) are a separate instantiation so that the steady-state loop
+        // body stays small.
         auto step = [&](const int j, auto last_tag) {
           constexpr bool kLast = decltype(last_tag)::value;
           const uint32_t gidx = g0 + j;
@@ -575,7 +587,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
           tmem_ld32(tm_s + 32, &sr[32]);
           tmem_wait_ld_regs(sr);
           if (kLast) {
-            const int keys_mine = it.n_keys - j * kKeys - wg * 64;   // valid keys among this thread's columns
+            const int keys_mine = lim_row - j * kKeys - wg * 64;   // valid keys among this thread's columns
 #pragma unroll
             for (int c = 0; c < 64; ++c)
               if (c >= keys_mine) sr[c] = 0xff800000u;  // -inf
@@ -625,7 +637,10 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             if (need) m_used = m_new;
           }
           float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
-          const float2 c2 = make_float2(args.scale_log2, args.scale_log2), nm2 = make_float2(-m_used, -m_used);
+          // (a row that has seen no key yet -- causal mode with more candidates than keys -- keeps m = -inf:
+          // subtract 0 instead, its logits are all -inf and its weights 0)
+          const float m_sub = (kLast && m_used == -INFINITY) ? 0.f : m_used;
+          const float2 c2 = make_float2(args.scale_log2, args.scale_log2), nm2 = make_float2(-m_sub, -m_sub);
 #pragma unroll
           for (int c0 = 0; c0 < 64; c0 += 32) {
             uint32_t pr[16];
@@ -653,8 +668,10 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(p_full_addr + sb * 16);
         };
-        for (int j = 0; j + 1 < nt; ++j) step(j, cuda::std::false_type{});
-        if (nt > 0) step(nt - 1, cuda::std::true_type{});
+        for (int j = 0; j < nt; ++j) {
+          if (j == nt - 1 || (j + 1) * kKeys > lim_cta) step(j, cuda::std::true_type{});
+          else step(j, cuda::std::false_type{});
+        }
         // hand the row's final state to the epilogue: the two partial sums (added there), and from
         // group 0 the weight of the candidate's own value row; split-K partial state by group 0
         // once both sums are in shared memory

@@ -119,7 +119,7 @@ constexpr bool kPairInAuto = true;
 
 bool use_pair(const upr_attn_params* p, bool have_workspace) {
   if (!have_workspace || p->kernel == UPR_KERNEL_SINGLE || !pair_capable(p)) return false;
-  if (p->kernel == UPR_KERNEL_PAIR) return true;
+  if (p->kernel == UPR_KERNEL_PAIR || p->causal) return true;
   if (!kPairInAuto) return false;
   const int G = p->H / kv_heads(p);
   if (G > 1) return true;   // grouped queries exist only in the pair kernel
@@ -127,6 +127,7 @@ bool use_pair(const upr_attn_params* p, bool have_workspace) {
 }
 
 int pick_splits(const upr_attn_params* p, bool pair) {
+  if (p->causal) return 1;
   if (p->num_splits >= 1) return p->num_splits;
   // heuristic: split the history when the (user, head, q-block) items cannot fill the SMs
   if (p->max_seq_len <= 0 || p->total_q <= 0 || p->B <= 0) return 1;
@@ -303,6 +304,7 @@ upr_status run_attn_pair(const upr_attn_params* p, int ns, cudaStream_t st) {
   a.pool_S = p->pool_slots;
   a.pool_n = p->pool_n_max;
   a.total_q = static_cast<int>(p->total_q);
+  a.causal = p->causal ? 1 : 0;
   const float sm = p->sm_scale > 0.f ? p->sm_scale : 1.0f / sqrtf(static_cast<float>(p->d));
   a.scale_log2 = sm * 1.4426950408889634f;
   if (ns > 1) {
@@ -355,6 +357,8 @@ upr_status run_attn(const upr_attn_params* p, bool have_workspace, cudaStream_t 
   if (s != UPR_OK) return s;
 
   const bool pair = use_pair(p, have_workspace);
+  if (p->causal && (!pair || p->num_splits > 1))
+    return fail(UPR_ERR_UNSUPPORTED, "causal attention needs the CTA-pair kernel (bf16 q and K/V, d = 128, a workspace) and no split-K");
   if (p->kernel == UPR_KERNEL_PAIR && !pair)
     return fail(UPR_ERR_UNSUPPORTED, "the CTA-pair kernel needs bf16 q and K/V, d = 128, H/H_kv in {1,2,4,8}");
   const int hkv = kv_heads(p);

@@ -72,7 +72,7 @@ class CrossAttention:
     """a2-a8 for a fixed problem shape: owns the output and workspace buffers."""
 
     def __init__(self, cache, cand_offsets_host, q_dtype: int = B_.UPR_BF16, num_splits: int = 0,
-                 device=None, H_q: Optional[int] = None, kernel: int = B_.UPR_KERNEL_AUTO):
+                 device=None, H_q: Optional[int] = None, kernel: int = B_.UPR_KERNEL_AUTO, causal: bool = False):
         """cache: a DecodeCache (packed) or a PoolView (zero copy).  H_q: query heads when they are a
         multiple of the KV heads (grouped queries); default = the KV head count."""
         self.cache = cache
@@ -92,6 +92,7 @@ class CrossAttention:
         self.H = H_q or self.H_kv
         self.kv_kwargs["H_kv"] = self.H_kv
         self.kv_kwargs["kernel"] = kernel
+        self.kv_kwargs["causal"] = int(causal)
         self.q_dtype = q_dtype
         co = np.asarray(cand_offsets_host, dtype=np.int32)
         self.total_q = int(co[-1])
@@ -99,9 +100,9 @@ class CrossAttention:
         self.cand_offsets = torch.as_tensor(co, device=device)
         self.num_splits = num_splits
         self.splits = B_.upr_cross_attn_num_splits(self.B, self.H, self.d, self.n_layers, self.total_q, num_splits,
-                                                   cache.max_seq_len, self.H_kv, self.kv_dtype, q_dtype, kernel)
+                                                   cache.max_seq_len, self.H_kv, self.kv_dtype, q_dtype, kernel, int(causal))
         nbytes = B_.upr_cross_attn_workspace_bytes(self.B, self.H, self.d, self.n_layers, self.total_q, num_splits,
-                                                   cache.max_seq_len, self.H_kv, self.kv_dtype, q_dtype, kernel)
+                                                   cache.max_seq_len, self.H_kv, self.kv_dtype, q_dtype, kernel, int(causal))
         self.workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
         self.out = torch.empty((self.n_layers, self.total_q, self.H, self.d), dtype=torch.float32, device=device)
 

@@ -261,6 +261,69 @@ def test_many_users(P, B):
     check(got, want)
 
 
+def _causal_oracle(inp):
+    """Row cl of user b sees keys j <= cl + (L_b - C_b): the plain definition, row by row (oracle.attn_block on the
+    visible prefix); for C_b == L_b also the dense masked full-sequence attention of PAPER.md:138 (history rows)."""
+    w = inp.w
+    out = np.zeros((w.n_layers, w.total_q, w.H, w.d))
+    co = w.cand_offsets
+    for l in range(w.n_layers):
+        for b in range(w.B):
+            Lb, Cb = int(w.seq_lens[b]), int(co[b + 1] - co[b])
+            for h in range(w.H):
+                K, V = inp.block_kv_f64(l, b, h)
+                q, _, _ = inp.block_q_f64(l, b, h)
+                if Cb == Lb and Lb > 0:
+                    out[l, co[b]:co[b + 1], h] = oracle.full_sequence_attention(q, K, V, Lb, 0, False)
+                    continue
+                for cl in range(Cb):
+                    lim = max(0, min(Lb, cl + (Lb - Cb) + 1))
+                    out[l, co[b] + cl, h] = oracle.attn_block(q[cl:cl + 1], K[:lim], V[:lim])[0]
+    return out
+
+
+CAUSAL_CASES = [
+    # name, seq_lens, cand_counts, H_q, H_kv, layers
+    ("prefill", [300, 129, 1, 640, 0], [300, 129, 1, 640, 0], 2, 2, 2),
+    ("prefill_gqa", [513, 77], [513, 77], 4, 2, 1),
+    ("suffix_queries", [500, 128], [200, 1], 2, 2, 1),          # the last C_b positions of a longer history
+    ("more_queries_than_keys", [5, 300], [20, 300], 1, 1, 1),   # rows that see no key at all -> zeros
+]
+
+
+@pytest.mark.parametrize("case", CAUSAL_CASES, ids=[c[0] for c in CAUSAL_CASES])
+@pytest.mark.parametrize("source", ["packed", "pool"])
+def test_causal_prefill_attention_matches_oracle(P, case, source):
+    """SURVEY 8(f)2, second half: the causal O(n^2) self-attention of the history prefill over
+    K/V that already sit in the pool layout: the same CTA-pair kernel with `causal = 1`, queries = the history
+    tokens' own queries."""
+    from paper_2606_00422_b200 import pipeline as pl
+    name, L, C, Hq, Hkv, layers = case
+    w = S.custom_workload(name, 888, L, C, Hq, 128, layers, n_max=max(L) + 9)
+    inp = Inputs(w, "cuda", H_kv=Hkv)
+    if source == "pool":
+        src = pl.PoolView.of(inp.k_pool, inp.v_pool, inp.slot_ids, w.seq_lens)
+    else:
+        src = pl.alloc_cache(w.seq_lens, Hkv, w.d, w.n_layers, P.UPR_BF16, "cuda")
+        pl.pack_cache(src, inp.k_pool, inp.v_pool, inp.slot_ids)
+    attn = pl.CrossAttention(src, w.cand_offsets, P.UPR_BF16, H_q=Hq, causal=True)
+    got = attn(inp.q).cpu().numpy()
+    torch.cuda.synchronize()
+    assert P.upr_last_attn_kernel() == "upr_attn_pair_kernel" and attn.splits == 1
+    check(got, _causal_oracle(inp))
+
+
+def test_causal_needs_the_pair_kernel(P):
+    from paper_2606_00422_b200 import pipeline as pl
+    w = S.custom_workload("causal_err", 1, [64], [64], 2, 64, 1)
+    inp = Inputs(w, "cuda")
+    view = pl.PoolView.of(inp.k_pool, inp.v_pool, inp.slot_ids, w.seq_lens)
+    attn = pl.CrossAttention(view, w.cand_offsets, P.UPR_BF16, causal=True)     # d = 64
+    with pytest.raises(P.UprError) as e:
+        attn(inp.q)
+    assert e.value.status == 2
+
+
 def test_zero_copy_rejects_bad_arguments(P):
     from paper_2606_00422_b200 import pipeline as pl
     w = S.custom_workload("poolerr", 1, [64, 10], [4, 4], 2, 64, 1, n_max=64)
