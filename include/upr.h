@@ -221,6 +221,19 @@ upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const
                           upr_dtype y_dtype, int64_t M, int N, int K, upr_activation act, void* stream);
 
 /*
+ * Prefill into the layout: the K (or V) projection of M history tokens written straight into
+ * the pool [n_layers, S, H, n, d] -- no intermediate [M, H*d] tensor and no scatter pass:
+ *     pool[layer, tok_slot[m], h, tok_pos[m], :] = (x[m] W^T + bias)[h*d : (h+1)*d]        (bf16)
+ * Same GEMM kernel as upr_linear_fwd (N = H * d), the epilogue addresses the pool.
+ *   x device [M, K] bf16 or fp32; w device bf16 [H*d, K]; bias device fp32 [H*d] or NULL
+ *   pool device bf16; tok_slot, tok_pos device int32 [M] (slot in [0, S), position in [0, n))
+ * The attention can then read the slot in place (kv_source = UPR_KV_POOL; causal = 1 for the prefill itself).
+ */
+upr_status upr_kv_project_into_pool(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* pool,
+                                    const int32_t* tok_slot, const int32_t* tok_pos, int64_t M, int K, int layer,
+                                    int n_layers, int S, int H, int n, int d, void* stream);
+
+/*
  * Per-action heads, second half: hid = act(W1_c z + b1_c) for the C heads side by
  * side comes from upr_linear_fwd (N = C * Dh); this call finishes them:
  *     logit_c = <w2_c, hid_c> + b2_c,  p_c = sigmoid(logit_c),  util = sum_c wc_c * p_c

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
     "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
     "upr_last_error", "upr_version", "upr_last_attn_kernel",
-    "upr_linear_fwd", "upr_action_utility", "upr_topk_per_user",
+    "upr_linear_fwd", "upr_kv_project_into_pool", "upr_action_utility", "upr_topk_per_user",
     "upr_pool_export", "upr_pool_open", "upr_pool_close", "upr_slot_ring_init", "upr_slot_ring_acquire",
 ]
 UPR_ACT_NONE, UPR_ACT_SILU, UPR_ACT_RELU = 0, 1, 2
@@ -96,6 +96,10 @@ def _load() -> ctypes.CDLL:
         lib.upr_linear_fwd.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                        ctypes.c_int, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                        ctypes.c_void_p]
+        lib.upr_kv_project_into_pool.restype = ctypes.c_int
+        lib.upr_kv_project_into_pool.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+                                                 ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64] + \
+                                                [ctypes.c_int] * 7 + [ctypes.c_void_p]
         lib.upr_action_utility.restype = ctypes.c_int
         lib.upr_action_utility.argtypes = [ctypes.c_void_p] * 4 + [ctypes.c_int64, ctypes.c_int, ctypes.c_int,
                                                                    ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
@@ -227,6 +231,15 @@ def upr_linear_fwd(x, w, bias, y, act: int = UPR_ACT_NONE, stream=None) -> None:
     N = int(w.shape[0])
     _check(_load().upr_linear_fwd(_ptr(x), _DT[x.dtype], _ptr(w), _ptr(bias), _ptr(y), _DT[y.dtype], M, N, K, act,
                                   _stream(stream)))
+
+
+def upr_kv_project_into_pool(x, w, bias, pool, tok_slot, tok_pos, layer: int, stream=None) -> None:
+    """pool[layer, tok_slot[m], h, tok_pos[m], :] = (x[m] W^T + bias)[h*d:(h+1)*d]; pool bf16 [layers,S,H,n,d]."""
+    n_layers, S, H, n, d = (int(v) for v in pool.shape)
+    M, K = int(x.shape[0]), int(x.shape[1])
+    assert int(w.shape[0]) == H * d and int(w.shape[1]) == K and pool.dtype == torch.bfloat16
+    _check(_load().upr_kv_project_into_pool(_ptr(x), _DT[x.dtype], _ptr(w), _ptr(bias), _ptr(pool), _ptr(tok_slot),
+                                            _ptr(tok_pos), M, K, layer, n_layers, S, H, n, d, _stream(stream)))
 
 
 def upr_action_utility(hid, w2, b2, wc, probs, util, stream=None) -> None:

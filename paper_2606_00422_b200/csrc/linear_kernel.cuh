@@ -46,6 +46,11 @@ struct Args {
   int N, K;
   int act;
   int y_is_f32;
+  // K/V projection written straight into the pool layout [layers, S, H, n, d]: row m of y is token
+  // m's [H, d] vector and goes to pool[layer, tok_slot[m], h, tok_pos[m], :]; y = the pool (bf16), N = H * d
+  const int32_t* tok_slot;
+  const int32_t* tok_pos;
+  int kv_layer, kv_S, kv_H, kv_n, kv_d;
 };
 
 struct __align__(16) Ctrl {
@@ -206,6 +211,11 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
       tc_fence_after();
       const long long row = static_cast<long long>(mb) * kBM + ew * 32 + lane;
       const bool row_ok = row < args.M;
+      // pool mode: first pool row of this token's slot (head 0), or -1
+      long long kv_row0 = -1;
+      if (args.tok_slot != nullptr && row_ok)
+        kv_row0 = ((static_cast<long long>(args.kv_layer) * args.kv_S + __ldg(args.tok_slot + row)) * args.kv_H) * args.kv_n +
+                  __ldg(args.tok_pos + row);
       // one 32-column chunk: + bias, activation, store.  The activation is a compile-time branch (the
       // per-element form with run-time tests made the epilogue, not the MMAs, the bound of the kernel)
       auto chunk = [&](auto act_tag, const int c0) {
@@ -240,7 +250,13 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
 #pragma unroll
             for (int k = 0; k < 8; ++k) v[k] = fmaxf(v[k], 0.f);
           }
-          if (args.y_is_f32) {
+          if (args.tok_slot != nullptr) {
+            const int col = col0 + c, h = col / args.kv_d, t = col - h * args.kv_d;   // 8 columns stay inside one head
+            __nv_bfloat16* dst = static_cast<__nv_bfloat16*>(args.y) +
+                                 (kv_row0 + static_cast<long long>(h) * args.kv_n) * args.kv_d + t;
+            *reinterpret_cast<uint4*>(dst) = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]),
+                                                        pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+          } else if (args.y_is_f32) {
             float* dst = static_cast<float*>(args.y) + row * args.N + col0 + c;
             *reinterpret_cast<float4*>(dst) = make_float4(v[0], v[1], v[2], v[3]);
             *reinterpret_cast<float4*>(dst + 4) = make_float4(v[4], v[5], v[6], v[7]);

@@ -624,8 +624,13 @@ upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream) {
 }
 
 // ------------------------------------------------------------------ decode-layer tail, consumer, pool
-upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
-                          upr_dtype y_dtype, int64_t M, int N, int K, upr_activation act, void* stream) {
+namespace {
+struct KvScatter { const int32_t* tok_slot; const int32_t* tok_pos; int layer, S, H, n, d; };
+}  // namespace
+
+static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
+                              upr_dtype y_dtype, int64_t M, int N, int K, upr_activation act, const KvScatter* kv,
+                              void* stream) {
   g_launches = 0;
   if (M < 0 || N <= 0 || K <= 0) return fail(UPR_ERR_INVALID_ARG, "bad sizes M=%lld N=%d K=%d", (long long)M, N, K);
   if (x_dtype != UPR_BF16 && x_dtype != UPR_F32) return fail(UPR_ERR_UNSUPPORTED, "x_dtype %d (bf16 or f32)", (int)x_dtype);
@@ -663,6 +668,16 @@ upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const
       return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for w");
   }
   upr::lin::Args a;
+  memset(&a, 0, sizeof(a));
+  if (kv != nullptr) {
+    a.tok_slot = kv->tok_slot;
+    a.tok_pos = kv->tok_pos;
+    a.kv_layer = kv->layer;
+    a.kv_S = kv->S;
+    a.kv_H = kv->H;
+    a.kv_n = kv->n;
+    a.kv_d = kv->d;
+  }
   a.bias = bias;
   a.y = y;
   a.M = M;
@@ -687,6 +702,22 @@ upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const
   UPR_CUDA_CHECK(cudaGetLastError());
   g_launches = 1;
   return UPR_OK;
+}
+
+upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
+                          upr_dtype y_dtype, int64_t M, int N, int K, upr_activation act, void* stream) {
+  return linear_impl(x, x_dtype, w, bias, y, y_dtype, M, N, K, act, nullptr, stream);
+}
+
+upr_status upr_kv_project_into_pool(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* pool,
+                                    const int32_t* tok_slot, const int32_t* tok_pos, int64_t M, int K, int layer,
+                                    int n_layers, int S, int H, int n, int d, void* stream) {
+  if (S <= 0 || H <= 0 || n <= 0 || n_layers <= 0 || layer < 0 || layer >= n_layers)
+    return fail(UPR_ERR_INVALID_ARG, "bad pool shape / layer (layers=%d S=%d H=%d n=%d layer=%d)", n_layers, S, H, n, layer);
+  if (d != 64 && d != 128) return fail(UPR_ERR_UNSUPPORTED, "head dim d=%d unsupported (64 or 128)", d);
+  if (M > 0 && (!tok_slot || !tok_pos)) return fail(UPR_ERR_INVALID_ARG, "tok_slot / tok_pos is NULL");
+  KvScatter kv{tok_slot, tok_pos, layer, S, H, n, d};
+  return linear_impl(x, x_dtype, w, bias, pool, UPR_BF16, M, H * d, K, UPR_ACT_NONE, &kv, stream);
 }
 
 upr_status upr_action_utility(const void* hid, const float* w2, const float* b2, const float* wc, int64_t M,

@@ -85,6 +85,69 @@ def test_linear_rejects_unsupported(P):
     assert e.value.status == 2
 
 
+def test_prefill_writes_kv_into_the_pool_layout_and_attends_in_place(P):
+    """history tokens -> K / V projections written STRAIGHT into the pool [L,S,H,n,D] by the GEMM's
+    epilogue (no [M, H d] intermediate, no scatter pass) -> causal attention reads the slots in place.
+    Checked: (i) the written rows against the oracle's linear layer (one bf16 rounding), every other pool
+    element untouched bit for bit; (ii) the causal attention over the pool the GPU wrote against the oracle on
+    the oracle's own projections (K / V rounded to bf16 as the pool stores them)."""
+    from paper_2606_00422_b200 import pipeline as pl
+    dev = "cuda"
+    H, d, D, S_slots, n_max, layers = 2, 128, 256, 5, 200, 2
+    L = np.array([150, 0, 37, 200], dtype=np.int32)
+    slots_h = np.array([3, 0, 4, 1], dtype=np.int32)
+    M = int(L.sum())
+    x = S.normal_bf16(31, "x_hist", (M, D), dev)
+    wk, wv, wq = weights(32, "wk", H * d, D, dev), weights(33, "wv", H * d, D, dev), weights(34, "wq", H * d, D, dev)
+    tok_slot = torch.from_numpy(np.repeat(slots_h, L).astype(np.int32)).to(dev)
+    tok_pos = torch.from_numpy(np.concatenate([np.arange(n) for n in L]).astype(np.int32)).to(dev)
+    sentinel = S.normal_bf16(35, "stale", (layers, S_slots, H, n_max, d), dev)      # stale K/V of earlier requests
+    k_pool, v_pool = sentinel.clone(), sentinel.clone()
+    layer = 1
+    P.upr_kv_project_into_pool(x, wk, None, k_pool, tok_slot, tok_pos, layer)
+    P.upr_kv_project_into_pool(x, wv, None, v_pool, tok_slot, tok_pos, layer)
+    q = torch.empty((M, H * d), dtype=torch.bfloat16, device=dev)
+    P.upr_linear_fwd(x, wq, None, q, P.UPR_ACT_NONE)
+    torch.cuda.synchronize()
+    k_want, v_want = oracle.linear(f64(x), f64(wk)), oracle.linear(f64(x), f64(wv))
+    written = torch.zeros((layers, S_slots, H, n_max), dtype=torch.bool)
+    off = np.concatenate([[0], np.cumsum(L)])
+    for b in range(len(L)):
+        for h in range(H):
+            got_k = f64(k_pool[layer, slots_h[b], h, : L[b]])
+            got_v = f64(v_pool[layer, slots_h[b], h, : L[b]])
+            wk_ = k_want[off[b]:off[b + 1], h * d:(h + 1) * d]
+            wv_ = v_want[off[b]:off[b + 1], h * d:(h + 1) * d]
+            if L[b]:
+                assert np.abs(got_k - wk_).max() <= 2.0 ** -8 * max(1.0, np.abs(wk_).max())
+                assert np.abs(got_v - wv_).max() <= 2.0 ** -8 * max(1.0, np.abs(wv_).max())
+            written[layer, slots_h[b], h, : L[b]] = True
+    untouched = ~written.to(dev)
+    assert torch.equal(k_pool[untouched], sentinel[untouched]) and torch.equal(v_pool[untouched], sentinel[untouched])
+    # causal attention over the slots the GPU just wrote, in place
+    co = np.concatenate([[0], np.cumsum(L)]).astype(np.int32)
+    view = pl.PoolView.of(k_pool[layer:layer + 1], v_pool[layer:layer + 1], torch.from_numpy(slots_h).to(dev), L)
+    attn = pl.CrossAttention(view, co, P.UPR_BF16, causal=True)
+    out = attn(q.view(1, M, H, d)).cpu().numpy()[0]
+    torch.cuda.synchronize()
+    q_want = oracle.linear(f64(x), f64(wq))
+    def r16(a):   # what a bf16 store keeps of an fp64 value (torch's RNE cast: a library routine)
+        return torch.from_numpy(a).to(torch.bfloat16).to(torch.float64).numpy()
+    worst = 0.0
+    for b in range(len(L)):
+        if L[b] == 0:
+            continue
+        for h in range(H):
+            sl = slice(off[b], off[b + 1])
+            want = oracle.full_sequence_attention(r16(q_want[sl, h * d:(h + 1) * d]), r16(k_want[sl, h * d:(h + 1) * d]),
+                                                  r16(v_want[sl, h * d:(h + 1) * d]), int(L[b]), 0, False)
+            worst = max(worst, float(np.abs(out[sl, h] - want).max()))
+    print(f"prefill chain max-abs {worst:.2e}")
+    # q, K, V each carry one bf16 rounding whose tie-breaks may differ from the oracle's by one ulp (2^-8 relative):
+    # logits move by ~2^-8 |q||k| / sqrt(d) ~ 4e-3, outputs by a few 1e-3
+    assert worst <= 1e-2
+
+
 def test_action_heads_and_utility_match_oracle(P):
     """z -> [stacked first layers of the C heads, SiLU] (tcgen05 GEMM) -> logits -> sigmoid -> utility."""
     dev = "cuda"
