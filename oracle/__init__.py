@@ -278,3 +278,12 @@ def topk_per_user(util, cand_offsets, K: int):
     cnt = np.zeros(B, dtype=np.int32)
     lib().upro_topk_per_user(_p(util), _p(cand_offsets), B, K, _p(idx), _p(cnt))
     return idx, cnt
+
+
+def layernorm(x, gamma, beta, eps: float = 1e-5):
+    """y = (x - mean) / sqrt(var + eps) * gamma + beta over the last axis, fp64; x [M,D]."""
+    x, gamma, beta = _c64(x), _c64(gamma), _c64(beta)
+    M, D = x.shape
+    y = np.zeros((M, D), dtype=np.float64)
+    lib().upro_layernorm(_p(x), _p(gamma), _p(beta), ctypes.c_int64(M), D, ctypes.c_double(eps), _p(y))
+    return y

@@ -660,3 +660,26 @@ void upro_topk_per_user(const float* util, const int32_t* cand_offsets, int B, i
     free(used);
   }
 }
+
+/* ------------------------------------------------------------------------------------
+ * upro_layernorm -- layer normalisation of one token's hidden vector (PAPER.md:206 names
+ * "fused modules that combine layer normalization, linear projection, and activation"):
+ *     y = (x - mean(x)) / sqrt(var(x) + eps) * gamma + beta,   var = mean((x - mean)^2)
+ * the textbook definition, fp64, two passes.  x, y [M, D]; gamma, beta [D].
+ * ---------------------------------------------------------------------------------- */
+void upro_layernorm(const double* x, const double* gamma, const double* beta, int64_t M, int D,
+                    double eps, double* y) {
+#pragma omp parallel for schedule(static)
+  for (int64_t m = 0; m < M; ++m) {
+    double mean = 0.0, var = 0.0;
+    for (int t = 0; t < D; ++t) mean += x[m * D + t];
+    mean /= D;
+    for (int t = 0; t < D; ++t) {
+      double c = x[m * D + t] - mean;
+      var += c * c;
+    }
+    var /= D;
+    double r = 1.0 / sqrt(var + eps);
+    for (int t = 0; t < D; ++t) y[m * D + t] = (x[m * D + t] - mean) * r * gamma[t] + beta[t];
+  }
+}

@@ -133,3 +133,19 @@ def test_topk_brute_force_against_stable_argsort(oracle):
             assert cnt[b] == min(K, len(seg))
             np.testing.assert_array_equal(idx[b, :cnt[b]], order)
             assert np.all(idx[b, cnt[b]:] == -1)
+
+
+# ----------------------------------------------------------------------------- layer norm
+def test_layernorm_against_torch_and_closed_forms(oracle):
+    r = rng(7)
+    x, g, b = r.standard_normal((6, 32)) * 3 + 1, r.standard_normal(32), r.standard_normal(32)
+    want = torch.nn.functional.layer_norm(torch.from_numpy(x), (32,), torch.from_numpy(g), torch.from_numpy(b), 1e-5)
+    np.testing.assert_allclose(oracle.layernorm(x, g, b), want.numpy(), rtol=0, atol=1e-12)
+    # gamma = 1, beta = 0: zero mean, unit variance (up to eps); a shift and a positive scale of x change nothing
+    y = oracle.layernorm(x, np.ones(32), np.zeros(32), eps=0.0)
+    np.testing.assert_allclose(y.mean(axis=1), 0.0, atol=1e-14)
+    np.testing.assert_allclose((y ** 2).mean(axis=1), 1.0, atol=1e-13)
+    np.testing.assert_allclose(oracle.layernorm(5.0 * x + 7.0, np.ones(32), np.zeros(32), eps=0.0), y, atol=1e-12)
+    # hand case: x = (1, 3): mean 2, var 1 -> (-1, 1) * gamma + beta
+    np.testing.assert_allclose(oracle.layernorm(np.array([[1.0, 3.0]]), np.array([2.0, 3.0]), np.array([0.5, -0.5]), eps=0.0),
+                               [[-1.5, 2.5]], atol=1e-15)
