@@ -219,6 +219,16 @@ typedef enum { UPR_ACT_NONE = 0, UPR_ACT_SILU = 1, UPR_ACT_RELU = 2 } upr_activa
  */
 upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
                           upr_dtype y_dtype, int64_t M, int N, int K, upr_activation act, void* stream);
+/* The same with the residual stream added after the activation: y = act(x W^T + bias) + residual, residual device
+ * bf16 [M, N] (may alias y).  The out-projection and the MLP's down-projection of a decode layer. */
+upr_status upr_linear_residual_fwd(const void* x, upr_dtype x_dtype, const void* w, const float* bias,
+                                   const void* residual, void* y, upr_dtype y_dtype, int64_t M, int N, int K,
+                                   upr_activation act, void* stream);
+
+/* Layer normalisation of candidate tokens: y = (x - mean) / sqrt(var + eps) * gamma + beta over the
+ * hidden dimension; x, y device bf16 [M, D]; gamma, beta device fp32 [D]; D % 8 == 0, D <= 4096. */
+upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,
+                             float eps, void* stream);
 
 /*
  * Prefill into the layout: the K (or V) projection of M history tokens written straight into

@@ -16,7 +16,7 @@ EXPORTED_SYMBOLS = [
     "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
     "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
     "upr_last_error", "upr_version", "upr_last_attn_kernel",
-    "upr_linear_fwd", "upr_kv_project_into_pool", "upr_action_utility", "upr_topk_per_user",
+    "upr_linear_fwd", "upr_linear_residual_fwd", "upr_layernorm_fwd", "upr_kv_project_into_pool", "upr_action_utility", "upr_topk_per_user",
     "upr_pool_export", "upr_pool_open", "upr_pool_close", "upr_slot_ring_init", "upr_slot_ring_acquire",
 ]
 UPR_ACT_NONE, UPR_ACT_SILU, UPR_ACT_RELU = 0, 1, 2
@@ -96,6 +96,13 @@ def _load() -> ctypes.CDLL:
         lib.upr_linear_fwd.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                        ctypes.c_int, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                        ctypes.c_void_p]
+        lib.upr_linear_residual_fwd.restype = ctypes.c_int
+        lib.upr_linear_residual_fwd.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
+                                                ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_int,
+                                                ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
+        lib.upr_layernorm_fwd.restype = ctypes.c_int
+        lib.upr_layernorm_fwd.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
+                                          ctypes.c_int, ctypes.c_float, ctypes.c_void_p]
         lib.upr_kv_project_into_pool.restype = ctypes.c_int
         lib.upr_kv_project_into_pool.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
                                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64] + \
@@ -231,6 +238,20 @@ def upr_linear_fwd(x, w, bias, y, act: int = UPR_ACT_NONE, stream=None) -> None:
     N = int(w.shape[0])
     _check(_load().upr_linear_fwd(_ptr(x), _DT[x.dtype], _ptr(w), _ptr(bias), _ptr(y), _DT[y.dtype], M, N, K, act,
                                   _stream(stream)))
+
+
+def upr_linear_residual_fwd(x, w, bias, residual, y, act: int = UPR_ACT_NONE, stream=None) -> None:
+    """y = act(x W^T + bias) + residual (bf16 [M,N], may alias y)."""
+    M, K = int(x.shape[0]), int(x.shape[1])
+    N = int(w.shape[0])
+    _check(_load().upr_linear_residual_fwd(_ptr(x), _DT[x.dtype], _ptr(w), _ptr(bias), _ptr(residual), _ptr(y),
+                                           _DT[y.dtype], M, N, K, act, _stream(stream)))
+
+
+def upr_layernorm_fwd(x, gamma, beta, y, eps: float = 1e-5, stream=None) -> None:
+    """x, y bf16 [M, D]; gamma, beta fp32 [D]."""
+    _check(_load().upr_layernorm_fwd(_ptr(x), _ptr(gamma), _ptr(beta), _ptr(y), int(x.shape[0]), int(x.shape[1]), eps,
+                                     _stream(stream)))
 
 
 def upr_kv_project_into_pool(x, w, bias, pool, tok_slot, tok_pos, layer: int, stream=None) -> None:

@@ -41,6 +41,7 @@ enum : int { ACT_NONE = 0, ACT_SILU = 1, ACT_RELU = 2 };
 
 struct Args {
   const float* bias;      // [N] fp32 or nullptr
+  const __nv_bfloat16* residual;   // [M, N] bf16 added after the activation (the residual stream), or nullptr
   void* y;                // [M, N] bf16 or fp32
   long long M;
   int N, K;
@@ -249,6 +250,15 @@ upr_linear_kernel(const __grid_constant__ CUtensorMap tmap_x,   // bf16: box 128
           } else if (kAct == ACT_RELU) {
 #pragma unroll
             for (int k = 0; k < 8; ++k) v[k] = fmaxf(v[k], 0.f);
+          }
+          if (args.residual != nullptr) {
+            const uint4 q = __ldg(reinterpret_cast<const uint4*>(args.residual + row * args.N + col0 + c));
+            const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              v[2 * k] += __uint_as_float(w[k] << 16);
+              v[2 * k + 1] += __uint_as_float(w[k] & 0xffff0000u);
+            }
           }
           if (args.tok_slot != nullptr) {
             const int col = col0 + c, h = col / args.kv_d, t = col - h * args.kv_d;   // 8 columns stay inside one head

@@ -8,6 +8,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "ptx.cuh"
+
 namespace upr {
 
 // hid [M, C*Dh] bf16 = act(W1_c z + b1_c) for the C heads side by side; w2 [C, Dh], b2 [C], wc [C] fp32.
@@ -93,6 +95,77 @@ __global__ void __launch_bounds__(kTopkThreads) upr_topk_kernel(const float* __r
   for (int r = threadIdx.x; r < K; r += kTopkThreads)
     out_idx[static_cast<long long>(b) * K + r] = r < kk ? c0 + static_cast<int>(keys[r] & 0xffffffffu) : -1;
   if (threadIdx.x == 0) out_cnt[b] = kk;
+}
+
+
+// Layer normalisation over the hidden dimension of candidate tokens, bf16 in / bf16 out, fp32
+// statistics, two passes over registers (D <= 4096, D % 8 == 0): one warp per row, 16-byte loads.  HBM-bound.
+constexpr int kLnMaxChunks = 16;   // 16-byte chunks per lane: D <= 32 * 8 * 16 = 4096
+
+__global__ void __launch_bounds__(256) upr_layernorm_kernel(const __nv_bfloat16* __restrict__ x,
+                                                            const float* __restrict__ gamma,
+                                                            const float* __restrict__ beta, long long M, int D,
+                                                            float eps, __nv_bfloat16* __restrict__ y) {
+  const int lane = threadIdx.x & 31;
+  const long long warp0 = (static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
+  const long long n_warps = (static_cast<long long>(gridDim.x) * blockDim.x) >> 5;
+  const int n_chunks = D / 8;   // 16-byte chunks per row
+  for (long long m = warp0; m < M; m += n_warps) {
+    const uint4* src = reinterpret_cast<const uint4*>(x + m * D);
+    float v[kLnMaxChunks][8];
+    float sum = 0.f;
+#pragma unroll
+    for (int i = 0; i < kLnMaxChunks; ++i) {
+      const int c = i * 32 + lane;
+      if (c < n_chunks) {
+        const uint4 q = __ldg(src + c);
+        const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          v[i][2 * k] = __uint_as_float(w[k] << 16);
+          v[i][2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+          sum += v[i][2 * k] + v[i][2 * k + 1];
+        }
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    const float mean = sum / static_cast<float>(D);
+    float sq = 0.f;
+#pragma unroll
+    for (int i = 0; i < kLnMaxChunks; ++i)
+      if (i * 32 + lane < n_chunks) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const float c = v[i][k] - mean;
+          sq = fmaf(c, c, sq);
+        }
+      }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+    const float rstd = rsqrtf(sq / static_cast<float>(D) + eps);
+    uint4* dst = reinterpret_cast<uint4*>(y + m * D);
+#pragma unroll
+    for (int i = 0; i < kLnMaxChunks; ++i) {
+      const int c = i * 32 + lane;
+      if (c < n_chunks) {
+        const float4 g0 = __ldg(reinterpret_cast<const float4*>(gamma + c * 8));
+        const float4 g1 = __ldg(reinterpret_cast<const float4*>(gamma + c * 8 + 4));
+        const float4 b0 = __ldg(reinterpret_cast<const float4*>(beta + c * 8));
+        const float4 b1 = __ldg(reinterpret_cast<const float4*>(beta + c * 8 + 4));
+        const float g[8] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w};
+        const float b[8] = {b0.x, b0.y, b0.z, b0.w, b1.x, b1.y, b1.z, b1.w};
+        uint32_t o[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          const float lo = fmaf((v[i][2 * k] - mean) * rstd, g[2 * k], b[2 * k]);
+          const float hi = fmaf((v[i][2 * k + 1] - mean) * rstd, g[2 * k + 1], b[2 * k + 1]);
+          o[k] = pack_bf16x2(lo, hi);
+        }
+        dst[c] = make_uint4(o[0], o[1], o[2], o[3]);
+      }
+    }
+  }
 }
 
 }  // namespace upr

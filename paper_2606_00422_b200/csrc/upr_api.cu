@@ -625,7 +625,7 @@ upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream) {
 
 // ------------------------------------------------------------------ decode-layer tail, consumer, pool
 namespace {
-struct KvScatter { const int32_t* tok_slot; const int32_t* tok_pos; int layer, S, H, n, d; };
+struct KvScatter { const int32_t* tok_slot; const int32_t* tok_pos; int layer, S, H, n, d; const void* residual; };
 }  // namespace
 
 static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
@@ -669,7 +669,8 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   }
   upr::lin::Args a;
   memset(&a, 0, sizeof(a));
-  if (kv != nullptr) {
+  if (kv != nullptr) a.residual = static_cast<const __nv_bfloat16*>(kv->residual);
+  if (kv != nullptr && kv->tok_slot != nullptr) {
     a.tok_slot = kv->tok_slot;
     a.tok_pos = kv->tok_pos;
     a.kv_layer = kv->layer;
@@ -709,6 +710,33 @@ upr_status upr_linear_fwd(const void* x, upr_dtype x_dtype, const void* w, const
   return linear_impl(x, x_dtype, w, bias, y, y_dtype, M, N, K, act, nullptr, stream);
 }
 
+upr_status upr_linear_residual_fwd(const void* x, upr_dtype x_dtype, const void* w, const float* bias,
+                                   const void* residual, void* y, upr_dtype y_dtype, int64_t M, int N, int K,
+                                   upr_activation act, void* stream) {
+  if (residual != nullptr && (reinterpret_cast<uintptr_t>(residual) & 15))
+    return fail(UPR_ERR_INVALID_ARG, "residual must be 16-byte aligned");
+  KvScatter kv{nullptr, nullptr, 0, 0, 0, 0, 0, residual};
+  return linear_impl(x, x_dtype, w, bias, y, y_dtype, M, N, K, act, &kv, stream);
+}
+
+upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,
+                             float eps, void* stream) {
+  g_launches = 0;
+  if (M < 0 || D <= 0) return fail(UPR_ERR_INVALID_ARG, "bad sizes M=%lld D=%d", (long long)M, D);
+  if (D % 8 != 0 || D > 4096) return fail(UPR_ERR_UNSUPPORTED, "D=%d must be a multiple of 8 and <= 4096", D);
+  if (M == 0) return UPR_OK;
+  if (!x || !gamma || !beta || !y) return fail(UPR_ERR_INVALID_ARG, "NULL tensor pointer");
+  upr_status s = check_device();
+  if (s != UPR_OK) return s;
+  const long long blocks = (M + 7) / 8;
+  const int grid = static_cast<int>(blocks < sm_count() * 8LL ? blocks : sm_count() * 8LL);
+  upr::upr_layernorm_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(
+      static_cast<const __nv_bfloat16*>(x), gamma, beta, M, D, eps, static_cast<__nv_bfloat16*>(y));
+  UPR_CUDA_CHECK(cudaGetLastError());
+  g_launches = 1;
+  return UPR_OK;
+}
+
 upr_status upr_kv_project_into_pool(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* pool,
                                     const int32_t* tok_slot, const int32_t* tok_pos, int64_t M, int K, int layer,
                                     int n_layers, int S, int H, int n, int d, void* stream) {
@@ -716,7 +744,7 @@ upr_status upr_kv_project_into_pool(const void* x, upr_dtype x_dtype, const void
     return fail(UPR_ERR_INVALID_ARG, "bad pool shape / layer (layers=%d S=%d H=%d n=%d layer=%d)", n_layers, S, H, n, layer);
   if (d != 64 && d != 128) return fail(UPR_ERR_UNSUPPORTED, "head dim d=%d unsupported (64 or 128)", d);
   if (M > 0 && (!tok_slot || !tok_pos)) return fail(UPR_ERR_INVALID_ARG, "tok_slot / tok_pos is NULL");
-  KvScatter kv{tok_slot, tok_pos, layer, S, H, n, d};
+  KvScatter kv{tok_slot, tok_pos, layer, S, H, n, d, nullptr};
   return linear_impl(x, x_dtype, w, bias, pool, UPR_BF16, M, H * d, K, UPR_ACT_NONE, &kv, stream);
 }
 

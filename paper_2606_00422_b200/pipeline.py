@@ -115,3 +115,45 @@ class CrossAttention:
                                  k_self, v_self, ks, vs, sm_scale, self.num_splits, c.max_seq_len,
                                  stream, **self.kv_kwargs)
         return self.out
+
+
+class RankingDecodeLayer:
+    """One pre-LN decoder layer of the candidate-only ranking pass (reading Q19), as a
+    sequence of C-ABI calls -- no arithmetic here:
+        h1 = LN1(x);  q, k_self, v_self = h1 Wq^T, h1 Wk^T, h1 Wv^T
+        a  = cross-attention(q; cached history K/V of the user; own key/value)        (fp32)
+        x2 = x + a Wo^T;  h2 = LN2(x2);  y = x2 + W2 silu(W1 h2 + b1) + b2
+    x: bf16 [total_q, D]; weights bf16 [out, in] (synthetic), LN parameters fp32.  Buffers are allocated once."""
+
+    def __init__(self, attn: CrossAttention, D: int, hidden: int, params: dict, device=None):
+        self.attn = attn
+        assert attn.n_layers == 1, "one attention object per layer"
+        self.D, self.hidden, self.p = D, hidden, params
+        M, Hq, Hkv, d = attn.total_q, attn.H, attn.H_kv, attn.d
+        dev = device or attn.out.device
+        bf = dict(dtype=torch.bfloat16, device=dev)
+        self.h1 = torch.empty((M, D), **bf)
+        self.q = torch.empty((1, M, Hq, d), **bf)
+        self.ks = torch.empty((1, M, Hq, d), **bf)
+        self.vs = torch.empty((1, M, Hq, d), **bf)
+        self.x2 = torch.empty((M, D), **bf)
+        self.h2 = torch.empty((M, D), **bf)
+        self.u = torch.empty((M, hidden), **bf)
+        self.y = torch.empty((M, D), **bf)
+        self.launches = 0
+
+    def __call__(self, x: torch.Tensor, stream=None) -> torch.Tensor:
+        p, a = self.p, self.attn
+        M, Hq, d = a.total_q, a.H, a.d
+        n = 0
+        B_.upr_layernorm_fwd(x, p["ln1_g"], p["ln1_b"], self.h1, stream=stream); n += 1
+        B_.upr_linear_fwd(self.h1, p["wq"], None, self.q.view(M, Hq * d), stream=stream); n += 1
+        B_.upr_linear_fwd(self.h1, p["wk"], None, self.ks.view(M, Hq * d), stream=stream); n += 1
+        B_.upr_linear_fwd(self.h1, p["wv"], None, self.vs.view(M, Hq * d), stream=stream); n += 1
+        out = a(self.q, self.ks, self.vs, stream=stream); n += B_.upr_last_launch_count()
+        B_.upr_linear_residual_fwd(out.view(M, Hq * d), p["wo"], None, x, self.x2, stream=stream); n += 1
+        B_.upr_layernorm_fwd(self.x2, p["ln2_g"], p["ln2_b"], self.h2, stream=stream); n += 1
+        B_.upr_linear_fwd(self.h2, p["w1"], p["b1"], self.u, B_.UPR_ACT_SILU, stream=stream); n += 1
+        B_.upr_linear_residual_fwd(self.u, p["w2"], p["b2"], self.x2, self.y, stream=stream); n += 1
+        self.launches = n
+        return self.y

@@ -148,6 +148,82 @@ def test_prefill_writes_kv_into_the_pool_layout_and_attends_in_place(P):
     assert worst <= 1e-2
 
 
+def test_layernorm_and_residual_epilogue_match_oracle(P):
+    dev = "cuda"
+    M, D = 333, 1024
+    x = (S.normal_bf16(41, "x", (M, D), dev).float() * 2.0 + 0.5).to(torch.bfloat16)
+    g = 1.0 + 0.1 * S.normal_bf16(42, "g", (D,), dev).float()
+    b = 0.1 * S.normal_bf16(43, "b", (D,), dev).float()
+    y = torch.empty_like(x)
+    P.upr_layernorm_fwd(x, g, b, y)
+    torch.cuda.synchronize()
+    want = oracle.layernorm(f64(x), f64(g), f64(b))
+    assert np.abs(f64(y) - want).max() <= 2.0 ** -8 * np.abs(want).max()          # one bf16 rounding of the output
+    # residual epilogue: y = x W^T + r
+    w = weights(44, "w", 256, D, dev)
+    r = S.normal_bf16(45, "r", (M, 256), dev)
+    z = torch.empty((M, 256), dtype=torch.bfloat16, device=dev)
+    P.upr_linear_residual_fwd(x, w, None, r, z)
+    torch.cuda.synchronize()
+    want = oracle.linear(f64(x), f64(w)) + f64(r)
+    assert np.abs(f64(z) - want).max() <= 2.0 ** -8 * np.abs(want).max() + 1e-3
+
+
+def test_one_ranking_decode_layer_matches_the_oracle_chain(P):
+    """a candidate token through a whole decode layer without leaving the chip -- LN, Q / self-K,V
+    projections, cross-attention over the cached history (+ own key/value), out-projection + residual, LN, MLP
+    (SiLU) + residual -- against the same chain of oracle functions in fp64.  The oracle rounds to bf16 exactly
+    where the GPU stores bf16 (torch's cast as the library routine), so what is compared is the kernels'
+    arithmetic, not the storage format."""
+    from paper_2606_00422_b200 import pipeline as pl
+    dev = "cuda"
+    H, d, hidden = 2, 128, 512
+    D = H * d
+    L, C = [300, 64, 0, 129], [130, 17, 5, 200]
+    w = S.custom_workload("layer", 51, L, C, H, d, 1, self_term=True)
+    M = w.total_q
+    k_pool, v_pool = S.gen_pool(w, "k_pool", dev), S.gen_pool(w, "v_pool", dev)
+    slots_h = S.slot_ids(w)
+    view = pl.PoolView.of(k_pool, v_pool, torch.as_tensor(slots_h, device=dev), w.seq_lens)
+    attn = pl.CrossAttention(view, w.cand_offsets, P.UPR_BF16, kernel=P.UPR_KERNEL_PAIR)
+    prm = {"ln1_g": 1.0 + 0.1 * S.normal_bf16(52, "g1", (D,), dev).float(), "ln1_b": 0.1 * S.normal_bf16(53, "b1", (D,), dev).float(),
+           "ln2_g": 1.0 + 0.1 * S.normal_bf16(54, "g2", (D,), dev).float(), "ln2_b": 0.1 * S.normal_bf16(55, "b2", (D,), dev).float(),
+           "wq": weights(56, "wq", D, D, dev), "wk": weights(57, "wk", D, D, dev), "wv": weights(58, "wv", D, D, dev),
+           "wo": weights(59, "wo", D, D, dev), "w1": weights(60, "w1", hidden, D, dev), "w2": weights(61, "w2", D, hidden, dev),
+           "b1": 0.1 * S.normal_bf16(62, "bb1", (hidden,), dev).float(), "b2": 0.1 * S.normal_bf16(63, "bb2", (D,), dev).float()}
+    x = S.normal_bf16(64, "x", (M, D), dev)
+    layer = pl.RankingDecodeLayer(attn, D, hidden, prm)
+    y = layer(x)
+    torch.cuda.synchronize()
+    assert layer.launches == 10            # 2 LN + 6 GEMM + schedule + attention
+
+    def r16(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).to(torch.bfloat16).to(torch.float64).numpy()
+    o = {k: f64(v) for k, v in prm.items()}
+    xf = f64(x)
+    h1 = r16(oracle.layernorm(xf, o["ln1_g"], o["ln1_b"]))
+    q, ks, vs = (r16(oracle.linear(h1, o[k])) for k in ("wq", "wk", "wv"))
+    a = np.zeros((M, H, d))
+    co = w.cand_offsets
+    for b in range(w.B):
+        if co[b + 1] == co[b]:
+            continue
+        sl = slice(int(co[b]), int(co[b + 1]))
+        for h in range(H):
+            K = f64(k_pool[0, slots_h[b], h, : L[b]])
+            V = f64(v_pool[0, slots_h[b], h, : L[b]])
+            a[sl, h] = oracle.attn_block(q[sl, h * d:(h + 1) * d], K, V, ks[sl, h * d:(h + 1) * d], vs[sl, h * d:(h + 1) * d])
+    x2 = r16(oracle.linear(r16(a.reshape(M, D)), o["wo"]) + xf)   # the GEMM rounds the fp32 attention output to bf16 on its way in
+    h2 = r16(oracle.layernorm(x2, o["ln2_g"], o["ln2_b"]))
+    u = r16(oracle.linear(h2, o["w1"], o["b1"], act=oracle.ACT_SILU))
+    want = oracle.linear(u, o["w2"], o["b2"]) + x2
+    err = np.abs(f64(y) - want).max()
+    print(f"decode layer max-abs {err:.2e} (max|y| {np.abs(want).max():.2f})")
+    # nine bf16 stores on the way; a value that sits near a rounding boundary may round the other way on the GPU
+    # (2^-8 relative) and that difference propagates through the later GEMMs with unit gain: a few 2^-8 max|y|
+    assert err <= 4 * 2.0 ** -8 * np.abs(want).max()
+
+
 def test_action_heads_and_utility_match_oracle(P):
     """z -> [stacked first layers of the C heads, SiLU] (tcgen05 GEMM) -> logits -> sigmoid -> utility."""
     dev = "cuda"
