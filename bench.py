@@ -269,6 +269,40 @@ def ranking_tail(P, w, attn, q, k_self, v_self, q_host, stream, dev, ev, n_heads
                                    "device, K indices per user back"}}
 
 
+def decode_layer_leg(P, pl, w, k_pool, v_pool, slots, stream, dev, ev, hidden_mult=4, iters=5):
+    """One whole pre-LN decode layer over all candidates of the batch (layer 0's K/V, read in place; synthetic
+    weights; self key/value from the layer's own projections): LN, Q / self-K,V projections, cross-attention,
+    out-projection + residual, LN, MLP + residual -- pipeline.RankingDecodeLayer, C-ABI calls only."""
+    import math
+    D, M = w.H * w.d, w.total_q
+    hidden = hidden_mult * D
+
+    def wgt(tag, n, k):
+        return (S.normal_bf16(w.seed, tag, (n, k), dev).float() / math.sqrt(k)).to(torch.bfloat16)
+    ones, zeros = torch.ones(D, device=dev), torch.zeros(D, device=dev)
+    prm = {"ln1_g": ones, "ln1_b": zeros, "ln2_g": ones, "ln2_b": zeros, "wq": wgt("dl_wq", D, D), "wk": wgt("dl_wk", D, D),
+           "wv": wgt("dl_wv", D, D), "wo": wgt("dl_wo", D, D), "w1": wgt("dl_w1", hidden, D), "w2": wgt("dl_w2", D, hidden),
+           "b1": torch.zeros(hidden, device=dev), "b2": zeros}
+    view = pl.PoolView.of(k_pool[:1], v_pool[:1], slots, w.seq_lens)
+    attn1 = pl.CrossAttention(view, w.cand_offsets, P.UPR_BF16, num_splits=0)
+    layer = pl.RankingDecodeLayer(attn1, D, hidden, prm)
+    x = S.normal_bf16(w.seed, "dl_x", (M, D), dev)
+    for _ in range(2):
+        layer(x, stream=stream)
+    torch.cuda.synchronize()
+    e0, e1 = ev(), ev()
+    e0.record(stream)
+    for _ in range(iters):
+        layer(x, stream=stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / iters
+    gemm_flops = 2.0 * M * D * (4 * D + 2 * hidden)
+    attn_flops = (w.flops / w.n_layers) + 4.0 * w.d * M * w.H      # one layer's pairs + the self pair
+    return {"ms": ms, "candidates_per_s": M / (ms * 1e-3), "launches": layer.launches, "D_model": D, "mlp_hidden": hidden,
+            "gemm_flops": gemm_flops, "attn_flops": attn_flops, "tflops": (gemm_flops + attn_flops) / (ms * 1e-3) / 1e12}
+
+
 # ----------------------------------------------------------------------------- CUDA arm
 def run_ours(args):
     import paper_2606_00422_b200 as P
@@ -439,6 +473,8 @@ def run_ours(args):
     tail = None
     if not args.skip_tail and w.q_dtype == "bf16":
         tail = ranking_tail(P, w, attn, q, k_self, v_self, q_host, stream, dev, ev)
+        if w.kv_dtype == "bf16" and w.d == 128:
+            tail["decode_layer"] = decode_layer_leg(P, pl, w, k_pool, v_pool, slots, stream, dev, ev)
 
     if rank != 0:
         if dist is not None:
