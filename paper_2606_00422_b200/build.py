@@ -8,7 +8,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libupr.so")
 SOURCES = ["upr_api.cu"]
-HEADERS = ["ptx.cuh", "attn_kernel.cuh", "attn2_kernel.cuh", "sched_kernel.cuh", "pack_kernels.cuh", "linear_kernel.cuh", "tail_kernels.cuh", os.path.join("..", "..", "include", "upr.h")]
+HEADERS = ["ptx.cuh", "attn_kernel.cuh", "attn2_kernel.cuh", "sched_kernel.cuh", "pack_kernels.cuh", "linear_kernel.cuh", "linear2_kernel.cuh", "tail_kernels.cuh", os.path.join("..", "..", "include", "upr.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC"]
 

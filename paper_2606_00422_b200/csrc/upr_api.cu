@@ -12,6 +12,7 @@
 #include "../../include/upr.h"
 #include "attn2_kernel.cuh"
 #include "attn_kernel.cuh"
+#include "linear2_kernel.cuh"
 #include "linear_kernel.cuh"
 #include "pack_kernels.cuh"
 #include "sched_kernel.cuh"
@@ -686,11 +687,32 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   a.K = K;
   a.act = static_cast<int>(act);
   a.y_is_f32 = y_dtype == UPR_F32;
-  const long long tiles = ((M + 127) / 128) * ((N + 127) / 128);
-  int grid = sm_count();
-  if (grid <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
-  if (tiles < grid) grid = static_cast<int>(tiles);
+  int sms = sm_count();
+  if (sms <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  // 256 x 256 tiles on CTA pairs when there are enough of them to fill the machine's SM pairs; small problems
+  // (and narrow layers, N <= 128) keep the 128 x 128 single-CTA kernel
+  const long long tiles2 = ((M + 255) / 256) * ((N + 255) / 256);
+  if (N > 128 && tiles2 >= sms / 2) {
+    int pairs = sms / 2;
+    if (x_dtype == UPR_F32) {
+      using C = upr::lin2::Cfg<true>;
+      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<true>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemTotal));
+      upr::lin2::upr_linear_pair_kernel<true><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
+    } else {
+      using C = upr::lin2::Cfg<false>;
+      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<false>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemTotal));
+      upr::lin2::upr_linear_pair_kernel<false><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
+    }
+    UPR_CUDA_CHECK(cudaGetLastError());
+    g_launches = 1;
+    return UPR_OK;
+  }
+  const long long tiles = ((M + 127) / 128) * ((N + 127) / 128);
+  int grid = sms;
+  if (tiles < grid) grid = static_cast<int>(tiles);
   if (x_dtype == UPR_F32) {
     UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin::upr_linear_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         upr::lin::kSmemTotal));

@@ -47,6 +47,10 @@ LINEAR_CASES = [
     (517, 1024, 1024, "f32", "bf16", 0, True),     # fp32 activations (the attention output) converted in-kernel
     (130, 264, 128, "f32", "f32", 2, True),
     (4099, 384, 256, "bf16", "f32", 1, False),     # more tiles than SMs
+    # enough 256 x 256 tiles for every SM pair: the CTA-pair kernel (cta_group::2) takes these
+    (9500, 640, 512, "bf16", "bf16", 1, True),     # ragged M, N = 2.5 tiles
+    (9500, 640, 512, "f32", "f32", 0, True),       # fp32 x: converters in both CTAs
+    (19001, 256, 128, "bf16", "f32", 2, False),    # a single N tile, two k-steps
 ]
 
 
@@ -222,6 +226,35 @@ def test_one_ranking_decode_layer_matches_the_oracle_chain(P):
     # nine bf16 stores on the way; a value that sits near a rounding boundary may round the other way on the GPU
     # (2^-8 relative) and that difference propagates through the later GEMMs with unit gain: a few 2^-8 max|y|
     assert err <= 4 * 2.0 ** -8 * np.abs(want).max()
+
+
+def test_pair_gemm_residual_and_pool_epilogues(P):
+    """The CTA-pair GEMM's residual and pool-addressing epilogues (M large enough for the pair kernel)."""
+    dev = "cuda"
+    M, D = 19200, 256
+    x = S.normal_bf16(71, "x", (M, D), dev)
+    w = weights(72, "w", D, D, dev)
+    r = S.normal_bf16(73, "r", (M, D), dev)
+    z = torch.empty((M, D), dtype=torch.bfloat16, device=dev)
+    P.upr_linear_residual_fwd(x, w, None, r, z)
+    torch.cuda.synchronize()
+    want = oracle.linear(f64(x), f64(w))
+    assert np.abs(f64(z) - (want + f64(r))).max() <= 2.0 ** -8 * np.abs(want + f64(r)).max() + 1e-3
+    # K projection of 19 200 tokens (96 users x 200 positions) into a pool [1, 100, 2, 200, 128]
+    H, d, S_slots, n = 2, 128, 100, 200
+    pool = torch.zeros((1, S_slots, H, n, d), dtype=torch.bfloat16, device=dev)
+    slot_of_user = np.random.default_rng(3).permutation(S_slots)[:96].astype(np.int32)
+    tok_slot = torch.from_numpy(np.repeat(slot_of_user, n)).to(dev)
+    tok_pos = torch.from_numpy(np.tile(np.arange(n, dtype=np.int32), 96)).to(dev)
+    P.upr_kv_project_into_pool(x, w, None, pool, tok_slot, tok_pos, 0)
+    torch.cuda.synchronize()
+    got = f64(pool)
+    for u in (0, 37, 95):
+        for h in range(H):
+            blk = want[u * n:(u + 1) * n, h * d:(h + 1) * d]
+            assert np.abs(got[0, slot_of_user[u], h] - blk).max() <= 2.0 ** -8 * max(1.0, np.abs(blk).max())
+    unused = np.setdiff1d(np.arange(S_slots), slot_of_user)
+    assert not got[0, unused].any()
 
 
 def test_action_heads_and_utility_match_oracle(P):
