@@ -297,10 +297,30 @@ def decode_layer_leg(P, pl, w, k_pool, v_pool, slots, stream, dev, ev, hidden_mu
     e1.record(stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / iters
+    # the MLP's up-projection alone, bf16 operands vs FP8 E4M3 operands with fused scaling
+    def time_it(fn):
+        fn(); fn()
+        torch.cuda.synchronize()
+        a0, a1 = ev(), ev()
+        a0.record(stream)
+        for _ in range(iters):
+            fn()
+        a1.record(stream)
+        torch.cuda.synchronize()
+        return a0.elapsed_time(a1) / iters
+    w1f = prm["w1"].float()
+    w_scale = float(w1f.abs().max().item()) / 448.0
+    w1_8 = (w1f / w_scale).to(torch.float8_e4m3fn).view(torch.uint8)
+    up_bf16 = time_it(lambda: P.upr_linear_fwd(layer.h2, prm["w1"], prm["b1"], layer.u, P.UPR_ACT_SILU, stream))
+    up_fp8 = time_it(lambda: P.upr_linear_fp8_fwd(layer.h2, 6.0 / 448.0, w1_8, w_scale, prm["b1"], None, layer.u,
+                                                  P.UPR_ACT_SILU, stream))
+    fl_up = 2.0 * M * D * hidden
     gemm_flops = 2.0 * M * D * (4 * D + 2 * hidden)
     attn_flops = (w.flops / w.n_layers) + 4.0 * w.d * M * w.H      # one layer's pairs + the self pair
     return {"ms": ms, "candidates_per_s": M / (ms * 1e-3), "launches": layer.launches, "D_model": D, "mlp_hidden": hidden,
-            "gemm_flops": gemm_flops, "attn_flops": attn_flops, "tflops": (gemm_flops + attn_flops) / (ms * 1e-3) / 1e12}
+            "gemm_flops": gemm_flops, "attn_flops": attn_flops, "tflops": (gemm_flops + attn_flops) / (ms * 1e-3) / 1e12,
+            "mlp_up_bf16_ms": up_bf16, "mlp_up_bf16_tflops": fl_up / (up_bf16 * 1e-3) / 1e12,
+            "mlp_up_fp8_ms": up_fp8, "mlp_up_fp8_tflops": fl_up / (up_fp8 * 1e-3) / 1e12}
 
 
 # ----------------------------------------------------------------------------- CUDA arm

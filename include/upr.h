@@ -225,6 +225,17 @@ upr_status upr_linear_residual_fwd(const void* x, upr_dtype x_dtype, const void*
                                    const void* residual, void* y, upr_dtype y_dtype, int64_t M, int N, int K,
                                    upr_activation act, void* stream);
 
+/*
+ * FP8 linear layer with fused scaling ("mixed-precision FP8 ... E4M3 during the forward pass"; the
+ * paper's are Transformer Engine modules): y = act((q(x) q(W)^T) * x_scale * w_scale + bias) [+ residual], where
+ *     q(x) = cvt.rn.satfinite.e4m3(x * (1.0f / x_scale))   -- quantised INSIDE the kernel, per-tensor scale
+ *     w_e4m3 = the weights already quantised to E4M3 bytes [N, K] with the per-tensor scale w_scale
+ * tcgen05.mma kind::f8f6f4 on CTA pairs, fp32 accumulation.  x device bf16 [M, K]; K % 128 == 0, N % 8 == 0.
+ */
+upr_status upr_linear_fp8_fwd(const void* x, float x_scale, const void* w_e4m3, float w_scale, const float* bias,
+                              const void* residual, void* y, upr_dtype y_dtype, int64_t M, int N, int K,
+                              upr_activation act, void* stream);
+
 /* Layer normalisation of candidate tokens: y = (x - mean) / sqrt(var + eps) * gamma + beta over the
  * hidden dimension; x, y device bf16 [M, D]; gamma, beta device fp32 [D]; D % 8 == 0, D <= 4096. */
 upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,

@@ -287,3 +287,16 @@ def layernorm(x, gamma, beta, eps: float = 1e-5):
     y = np.zeros((M, D), dtype=np.float64)
     lib().upro_layernorm(_p(x), _p(gamma), _p(beta), ctypes.c_int64(M), D, ctypes.c_double(eps), _p(y))
     return y
+
+
+def linear_fp8(x, x_scale: float, w8, w_scale: float, b=None, act: int = ACT_NONE):
+    """FP8 E4M3 linear layer with fused per-tensor scaling: x [M,K] float32 values, w8 [N,K] E4M3 bytes."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    w8 = np.ascontiguousarray(w8, dtype=np.uint8)
+    M, K = x.shape
+    N = w8.shape[0]
+    bb = _c64(b) if b is not None else None
+    y = np.zeros((M, N), dtype=np.float64)
+    lib().upro_linear_fp8(_p(x), ctypes.c_float(x_scale), _p(w8), ctypes.c_float(w_scale), _p(bb), ctypes.c_int64(M), N, K,
+                          act, _p(y))
+    return y

@@ -683,3 +683,36 @@ void upro_layernorm(const double* x, const double* gamma, const double* beta, in
     for (int t = 0; t < D; ++t) y[m * D + t] = (x[m * D + t] - mean) * r * gamma[t] + beta[t];
   }
 }
+
+/* ------------------------------------------------------------------------------------
+ * upro_linear_fp8 -- a linear layer with FP8 E4M3 operands and fused per-tensor scaling
+ * (FP8 forward in E4M3; reading Q20):
+ *     q(x)   = e4m3_rne_satfinite( x * (1.0f / x_scale) )      product rounded once in fp32
+ *     y[m,n] = act( x_scale * w_scale * sum_k dec(q(x)[m,k]) * dec(w8[n,k]) + b[n] )
+ * x [M,K] fp32 values (the bf16 activations widened), w8 [N,K] E4M3 bytes.  fp64 accumulation.
+ * ---------------------------------------------------------------------------------- */
+void upro_linear_fp8(const float* x, float x_scale, const uint8_t* w8, float w_scale,
+                     const double* b, int64_t M, int N, int K, int act, double* y) {
+  float mult = 1.0f / x_scale;
+  double* xq = (double*)malloc(sizeof(double) * (size_t)M * K);
+  double* wq = (double*)malloc(sizeof(double) * (size_t)N * K);
+  for (int64_t i = 0; i < M * (int64_t)K; ++i) {
+    volatile float p = x[i] * mult; /* one fp32 rounding */
+    xq[i] = upro_e4m3_decode(upro_e4m3_encode(p));
+  }
+  for (int64_t i = 0; i < (int64_t)N * K; ++i) wq[i] = upro_e4m3_decode(w8[i]);
+  double s = (double)x_scale * (double)w_scale;
+#pragma omp parallel for schedule(static)
+  for (int64_t m = 0; m < M; ++m)
+    for (int n = 0; n < N; ++n) {
+      double acc = 0.0;
+      for (int k = 0; k < K; ++k) acc += xq[m * K + k] * wq[(int64_t)n * K + k];
+      acc *= s;
+      if (b) acc += b[n];
+      if (act == 1) acc = acc / (1.0 + exp(-acc));
+      else if (act == 2) acc = acc > 0.0 ? acc : 0.0;
+      y[m * N + n] = acc;
+    }
+  free(xq);
+  free(wq);
+}

@@ -10,6 +10,7 @@
 #pragma once
 #include <cuda.h>
 #include <cuda_bf16.h>
+#include <cuda_fp8.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -26,16 +27,20 @@ using lin::ACT_NONE;
 using lin::ACT_RELU;
 using lin::ACT_SILU;
 
-constexpr int kThreads = 320;
+constexpr int kThreads = 448;                   // warps: 0 producer, 1 MMA, 2-3 + 8-9 converters, 4-7 + 10-13 epilogue
 constexpr int kBM = 256, kBN = 256, kBK = 64;   // per pair; each CTA: 128 rows of x, 128 rows of W
 constexpr int kTileBytes = 128 * kBK * 2;       // 16 KB: one CTA's x tile or W half tile (bf16)
 constexpr int kRawBytes = 128 * kBK * 4;        // 32 KB: one CTA's fp32 x tile as loaded
 constexpr int kConvThreads = 128;               // warps 2, 3, 8, 9
 
-template <bool X_F32>
+enum : int { MODE_BF16 = 0, MODE_XF32 = 1, MODE_FP8 = 2 };   // operands: bf16 x bf16; fp32 x converted; e4m3 x e4m3 (x quantised in-kernel)
+
+template <int MODE>
 struct Cfg {
-  static constexpr int kStages = X_F32 ? 4 : 6;
-  static constexpr int kRawStages = X_F32 ? 2 : 0;
+  static constexpr bool kConv = MODE != MODE_BF16;
+  static constexpr int kStages = kConv ? 4 : 6;
+  static constexpr int kRawStages = kConv ? 2 : 0;
+  static constexpr int kKStep = (MODE == MODE_FP8) ? 128 : 64;   // elements of K per stage: one 128-byte row per operand row
   static constexpr int kSmemCtrl = 1024;
   static constexpr int kSmemTotal = kStages * 2 * kTileBytes + kRawStages * kRawBytes + kSmemCtrl + 1024;
   static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
@@ -49,12 +54,13 @@ struct __align__(16) Ctrl {
 };
 static_assert(sizeof(Ctrl) <= 1024, "control block too large");
 
-template <bool X_F32>
+template <int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 rows x 64 k (bf16: SWIZZLE_128B; fp32: none)
                        const __grid_constant__ CUtensorMap tmap_w,   // bf16 [N, K], box 128 x 64, SWIZZLE_128B
                        const Args args) {
-  using C = Cfg<X_F32>;
+  using C = Cfg<MODE>;
+  constexpr bool X_F32 = C::kConv;   // x goes through the converter warps
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   uint8_t* smem_aligned = smem_raw + (smem_base - smem_u32(smem_raw));
@@ -69,7 +75,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
   const int pair_id = blockIdx.x >> 1, n_pairs = gridDim.x >> 1;
   const int m_tiles = static_cast<int>((args.M + kBM - 1) / kBM);
   const int n_tiles = (args.N + kBN - 1) / kBN;
-  const int k_steps = args.K / kBK;
+  const int k_steps = args.K / C::kKStep;
   const long long total_tiles = static_cast<long long>(m_tiles) * n_tiles;
 
   if (threadIdx.x == 0) {
@@ -83,7 +89,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
       mbar_init(smem_u32(&ctrl->raw_full[i]), 1);
       mbar_init(smem_u32(&ctrl->raw_empty[i]), 4);
       mbar_init(smem_u32(&ctrl->acc_full[i]), 1);   // multicast commit
-      mbar_init(smem_u32(&ctrl->acc_empty[i]), 8);  // 4 epilogue warps of each CTA (leader's copy)
+      mbar_init(smem_u32(&ctrl->acc_empty[i]), 16); // 8 epilogue warps of each CTA (leader's copy)
     }
     fence_mbar_init();
   }
@@ -116,12 +122,12 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
           const uint32_t full = lead_full + s * 8;
           if (X_F32) {
             if (leader) mbar_arrive_expect_tx(smem_u32(&ctrl->full[s]), 2 * kTileBytes);
-            tma_load_2d_pair(b_smem + s * kTileBytes, &tmap_w, ks * kBK, wrow, full);
+            tma_load_2d_pair(b_smem + s * kTileBytes, &tmap_w, ks * C::kKStep, wrow, full);
             const uint32_t rs = raw_it % 2, rph = (raw_it / 2) & 1;
             mbar_wait<2>(smem_u32(&ctrl->raw_empty[rs]), rph ^ 1);
             const uint32_t rfull = smem_u32(&ctrl->raw_full[rs]);
             mbar_arrive_expect_tx(rfull, kRawBytes);
-            tma_load_2d(raw_smem + rs * kRawBytes, &tmap_x, ks * kBK, xrow, rfull);
+            tma_load_2d(raw_smem + rs * kRawBytes, &tmap_x, ks * C::kKStep, xrow, rfull);
             ++raw_it;
           } else {
             if (leader) mbar_arrive_expect_tx(smem_u32(&ctrl->full[s]), 4 * kTileBytes);
@@ -138,7 +144,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
       if (elect_one()) {
         constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);   // SBO 1024, version 1, SWIZZLE_128B
         constexpr uint32_t kLoK = (16u >> 4) << 16;
-        constexpr uint32_t kIdesc = make_idesc_bf16(kBM, kBN, 0, 0);
+        constexpr uint32_t kIdesc = (MODE == MODE_FP8) ? make_idesc_e4m3(kBM, kBN) : make_idesc_bf16(kBM, kBN, 0, 0);
         auto mk_desc = [](uint32_t lo) {
           return (static_cast<uint64_t>(kDescHi) << 32) | static_cast<uint64_t>(lo);
         };
@@ -154,9 +160,12 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
             mbar_wait<4>(smem_u32(&ctrl->full[s]), ph);
             tc_fence_after();
 #pragma unroll
-            for (int k = 0; k < kBK / 16; ++k)
-              umma_ss_pair(tmem_base + ab * kBN, mk_desc(a_lo + ((s * kTileBytes + k * 32) >> 4)),
-                           mk_desc(b_lo + ((s * kTileBytes + k * 32) >> 4)), kIdesc, (ks > 0 || k > 0) ? 1u : 0u);
+            for (int k = 0; k < 4; ++k) {   // 32 bytes of K per instruction: 16 bf16 or 32 e4m3 elements
+              const uint64_t da = mk_desc(a_lo + ((s * kTileBytes + k * 32) >> 4));
+              const uint64_t db = mk_desc(b_lo + ((s * kTileBytes + k * 32) >> 4));
+              if (MODE == MODE_FP8) umma_ss_pair_f8(tmem_base + ab * kBN, da, db, kIdesc, (ks > 0 || k > 0) ? 1u : 0u);
+              else umma_ss_pair(tmem_base + ab * kBN, da, db, kIdesc, (ks > 0 || k > 0) ? 1u : 0u);
+            }
             umma_commit_pair(smem_u32(&ctrl->empty[s]));
           }
           umma_commit_pair(smem_u32(&ctrl->acc_full[ab]));
@@ -164,8 +173,8 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
       }
     }
     __syncwarp();
-  } else if (warp == 2 || warp == 3 || warp >= 8) {
-    // ================================================================= converters (fp32 x), both CTAs
+  } else if (warp == 2 || warp == 3 || warp == 8 || warp == 9) {
+    // ================================================================= converters (fp32 x / FP8), both CTAs
     if constexpr (X_F32) {
       const int ctid = (warp < 4 ? warp - 2 : warp - 6) * 32 + lane;   // 0..127
       const uint32_t lead_full = mapa_shared(smem_u32(&ctrl->full[0]), 0);
@@ -178,6 +187,27 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
           mbar_wait<6>(smem_u32(&ctrl->raw_full[rs]), rph);
           const uint32_t raw = raw_smem + rs * kRawBytes;
           const uint32_t tile = a_smem + s * kTileBytes;
+          if constexpr (MODE == MODE_FP8) {
+            // raw: 128 rows x 128 bf16 (256 B per row) -> 128 rows x 128 e4m3 (one swizzled 128-byte row each);
+            // byte = cvt.rn.satfinite.e4m3(x * x_mult), the product rounded once in fp32
+#pragma unroll 4
+            for (int p = ctid; p < 128 * 8; p += kConvThreads) {
+              const int row = p >> 3, c16 = p & 7;                 // 16 bf16 -> one 16-byte e4m3 chunk
+              const uint4 a = lds128(raw + row * 256 + c16 * 32), b = lds128(raw + row * 256 + c16 * 32 + 16);
+              const uint32_t in[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+              uint32_t o[4];
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                const float f0 = __uint_as_float(in[2 * k] << 16) * args.x_mult;
+                const float f1 = __uint_as_float(in[2 * k] & 0xffff0000u) * args.x_mult;
+                const float f2 = __uint_as_float(in[2 * k + 1] << 16) * args.x_mult;
+                const float f3 = __uint_as_float(in[2 * k + 1] & 0xffff0000u) * args.x_mult;
+                o[k] = static_cast<uint32_t>(__nv_cvt_float2_to_fp8x2(make_float2(f0, f1), __NV_SATFINITE, __NV_E4M3)) |
+                       (static_cast<uint32_t>(__nv_cvt_float2_to_fp8x2(make_float2(f2, f3), __NV_SATFINITE, __NV_E4M3)) << 16);
+              }
+              sts128(tile + row * 128 + ((c16 ^ (row & 7)) << 4), o[0], o[1], o[2], o[3]);
+            }
+          } else {
 #pragma unroll 4
           for (int p = ctid; p < 128 * 8; p += kConvThreads) {
             const int row = p >> 3, c8 = p & 7;                  // 8 floats -> one 16-byte bf16 chunk
@@ -187,6 +217,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
                    pack_bf16x2(__uint_as_float(a.z), __uint_as_float(a.w)),
                    pack_bf16x2(__uint_as_float(b.x), __uint_as_float(b.y)),
                    pack_bf16x2(__uint_as_float(b.z), __uint_as_float(b.w)));
+          }
           }
           fence_proxy_async_smem();   // generic-proxy tile writes -> visible to tcgen05.mma
           __syncwarp();
@@ -198,8 +229,11 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
       }
     }
   } else {
-    // ================================================================= epilogue (warps 4-7, both CTAs)
-    const int ew = warp - 4;                                   // TMEM lane quarter
+    // ================================================================= epilogue (both CTAs)
+    // two groups of four warps: warps 4-7 take the accumulator's columns [0, 128), warps 10-13 [128, 256) -- with
+    // a fused activation the epilogue of a 256-column tile is otherwise slower than the tile's MMAs
+    const int ew = warp & 3;                                   // TMEM lane quarter (== warp % 4)
+    const int ehalf = warp >= 10 ? 1 : 0;
     const uint32_t lane_base = static_cast<uint32_t>(ew * 32) << 16;
     const uint32_t lead_acc_empty = mapa_shared(smem_u32(&ctrl->acc_empty[0]), 0);
     uint32_t n_acc = 0;
@@ -221,7 +255,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
         uint32_t r[32];
         tmem_ld32(tmem_base + lane_base + ab * kBN + c0, r);
         tmem_wait_ld_regs(r);
-        if (c0 + 32 == kBN) {
+        if (c0 + 32 == (ehalf + 1) * (kBN / 2)) {   // this warp's last chunk is in registers
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(lead_acc_empty + ab * 8);
@@ -235,6 +269,10 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
           float v[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k) v[k] = __uint_as_float(r[c + k]);
+          if (MODE == MODE_FP8) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) v[k] *= args.out_scale;
+          }
           if (args.bias != nullptr) {
             const float4 b0 = __ldg(reinterpret_cast<const float4*>(args.bias + col0 + c));
             const float4 b1 = __ldg(reinterpret_cast<const float4*>(args.bias + col0 + c + 4));
@@ -275,7 +313,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
         }
       };
 #pragma unroll 1
-      for (int c0 = 0; c0 < kBN; c0 += 32) {
+      for (int c0 = ehalf * (kBN / 2); c0 < (ehalf + 1) * (kBN / 2); c0 += 32) {
         if (args.act == ACT_SILU) chunk(cuda::std::integral_constant<int, ACT_SILU>{}, c0);
         else if (args.act == ACT_RELU) chunk(cuda::std::integral_constant<int, ACT_RELU>{}, c0);
         else chunk(cuda::std::integral_constant<int, ACT_NONE>{}, c0);

@@ -47,6 +47,8 @@ struct Args {
   int N, K;
   int act;
   int y_is_f32;
+  float out_scale;        // multiplies the accumulator before the bias (FP8 operands: x_scale * w_scale; else 1)
+  float x_mult;           // FP8 operands: x is quantised as e4m3(x * x_mult), x_mult = 1 / x_scale
   // K/V projection written straight into the pool layout [layers, S, H, n, d]: row m of y is token
   // m's [H, d] vector and goes to pool[layer, tok_slot[m], h, tok_pos[m], :]; y = the pool (bf16), N = H * d
   const int32_t* tok_slot;

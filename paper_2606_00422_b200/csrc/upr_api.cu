@@ -626,7 +626,8 @@ upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream) {
 
 // ------------------------------------------------------------------ decode-layer tail, consumer, pool
 namespace {
-struct KvScatter { const int32_t* tok_slot; const int32_t* tok_pos; int layer, S, H, n, d; const void* residual; };
+struct KvScatter { const int32_t* tok_slot; const int32_t* tok_pos; int layer, S, H, n, d; const void* residual;
+                   int fp8; float x_scale, w_scale; };
 }  // namespace
 
 static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
@@ -638,7 +639,11 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   if (y_dtype != UPR_BF16 && y_dtype != UPR_F32) return fail(UPR_ERR_UNSUPPORTED, "y_dtype %d (bf16 or f32)", (int)y_dtype);
   if (act != UPR_ACT_NONE && act != UPR_ACT_SILU && act != UPR_ACT_RELU)
     return fail(UPR_ERR_INVALID_ARG, "activation %d unknown", (int)act);
-  if (K % 64 != 0 || N % 8 != 0) return fail(UPR_ERR_UNSUPPORTED, "K=%d must be a multiple of 64, N=%d of 8", K, N);
+  const bool fp8 = kv != nullptr && kv->fp8;
+  if (K % (fp8 ? 128 : 64) != 0 || N % 8 != 0)
+    return fail(UPR_ERR_UNSUPPORTED, "K=%d must be a multiple of %d, N=%d of 8", K, fp8 ? 128 : 64, N);
+  if (fp8 && x_dtype != UPR_BF16) return fail(UPR_ERR_UNSUPPORTED, "FP8 linear layers take bf16 activations");
+  if (fp8 && (!(kv->x_scale > 0.f) || !(kv->w_scale > 0.f))) return fail(UPR_ERR_INVALID_ARG, "scales must be > 0");
   if (M == 0) return UPR_OK;
   if (!x || !w || !y) return fail(UPR_ERR_INVALID_ARG, "NULL tensor pointer");
   if ((reinterpret_cast<uintptr_t>(x) & 15) || (reinterpret_cast<uintptr_t>(w) & 15) || (reinterpret_cast<uintptr_t>(y) & 15))
@@ -649,21 +654,22 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   EncodeTiledFn enc = get_encode_fn();
   if (enc == nullptr) return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled entry point not found");
   CUtensorMap tx, tw;
-  cuuint32_t box[2] = {64, 128}, estr[2] = {1, 1};
+  cuuint32_t box[2] = {static_cast<cuuint32_t>(fp8 ? 128 : 64), 128}, estr[2] = {1, 1};
   {
     const bool f32 = x_dtype == UPR_F32;
     cuuint64_t gdim[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(M)};
     cuuint64_t gstride[1] = {static_cast<cuuint64_t>(K) * (f32 ? 4 : 2)};
     if (enc(&tx, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(x),
             gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            f32 ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            (f32 || fp8) ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for x");
   }
   {
     cuuint64_t gdim[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(N)};
-    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(K) * 2};
-    if (enc(&tw, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(w), gdim, gstride, box, estr,
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(K) * (fp8 ? 1 : 2)};
+    if (enc(&tw, fp8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(w), gdim,
+            gstride, box, estr,
             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for w");
@@ -687,24 +693,32 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   a.K = K;
   a.act = static_cast<int>(act);
   a.y_is_f32 = y_dtype == UPR_F32;
+  a.out_scale = fp8 ? kv->x_scale * kv->w_scale : 1.0f;
+  a.x_mult = fp8 ? 1.0f / kv->x_scale : 1.0f;
   int sms = sm_count();
   if (sms <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   // 256 x 256 tiles on CTA pairs when there are enough of them to fill the machine's SM pairs; small problems
   // (and narrow layers, N <= 128) keep the 128 x 128 single-CTA kernel
   const long long tiles2 = ((M + 255) / 256) * ((N + 255) / 256);
-  if (N > 128 && tiles2 >= sms / 2) {
+  if (fp8 || (N > 128 && tiles2 >= sms / 2)) {
     int pairs = sms / 2;
-    if (x_dtype == UPR_F32) {
-      using C = upr::lin2::Cfg<true>;
-      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<true>,
+    if (tiles2 < pairs) pairs = static_cast<int>(tiles2);
+    if (fp8) {
+      using C = upr::lin2::Cfg<upr::lin2::MODE_FP8>;
+      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_FP8>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemTotal));
-      upr::lin2::upr_linear_pair_kernel<true><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
+      upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_FP8><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
+    } else if (x_dtype == UPR_F32) {
+      using C = upr::lin2::Cfg<upr::lin2::MODE_XF32>;
+      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_XF32>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemTotal));
+      upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_XF32><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
     } else {
-      using C = upr::lin2::Cfg<false>;
-      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<false>,
+      using C = upr::lin2::Cfg<upr::lin2::MODE_BF16>;
+      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_BF16>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemTotal));
-      upr::lin2::upr_linear_pair_kernel<false><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
+      upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_BF16><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
     }
     UPR_CUDA_CHECK(cudaGetLastError());
     g_launches = 1;
@@ -737,8 +751,17 @@ upr_status upr_linear_residual_fwd(const void* x, upr_dtype x_dtype, const void*
                                    upr_activation act, void* stream) {
   if (residual != nullptr && (reinterpret_cast<uintptr_t>(residual) & 15))
     return fail(UPR_ERR_INVALID_ARG, "residual must be 16-byte aligned");
-  KvScatter kv{nullptr, nullptr, 0, 0, 0, 0, 0, residual};
+  KvScatter kv{nullptr, nullptr, 0, 0, 0, 0, 0, residual, 0, 1.f, 1.f};
   return linear_impl(x, x_dtype, w, bias, y, y_dtype, M, N, K, act, &kv, stream);
+}
+
+upr_status upr_linear_fp8_fwd(const void* x, float x_scale, const void* w_e4m3, float w_scale, const float* bias,
+                              const void* residual, void* y, upr_dtype y_dtype, int64_t M, int N, int K,
+                              upr_activation act, void* stream) {
+  if (residual != nullptr && (reinterpret_cast<uintptr_t>(residual) & 15))
+    return fail(UPR_ERR_INVALID_ARG, "residual must be 16-byte aligned");
+  KvScatter kv{nullptr, nullptr, 0, 0, 0, 0, 0, residual, 1, x_scale, w_scale};
+  return linear_impl(x, UPR_BF16, w_e4m3, bias, y, y_dtype, M, N, K, act, &kv, stream);
 }
 
 upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,
@@ -766,7 +789,7 @@ upr_status upr_kv_project_into_pool(const void* x, upr_dtype x_dtype, const void
     return fail(UPR_ERR_INVALID_ARG, "bad pool shape / layer (layers=%d S=%d H=%d n=%d layer=%d)", n_layers, S, H, n, layer);
   if (d != 64 && d != 128) return fail(UPR_ERR_UNSUPPORTED, "head dim d=%d unsupported (64 or 128)", d);
   if (M > 0 && (!tok_slot || !tok_pos)) return fail(UPR_ERR_INVALID_ARG, "tok_slot / tok_pos is NULL");
-  KvScatter kv{tok_slot, tok_pos, layer, S, H, n, d, nullptr};
+  KvScatter kv{tok_slot, tok_pos, layer, S, H, n, d, nullptr, 0, 1.f, 1.f};
   return linear_impl(x, x_dtype, w, bias, pool, UPR_BF16, M, H * d, K, UPR_ACT_NONE, &kv, stream);
 }
 

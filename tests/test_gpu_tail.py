@@ -257,6 +257,29 @@ def test_pair_gemm_residual_and_pool_epilogues(P):
     assert not got[0, unused].any()
 
 
+@pytest.mark.parametrize("shape", [(300, 136, 256), (9500, 640, 512), (64, 8, 128)], ids=["ragged", "many_tiles", "tiny"])
+def test_linear_fp8_matches_oracle(P, shape):
+    """PAPER.md:206 / SURVEY 8(f)1: FP8 E4M3 linear layer with fused scaling (tcgen05 kind::f8f6f4 on CTA pairs): the
+    activations are quantised inside the kernel exactly as the oracle does (one fp32 product, RNE, satfinite), the
+    weights arrive as E4M3 bytes, so both sides multiply the SAME operands: what differs is fp32 accumulation."""
+    M, N, K = shape
+    dev = "cuda"
+    x = S.normal_bf16(81, "x", (M, K), dev)
+    wf = (S.normal_bf16(82, "w", (N, K), dev).float() / np.sqrt(K))
+    x_scale = float(np.float32(4.5) / np.float32(448.0))            # a fixed ("delayed") activation scale: clips beyond 4.5 sigma
+    w_scale = float(np.float32(wf.abs().max().item()) / np.float32(448.0))
+    w8 = (wf * (np.float32(1.0) / np.float32(w_scale))).to(torch.float8_e4m3fn).view(torch.uint8)   # offline weight quantisation
+    b = S.normal_bf16(83, "b", (N,), dev).float() * 0.5
+    r = S.normal_bf16(84, "r", (M, N), dev)
+    y = torch.empty((M, N), dtype=torch.float32, device=dev)
+    P.upr_linear_fp8_fwd(x, x_scale, w8, w_scale, b, r, y, P.UPR_ACT_SILU)
+    torch.cuda.synchronize()
+    want = oracle.linear_fp8(x.float().cpu().numpy(), x_scale, w8.cpu().numpy(), w_scale, f64(b), act=oracle.ACT_SILU) + f64(r)
+    err = np.abs(f64(y) - want).max()
+    print(f"fp8 linear max-abs {err:.2e} (max|y| {np.abs(want).max():.2f})")
+    assert err <= 2e-4 * max(1.0, np.abs(want).max())
+
+
 def test_action_heads_and_utility_match_oracle(P):
     """z -> [stacked first layers of the C heads, SiLU] (tcgen05 GEMM) -> logits -> sigmoid -> utility."""
     dev = "cuda"

@@ -149,3 +149,27 @@ def test_layernorm_against_torch_and_closed_forms(oracle):
     # hand case: x = (1, 3): mean 2, var 1 -> (-1, 1) * gamma + beta
     np.testing.assert_allclose(oracle.layernorm(np.array([[1.0, 3.0]]), np.array([2.0, 3.0]), np.array([0.5, -0.5]), eps=0.0),
                                [[-1.5, 2.5]], atol=1e-15)
+
+
+# ----------------------------------------------------------------------------- FP8 linear
+def test_linear_fp8_against_torch_float8_and_the_exact_case(oracle):
+    r = rng(8)
+    M, N, K = 7, 5, 32
+    x = r.standard_normal((M, K)).astype(np.float32)
+    w = r.standard_normal((N, K)).astype(np.float32)
+    xs, ws = np.float32(np.abs(x).max() / 448.0), np.float32(np.abs(w).max() / 448.0)
+    w8 = torch.from_numpy(w * (np.float32(1.0) / ws)).to(torch.float8_e4m3fn).view(torch.uint8).numpy()
+    got = oracle.linear_fp8(x, float(xs), w8, float(ws))
+    # torch's float8 cast as the library routine for both operands
+    xq = torch.from_numpy(x * (np.float32(1.0) / xs)).to(torch.float8_e4m3fn).to(torch.float64).numpy()
+    wq = torch.from_numpy(w8).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+    np.testing.assert_allclose(got, (xq @ wq.T) * float(xs) * float(ws), rtol=0, atol=1e-12)
+    # quantisation error is what FP8 costs: ~2^-4 relative per operand, averaged over K
+    assert np.abs(got - x.astype(np.float64) @ w.astype(np.float64).T).max() < 0.6
+    # operands that are exactly representable with scale 1: identical to the plain linear layer
+    xi = r.integers(-8, 9, size=(M, K)).astype(np.float32)
+    wi = r.integers(-8, 9, size=(N, K)).astype(np.float32)
+    wi8 = oracle.e4m3_encode(wi)
+    np.testing.assert_array_equal(oracle.linear_fp8(xi, 1.0, wi8, 1.0), oracle.linear(xi, wi))
+    # scales factor out: y(x, 2 x_scale) with x doubled == 2 y
+    np.testing.assert_allclose(oracle.linear_fp8(2 * xi, 2.0, wi8, 1.0), 2 * oracle.linear(xi, wi), rtol=0, atol=1e-12)
