@@ -324,6 +324,45 @@ def test_causal_needs_the_pair_kernel(P):
     assert e.value.status == 2
 
 
+@pytest.mark.parametrize("kernel", ["single", "pair"])
+def test_forward_is_cuda_graph_capturable(P, kernel):
+    """upr.h: calls never synchronise, never read device tables on the host and are CUDA-graph capturable.  Capture
+    schedule kernel + attention (+ combine) once, replay with NEW query values and NEW history lengths / candidate
+    offsets written into the same device buffers: the replayed result must match the oracle for the new inputs."""
+    from paper_2606_00422_b200 import pipeline as pl
+    L1, C1 = [300, 64, 0, 129], [130, 17, 5, 200]
+    L2, C2 = [200, 500, 31, 0], [64, 200, 87, 1]            # same total_q = 352, different ragged structure
+    assert sum(C1) == sum(C2)
+    kid = {"single": P.UPR_KERNEL_SINGLE, "pair": P.UPR_KERNEL_PAIR}[kernel]
+    w1 = S.custom_workload("graph1", 61, L1, C1, 2, 128, 1, self_term=True, n_max=512)
+    w2 = S.custom_workload("graph2", 62, L2, C2, 2, 128, 1, self_term=True, n_max=512)
+    i1, i2 = Inputs(w1, "cuda"), Inputs(w2, "cuda")
+    view = pl.PoolView.of(i1.k_pool.clone(), i1.v_pool.clone(), i1.slot_ids.clone(), w1.seq_lens)
+    view.max_seq_len = 512
+    attn = pl.CrossAttention(view, w1.cand_offsets, P.UPR_BF16, num_splits=2, kernel=kid)
+    q, ks, vs = i1.q.clone(), i1.k_self.clone(), i1.v_self.clone()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        attn(q, ks, vs, stream=side)                        # warm-up outside the capture
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        attn(q, ks, vs, stream=torch.cuda.current_stream())
+    graph.replay()
+    torch.cuda.synchronize()
+    check(attn.out.cpu().numpy(), oracle_all(i1))
+    # new batch in the SAME buffers, replay only
+    q.copy_(i2.q); ks.copy_(i2.k_self); vs.copy_(i2.v_self)
+    view.k_pool.copy_(i2.k_pool); view.v_pool.copy_(i2.v_pool); view.slot_ids.copy_(i2.slot_ids)
+    view.seq_lens.copy_(torch.as_tensor(w2.seq_lens, device="cuda"))
+    attn.cand_offsets.copy_(torch.as_tensor(w2.cand_offsets, device="cuda"))
+    graph.replay()
+    torch.cuda.synchronize()
+    check(attn.out.cpu().numpy(), oracle_all(i2))
+
+
 def test_zero_copy_rejects_bad_arguments(P):
     from paper_2606_00422_b200 import pipeline as pl
     w = S.custom_workload("poolerr", 1, [64, 10], [4, 4], 2, 64, 1, n_max=64)
