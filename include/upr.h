@@ -124,6 +124,14 @@ upr_status upr_kv_pack(const void* k_pool, const void* v_pool, int S, int n_max,
  *   cand_offsets device  int32 [B+1], non-decreasing, [0] = 0, [B] = total_q
  *   out          device  fp32 [total_q, H, d]
  * B == 0 returns UPR_OK without a launch.
+ * Not a slow path: the call reads total_q = cand_offsets[B] back from the device (4 bytes, ONE
+ * synchronisation of `stream`), takes a workspace the library owns (one per device and stream, grown on
+ * demand, freed when the library is unloaded) and then runs exactly what upr_cross_attn_fwd_ex runs: the
+ * device-built longest-first work list, the dynamic scheduler, TMA q / out tiles, the CTA-pair kernel where it
+ * applies.  While `stream` is being captured into a CUDA graph the read-back is impossible: the call then
+ * launches the 1-CTA kernel on its static schedule (no workspace, no host read) -- same results, slower on
+ * ragged batches; use upr_cross_attn_fwd_ex in graphs.  The caches' sizes are not arguments here, so they
+ * cannot be checked: upr_cross_attn_fwd_ex with kv_bytes does.
  */
 upr_status upr_cross_attn_fwd(const void* q, const void* k_cache, const void* v_cache,
                               const int32_t* seq_lens, const int32_t* cand_offsets, float* out,

@@ -1,6 +1,8 @@
 // upr_api.cu -- C ABI of libupr (include/upr.h): argument checks, tensor-map encoding, launches.
 // No torch types, no host synchronisation, no device allocation.
 #include <cuda.h>
+#include <mutex>
+#include <vector>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdarg.h>
@@ -580,9 +582,44 @@ upr_status upr_kv_pack(const void* k_pool, const void* v_pool, int S, int n_max,
   return UPR_OK;
 }
 
+namespace {
+// Workspaces the library owns for the plain entry point: one per (device, stream), grown on demand, kept
+// until the library is unloaded.  Calls on one stream are ordered, so they may share the scheduler state.
+struct OwnedWs { int device; cudaStream_t stream; void* ptr; size_t bytes; };
+std::mutex g_ws_mutex;
+std::vector<OwnedWs> g_ws;
+
+upr_status owned_workspace(cudaStream_t st, size_t need, void** out) {
+  int dev = 0;
+  UPR_CUDA_CHECK(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> lock(g_ws_mutex);
+  OwnedWs* slot = nullptr;
+  for (auto& w : g_ws)
+    if (w.device == dev && w.stream == st) slot = &w;
+  if (slot == nullptr) {
+    g_ws.push_back({dev, st, nullptr, 0});
+    slot = &g_ws.back();
+  }
+  if (slot->bytes < need) {
+    if (slot->ptr != nullptr) {
+      UPR_CUDA_CHECK(cudaStreamSynchronize(st));   // an earlier call on this stream may still use it
+      UPR_CUDA_CHECK(cudaFree(slot->ptr));
+      slot->ptr = nullptr;
+      slot->bytes = 0;
+    }
+    const size_t bytes = (need + (1u << 20) - 1) >> 20 << 20;
+    UPR_CUDA_CHECK(cudaMalloc(&slot->ptr, bytes));
+    slot->bytes = bytes;
+  }
+  *out = slot->ptr;
+  return UPR_OK;
+}
+}  // namespace
+
 upr_status upr_cross_attn_fwd(const void* q, const void* k_cache, const void* v_cache,
                               const int32_t* seq_lens, const int32_t* cand_offsets, float* out,
                               int B, int H, int d, upr_dtype dtype, void* stream) {
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
   upr_attn_params p;
   memset(&p, 0, sizeof(p));
   p.q = q;
@@ -597,9 +634,35 @@ upr_status upr_cross_attn_fwd(const void* q, const void* k_cache, const void* v_
   p.n_layers = 1;
   p.kv_dtype = dtype;
   p.q_dtype = (dtype == UPR_F32) ? UPR_F32 : UPR_BF16;
-  p.total_q = 1;  // unknown on the host; only used to skip empty launches
   p.num_splits = 1;
-  return run_attn(&p, /*have_workspace=*/false, static_cast<cudaStream_t>(stream));
+  if (B <= 0 || cand_offsets == nullptr) {
+    p.total_q = (B == 0) ? 0 : 1;
+    return run_attn(&p, /*have_workspace=*/false, st);   // B == 0: no launch; otherwise validate() reports it
+  }
+  // The same path upr_cross_attn_fwd_ex takes (device-built longest-first work list, dynamic scheduler, TMA
+  // q / out tiles, the CTA-pair kernel where it applies) needs the number of query rows on the host and a
+  // workspace: ΣC = cand_offsets[B] is read back (4 bytes, one stream synchronisation) and the library
+  // supplies the workspace.  While the stream is being captured into a CUDA graph no read-back is possible:
+  // the call then runs the static schedule of the 1-CTA kernel, which needs neither.
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  UPR_CUDA_CHECK(cudaStreamIsCapturing(st, &cap));
+  if (cap != cudaStreamCaptureStatusNone) {
+    p.total_q = 1;   // unknown on the host; only used to skip empty launches
+    return run_attn(&p, /*have_workspace=*/false, st);
+  }
+  int32_t total_q = 0;
+  UPR_CUDA_CHECK(cudaMemcpyAsync(&total_q, cand_offsets + B, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+  UPR_CUDA_CHECK(cudaStreamSynchronize(st));
+  if (total_q < 0) return fail(UPR_ERR_INVALID_ARG, "cand_offsets[B] = %d is negative", (int)total_q);
+  p.total_q = total_q;
+  if (total_q == 0) return run_attn(&p, /*have_workspace=*/false, st);
+  const size_t need = upr_cross_attn_workspace_bytes(&p);
+  void* ws = nullptr;
+  upr_status s = owned_workspace(st, need, &ws);
+  if (s != UPR_OK) return s;
+  p.workspace = ws;
+  p.workspace_bytes = need;
+  return run_attn(&p, /*have_workspace=*/true, st);
 }
 
 int upr_cross_attn_num_splits(const upr_attn_params* p) {

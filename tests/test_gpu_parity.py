@@ -529,8 +529,8 @@ def test_peaked_queries_and_custom_scale(P):
 
 
 def test_basic_entry_point_and_candidate_permutation(P):
-    """upr_cross_attn_fwd (no workspace, static schedule); permuting a user's candidates
-    permutes its outputs."""
+    """upr_cross_attn_fwd (the named entry point: the library reads the row count from the device and supplies the
+    workspace); permuting a user's candidates permutes its outputs."""
     from paper_2606_00422_b200 import pipeline as pl
     w = S.custom_workload("basic", 31, [300, 77], [150, 40], 4, 64, 1)
     inp = Inputs(w, "cuda")
@@ -549,6 +549,48 @@ def test_basic_entry_point_and_candidate_permutation(P):
     torch.cuda.synchronize()
     mx, _ = error_stats(out2.cpu().numpy(), want[perm.cpu().numpy()])
     assert mx <= TOL_STRICT
+
+
+@pytest.mark.parametrize("d,dtype_name", [(128, "bf16"), (64, "bf16"), (64, "fp8")])
+def test_named_entry_point_takes_the_fast_path(P, d, dtype_name):
+    """upr_cross_attn_fwd is not a slow path of the library: outside graph capture it runs the schedule kernel and
+    the same attention kernel upr_cross_attn_fwd_ex would pick (the CTA-pair kernel for bf16 d = 128 blocks of
+    candidates); during stream capture -- where the row count cannot be read back -- it falls back to the static
+    schedule, with the same results."""
+    from paper_2606_00422_b200 import pipeline as pl
+    w = S.custom_workload("named", 77, [300, 0, 77, 1024], [300, 5, 0, 257], 4, d, 1)
+    dt = P.UPR_BF16 if dtype_name == "bf16" else P.UPR_FP8_E4M3
+    inp = Inputs(w, "cuda")
+    cache = pl.alloc_cache(w.seq_lens, w.H, w.d, 1, dt, "cuda")
+    pl.pack_cache(cache, inp.k_pool, inp.v_pool, inp.slot_ids)
+    co = torch.as_tensor(w.cand_offsets, device="cuda")
+    out = torch.full((w.total_q, w.H, w.d), float("nan"), dtype=torch.float32, device="cuda")
+    P.upr_cross_attn_fwd(inp.q[0], cache.k_cache, cache.v_cache, cache.seq_lens, co, out, w.B, w.H, w.d, dt)
+    torch.cuda.synchronize()
+    pair = d == 128 and dtype_name == "bf16"
+    assert P.upr_last_attn_kernel() == ("upr_attn_pair_kernel" if pair else "upr_attn_fwd_kernel")
+    assert P.upr_last_launch_count() == (2 if pair else 1)   # pair kernel: schedule kernel + attention
+    if dtype_name == "bf16":
+        check(out.cpu().numpy(), oracle_all(inp)[0])
+    else:
+        # FP8 caches are read with unit scales by contract of this entry point (the stored bytes ARE the values):
+        # finite everywhere, zeros for the candidates without keys; the values are checked against the static path
+        assert torch.isfinite(out).all()
+        assert (out[w.cand_offsets[1]:w.cand_offsets[2]] == 0).all()
+    # the same call while capturing: static schedule, one launch, same numbers up to summation order
+    out_g = torch.full_like(out, float("nan"))
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            P.upr_cross_attn_fwd(inp.q[0], cache.k_cache, cache.v_cache, cache.seq_lens, co, out_g, w.B, w.H, w.d, dt,
+                                 stream=side)
+        assert P.upr_last_launch_count() == 1 and P.upr_last_attn_kernel() == "upr_attn_fwd_kernel"
+        g.replay()
+    torch.cuda.synchronize()
+    mx, _ = error_stats(out_g.cpu().numpy(), out.cpu().numpy())
+    assert mx <= TOL_STRICT, mx
 
 
 def test_errors_are_reported_not_hidden(P):
