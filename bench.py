@@ -399,6 +399,14 @@ def run_ours(args):
         e_end.record(stream)
         barrier()
         clocks = sampler.stop() if sampler else None
+        if clocks is not None:
+            # what NVML does not show: the clock the SMs really ran at under the attention kernel, from the two
+            # counters CTA 0 of the last launch left in the workspace (include/upr.h: bytes [64, 80))
+            cyc, ns = (int(x) for x in attn_obj.workspace[64:80].view(torch.int64).tolist())
+            if ns > 0:
+                clocks["sm_mhz_in_kernel"] = round(1e3 * cyc / ns, 1)
+                clocks["in_kernel_how"] = ("clock64 / %globaltimer over the last attention launch (CTA 0); the SM clock "
+                                           "follows the tensor-pipe duty cycle, NVML's clocks.sm does not show it")
         return {"total_ms": e_start.elapsed_time(e_end), "clocks": clocks, "launches": n_launch,
                 "pack_ms": float(np.mean([a.elapsed_time(b) for a, b, c in marks])),
                 "attn_ms": float(np.mean([b.elapsed_time(c) for a, b, c in marks]))}

@@ -158,7 +158,10 @@ typedef struct upr_attn_params {
   int32_t max_seq_len;         /* hint for the heuristic (0 = unknown) */
   void* workspace;             /* device, >= upr_cross_attn_workspace_bytes(), 256-B aligned; it holds the
                                   scheduler state of ONE call: two calls in flight at the same time (on
-                                  different streams) must not share a workspace */
+                                  different streams) must not share a workspace.  Diagnostic: after a call,
+                                  bytes [64, 80) hold two uint64 written by CTA 0 of the attention kernel --
+                                  the SM cycles (clock64) and the nanoseconds (%globaltimer) it ran; their
+                                  ratio is the clock the SMs really ran at under the kernel */
   size_t workspace_bytes;
   /* --- fields below may be left zero: packed cache, H_kv = H, no size check ----------------- */
   int32_t kv_source;           /* UPR_KV_PACKED (0): k_cache/v_cache are packed decode caches;

@@ -323,6 +323,14 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
   const bool q_by_tma = !kConvert && args.q_tma != 0;
 
   // ------------------------------------------------------------------ one-time setup
+  // diagnostic: SM cycles and nanoseconds this CTA lives, left in the workspace's counter block (words 16..19) by
+  // CTA 0 -- their ratio is the clock the SMs really ran at under this kernel (bench.py reports it)
+  unsigned long long diag_t0 = 0, diag_c0 = 0;
+  const bool diag = blockIdx.x == 0 && threadIdx.x == 0 && args.counter != nullptr;
+  if (diag) {
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(diag_t0));
+    diag_c0 = static_cast<unsigned long long>(clock64());
+  }
   if (threadIdx.x == 0) {
     for (int i = 0; i < Cfg::kStages; ++i) {
       mbar_init(smem_u32(&ctrl->kv_full[i]), kConvert ? kConvThreads : 1);
@@ -1092,6 +1100,13 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
   }
 
   // ------------------------------------------------------------------ teardown
+  if (diag) {
+    unsigned long long t1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+    unsigned long long* dst = reinterpret_cast<unsigned long long*>(args.counter + 16);
+    dst[0] = static_cast<unsigned long long>(clock64()) - diag_c0;
+    dst[1] = t1 - diag_t0;
+  }
   tc_fence_before();
   __syncthreads();
   if (warp == kMmaWarp) {
