@@ -133,16 +133,16 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
     for (int u = 0; u < U; ++u) {
       if (lh_u[u] < 0) continue;
       if constexpr (MODE == 3) {
-        float wmax = 0.f;
+        // the maximum of bf16 magnitudes is exact in bf16: packed HMNMX2 on the raw pairs, widened once per block
+        __nv_bfloat162 m2a = __float2bfloat162_rn(0.f), m2b = m2a;
 #pragma unroll
         for (int i = 0; i < NI; ++i) {
           const __nv_bfloat162* p2 = reinterpret_cast<const __nv_bfloat162*>(&v[u][i]);
-#pragma unroll
-          for (int k = 0; k < 4; ++k) {
-            const float2 f = __bfloat1622float2(p2[k]);
-            wmax = fmaxf(wmax, fmaxf(fabsf(f.x), fabsf(f.y)));
-          }
+          m2a = __hmax2(m2a, __hmax2(__habs2(p2[0]), __habs2(p2[1])));
+          m2b = __hmax2(m2b, __hmax2(__habs2(p2[2]), __habs2(p2[3])));
         }
+        const float2 mf = __bfloat1622float2(__hmax2(m2a, m2b));
+        const float wmax = fmaxf(mf.x, mf.y);
         if (lh_u[u] != cur_lh) {
           // flush the finished (layer, head): non-negative floats order like their bit patterns
 #pragma unroll
