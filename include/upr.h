@@ -246,6 +246,20 @@ upr_status upr_linear_residual_fwd(const void* x, upr_dtype x_dtype, const void*
 upr_status upr_linear_fp8_fwd(const void* x, float x_scale, const void* w_e4m3, float w_scale, const float* bias,
                               const void* residual, void* y, upr_dtype y_dtype, int64_t M, int N, int K,
                               upr_activation act, void* stream);
+/*
+ * The same layer inside an FP8 CHAIN (MLP up -> down): the activations may arrive as E4M3 bytes and / or leave as
+ * E4M3 bytes, so that between two FP8 layers the tensor crosses HBM once, at one byte per element, and the second
+ * layer's operands both come straight through TMA (no in-kernel quantisation):
+ *   x_dtype UPR_BF16      x device bf16 [M, K], quantised in the kernel with x_scale (as upr_linear_fp8_fwd)
+ *           UPR_FP8_E4M3  x device E4M3 bytes [M, K], real value = dec(byte) * x_scale
+ *   y_dtype UPR_BF16 / UPR_F32  as above (y_scale ignored)
+ *           UPR_FP8_E4M3  y device E4M3 bytes [M, N]:
+ *                         byte = cvt.rn.satfinite.e4m3( fp32(act(...) [+ residual]) * (1.0f / y_scale) )
+ * K % 128 == 0, N % 8 == 0; scales > 0 (else UPR_ERR_INVALID_ARG).
+ */
+upr_status upr_linear_fp8_ex_fwd(const void* x, upr_dtype x_dtype, float x_scale, const void* w_e4m3, float w_scale,
+                                 const float* bias, const void* residual, void* y, upr_dtype y_dtype, float y_scale,
+                                 int64_t M, int N, int K, upr_activation act, void* stream);
 
 /* Layer normalisation of candidate tokens: y = (x - mean) / sqrt(var + eps) * gamma + beta over the
  * hidden dimension; x, y device bf16 [M, D]; gamma, beta device fp32 [D]; D % 8 == 0, D <= 4096. */

@@ -300,3 +300,16 @@ def linear_fp8(x, x_scale: float, w8, w_scale: float, b=None, act: int = ACT_NON
     lib().upro_linear_fp8(_p(x), ctypes.c_float(x_scale), _p(w8), ctypes.c_float(w_scale), _p(bb), ctypes.c_int64(M), N, K,
                           act, _p(y))
     return y
+
+
+def linear_fp8q(x8, x_scale: float, w8, w_scale: float, b=None, act: int = ACT_NONE):
+    """FP8 E4M3 linear layer whose activations arrive as E4M3 bytes: x8 [M,K], w8 [N,K] E4M3 bytes."""
+    x8 = np.ascontiguousarray(x8, dtype=np.uint8)
+    w8 = np.ascontiguousarray(w8, dtype=np.uint8)
+    M, K = x8.shape
+    N = w8.shape[0]
+    bb = _c64(b) if b is not None else None
+    y = np.zeros((M, N), dtype=np.float64)
+    lib().upro_linear_fp8q(_p(x8), ctypes.c_float(x_scale), _p(w8), ctypes.c_float(w_scale), _p(bb), ctypes.c_int64(M), N,
+                           K, act, _p(y))
+    return y

@@ -685,6 +685,30 @@ void upro_layernorm(const double* x, const double* gamma, const double* beta, in
 }
 
 /* ------------------------------------------------------------------------------------
+ * upro_linear_fp8q -- the same layer when the activations ARRIVE as E4M3 bytes (the output
+ * of an FP8 layer before it, quantised there with x_scale, reading Q20):
+ *     y[m,n] = act( x_scale * w_scale * sum_k dec(x8[m,k]) * dec(w8[n,k]) + b[n] )
+ * x8 [M,K], w8 [N,K] E4M3 bytes.  fp64 accumulation (every product of two E4M3 values and
+ * their sums over K <= 2^20 terms are exact in fp64).
+ * ---------------------------------------------------------------------------------- */
+void upro_linear_fp8q(const uint8_t* x8, float x_scale, const uint8_t* w8, float w_scale,
+                      const double* b, int64_t M, int N, int K, int act, double* y) {
+  double s = (double)x_scale * (double)w_scale;
+#pragma omp parallel for schedule(static)
+  for (int64_t m = 0; m < M; ++m)
+    for (int n = 0; n < N; ++n) {
+      double acc = 0.0;
+      for (int k = 0; k < K; ++k)
+        acc += upro_e4m3_decode(x8[m * K + k]) * upro_e4m3_decode(w8[(int64_t)n * K + k]);
+      acc *= s;
+      if (b) acc += b[n];
+      if (act == 1) acc = acc / (1.0 + exp(-acc));
+      else if (act == 2) acc = acc > 0.0 ? acc : 0.0;
+      y[m * N + n] = acc;
+    }
+}
+
+/* ------------------------------------------------------------------------------------
  * upro_linear_fp8 -- a linear layer with FP8 E4M3 operands and fused per-tensor scaling
  * (FP8 forward in E4M3; reading Q20):
  *     q(x)   = e4m3_rne_satfinite( x * (1.0f / x_scale) )      product rounded once in fp32

@@ -15,7 +15,7 @@ UPR_ROW_ALIGN, UPR_TAIL_ROWS = 16, 128
 EXPORTED_SYMBOLS = [
     "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
     "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
-    "upr_last_error", "upr_version", "upr_last_attn_kernel",
+    "upr_last_error", "upr_version", "upr_last_attn_kernel", "upr_linear_fp8_ex_fwd",
     "upr_linear_fwd", "upr_linear_residual_fwd", "upr_linear_fp8_fwd", "upr_layernorm_fwd", "upr_kv_project_into_pool", "upr_action_utility", "upr_topk_per_user",
     "upr_pool_export", "upr_pool_open", "upr_pool_close", "upr_slot_ring_init", "upr_slot_ring_acquire",
 ]
@@ -104,6 +104,11 @@ def _load() -> ctypes.CDLL:
         lib.upr_linear_fp8_fwd.argtypes = [ctypes.c_void_p, ctypes.c_float, ctypes.c_void_p, ctypes.c_float, ctypes.c_void_p,
                                            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_int,
                                            ctypes.c_int, ctypes.c_int, ctypes.c_void_p]
+        lib.upr_linear_fp8_ex_fwd.restype = ctypes.c_int
+        lib.upr_linear_fp8_ex_fwd.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_void_p, ctypes.c_float,
+                                              ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
+                                              ctypes.c_float, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                              ctypes.c_void_p]
         lib.upr_layernorm_fwd.restype = ctypes.c_int
         lib.upr_layernorm_fwd.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
                                           ctypes.c_int, ctypes.c_float, ctypes.c_void_p]
@@ -259,6 +264,18 @@ def upr_linear_fp8_fwd(x, x_scale: float, w8, w_scale: float, bias, residual, y,
     N = int(w8.shape[0])
     _check(_load().upr_linear_fp8_fwd(_ptr(x), x_scale, _ptr(w8), w_scale, _ptr(bias), _ptr(residual), _ptr(y),
                                       _DT[y.dtype], M, N, K, act, _stream(stream)))
+
+
+def upr_linear_fp8_ex_fwd(x, x_scale: float, w8, w_scale: float, bias, residual, y, y_scale: float = 1.0,
+                          act: int = UPR_ACT_NONE, stream=None) -> None:
+    """FP8 E4M3 linear inside a chain: x bf16 [M,K] (quantised in-kernel) or uint8 E4M3 bytes; y bf16 / fp32 or
+    uint8 E4M3 bytes (quantised with y_scale)."""
+    M, K = int(x.shape[0]), int(x.shape[1])
+    N = int(w8.shape[0])
+    xd = UPR_FP8_E4M3 if x.dtype == torch.uint8 else _DT[x.dtype]
+    yd = UPR_FP8_E4M3 if y.dtype == torch.uint8 else _DT[y.dtype]
+    _check(_load().upr_linear_fp8_ex_fwd(_ptr(x), xd, x_scale, _ptr(w8), w_scale, _ptr(bias), _ptr(residual), _ptr(y),
+                                         yd, y_scale, M, N, K, act, _stream(stream)))
 
 
 def upr_layernorm_fwd(x, gamma, beta, y, eps: float = 1e-5, stream=None) -> None:

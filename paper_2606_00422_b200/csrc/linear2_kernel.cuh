@@ -33,14 +33,17 @@ constexpr int kTileBytes = 128 * kBK * 2;       // 16 KB: one CTA's x tile or W 
 constexpr int kRawBytes = 128 * kBK * 4;        // 32 KB: one CTA's fp32 x tile as loaded
 constexpr int kConvThreads = 128;               // warps 2, 3, 8, 9
 
-enum : int { MODE_BF16 = 0, MODE_XF32 = 1, MODE_FP8 = 2 };   // operands: bf16 x bf16; fp32 x converted; e4m3 x e4m3 (x quantised in-kernel)
+// operands: bf16 x bf16; fp32 x converted to bf16; e4m3 x e4m3 with bf16 x quantised in-kernel; e4m3 x e4m3 with x
+// already e4m3 in memory (the output of an FP8 layer before it: both operands come straight through TMA)
+enum : int { MODE_BF16 = 0, MODE_XF32 = 1, MODE_FP8 = 2, MODE_FP8Q = 3 };
 
 template <int MODE>
 struct Cfg {
-  static constexpr bool kConv = MODE != MODE_BF16;
+  static constexpr bool kConv = MODE == MODE_XF32 || MODE == MODE_FP8;
+  static constexpr bool kF8 = MODE == MODE_FP8 || MODE == MODE_FP8Q;
   static constexpr int kStages = kConv ? 4 : 6;
   static constexpr int kRawStages = kConv ? 2 : 0;
-  static constexpr int kKStep = (MODE == MODE_FP8) ? 128 : 64;   // elements of K per stage: one 128-byte row per operand row
+  static constexpr int kKStep = kF8 ? 128 : 64;   // elements of K per stage: one 128-byte row per operand row
   static constexpr int kSmemCtrl = 1024;
   static constexpr int kSmemTotal = kStages * 2 * kTileBytes + kRawStages * kRawBytes + kSmemCtrl + 1024;
   static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
@@ -131,8 +134,8 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
             ++raw_it;
           } else {
             if (leader) mbar_arrive_expect_tx(smem_u32(&ctrl->full[s]), 4 * kTileBytes);
-            tma_load_2d_pair(a_smem + s * kTileBytes, &tmap_x, ks * kBK, xrow, full);
-            tma_load_2d_pair(b_smem + s * kTileBytes, &tmap_w, ks * kBK, wrow, full);
+            tma_load_2d_pair(a_smem + s * kTileBytes, &tmap_x, ks * C::kKStep, xrow, full);
+            tma_load_2d_pair(b_smem + s * kTileBytes, &tmap_w, ks * C::kKStep, wrow, full);
           }
         }
       }
@@ -144,7 +147,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
       if (elect_one()) {
         constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);   // SBO 1024, version 1, SWIZZLE_128B
         constexpr uint32_t kLoK = (16u >> 4) << 16;
-        constexpr uint32_t kIdesc = (MODE == MODE_FP8) ? make_idesc_e4m3(kBM, kBN) : make_idesc_bf16(kBM, kBN, 0, 0);
+        constexpr uint32_t kIdesc = C::kF8 ? make_idesc_e4m3(kBM, kBN) : make_idesc_bf16(kBM, kBN, 0, 0);
         auto mk_desc = [](uint32_t lo) {
           return (static_cast<uint64_t>(kDescHi) << 32) | static_cast<uint64_t>(lo);
         };
@@ -163,7 +166,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
             for (int k = 0; k < 4; ++k) {   // 32 bytes of K per instruction: 16 bf16 or 32 e4m3 elements
               const uint64_t da = mk_desc(a_lo + ((s * kTileBytes + k * 32) >> 4));
               const uint64_t db = mk_desc(b_lo + ((s * kTileBytes + k * 32) >> 4));
-              if (MODE == MODE_FP8) umma_ss_pair_f8(tmem_base + ab * kBN, da, db, kIdesc, (ks > 0 || k > 0) ? 1u : 0u);
+              if (C::kF8) umma_ss_pair_f8(tmem_base + ab * kBN, da, db, kIdesc, (ks > 0 || k > 0) ? 1u : 0u);
               else umma_ss_pair(tmem_base + ab * kBN, da, db, kIdesc, (ks > 0 || k > 0) ? 1u : 0u);
             }
             umma_commit_pair(smem_u32(&ctrl->empty[s]));
@@ -269,7 +272,7 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
           float v[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k) v[k] = __uint_as_float(r[c + k]);
-          if (MODE == MODE_FP8) {
+          if (C::kF8) {
 #pragma unroll
             for (int k = 0; k < 8; ++k) v[k] *= args.out_scale;
           }
@@ -301,6 +304,17 @@ upr_linear_pair_kernel(const __grid_constant__ CUtensorMap tmap_x,   // box 128 
                                  (kv_row0 + static_cast<long long>(h) * args.kv_n) * args.kv_d + tt;
             *reinterpret_cast<uint4*>(dst) = make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]),
                                                         pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7]));
+          } else if (C::kF8 && args.y_is_fp8) {
+            // the next FP8 layer's operand: byte = cvt.rn.satfinite.e4m3(value * y_mult), product rounded once in fp32
+            uint32_t o[2];
+#pragma unroll
+            for (int k = 0; k < 2; ++k)
+              o[k] = static_cast<uint32_t>(__nv_cvt_float2_to_fp8x2(
+                         make_float2(v[4 * k] * args.y_mult, v[4 * k + 1] * args.y_mult), __NV_SATFINITE, __NV_E4M3)) |
+                     (static_cast<uint32_t>(__nv_cvt_float2_to_fp8x2(
+                          make_float2(v[4 * k + 2] * args.y_mult, v[4 * k + 3] * args.y_mult), __NV_SATFINITE, __NV_E4M3))
+                      << 16);
+            *reinterpret_cast<uint2*>(static_cast<uint8_t*>(args.y) + row * args.N + col0 + c) = make_uint2(o[0], o[1]);
           } else if (args.y_is_f32) {
             float* dst = static_cast<float*>(args.y) + row * args.N + col0 + c;
             *reinterpret_cast<float4*>(dst) = make_float4(v[0], v[1], v[2], v[3]);

@@ -49,6 +49,8 @@ struct Args {
   int y_is_f32;
   float out_scale;        // multiplies the accumulator before the bias (FP8 operands: x_scale * w_scale; else 1)
   float x_mult;           // FP8 operands: x is quantised as e4m3(x * x_mult), x_mult = 1 / x_scale
+  int y_is_fp8;           // pair kernel only: y is e4m3 [M, N], byte = cvt.rn.satfinite.e4m3(value * y_mult)
+  float y_mult;           // 1 / y_scale
   // K/V projection written straight into the pool layout [layers, S, H, n, d]: row m of y is token
   // m's [H, d] vector and goes to pool[layer, tok_slot[m], h, tok_pos[m], :]; y = the pool (bf16), N = H * d
   const int32_t* tok_slot;

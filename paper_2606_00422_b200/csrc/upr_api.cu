@@ -690,7 +690,7 @@ upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream) {
 // ------------------------------------------------------------------ decode-layer tail, consumer, pool
 namespace {
 struct KvScatter { const int32_t* tok_slot; const int32_t* tok_pos; int layer, S, H, n, d; const void* residual;
-                   int fp8; float x_scale, w_scale; };
+                   int fp8; float x_scale, w_scale; float y_scale = 1.f; };
 }  // namespace
 
 static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* y,
@@ -698,15 +698,20 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
                               void* stream) {
   g_launches = 0;
   if (M < 0 || N <= 0 || K <= 0) return fail(UPR_ERR_INVALID_ARG, "bad sizes M=%lld N=%d K=%d", (long long)M, N, K);
-  if (x_dtype != UPR_BF16 && x_dtype != UPR_F32) return fail(UPR_ERR_UNSUPPORTED, "x_dtype %d (bf16 or f32)", (int)x_dtype);
-  if (y_dtype != UPR_BF16 && y_dtype != UPR_F32) return fail(UPR_ERR_UNSUPPORTED, "y_dtype %d (bf16 or f32)", (int)y_dtype);
+  const bool fp8 = kv != nullptr && kv->fp8;
+  const bool xq = fp8 && x_dtype == UPR_FP8_E4M3;   // x already e4m3 in memory
+  const bool yq = fp8 && y_dtype == UPR_FP8_E4M3;   // y leaves as e4m3
+  if (x_dtype != UPR_BF16 && x_dtype != UPR_F32 && !xq)
+    return fail(UPR_ERR_UNSUPPORTED, "x_dtype %d (bf16 or f32; e4m3 for FP8 layers)", (int)x_dtype);
+  if (y_dtype != UPR_BF16 && y_dtype != UPR_F32 && !yq)
+    return fail(UPR_ERR_UNSUPPORTED, "y_dtype %d (bf16 or f32; e4m3 for FP8 layers)", (int)y_dtype);
   if (act != UPR_ACT_NONE && act != UPR_ACT_SILU && act != UPR_ACT_RELU)
     return fail(UPR_ERR_INVALID_ARG, "activation %d unknown", (int)act);
-  const bool fp8 = kv != nullptr && kv->fp8;
   if (K % (fp8 ? 128 : 64) != 0 || N % 8 != 0)
     return fail(UPR_ERR_UNSUPPORTED, "K=%d must be a multiple of %d, N=%d of 8", K, fp8 ? 128 : 64, N);
-  if (fp8 && x_dtype != UPR_BF16) return fail(UPR_ERR_UNSUPPORTED, "FP8 linear layers take bf16 activations");
-  if (fp8 && (!(kv->x_scale > 0.f) || !(kv->w_scale > 0.f))) return fail(UPR_ERR_INVALID_ARG, "scales must be > 0");
+  if (fp8 && x_dtype == UPR_F32) return fail(UPR_ERR_UNSUPPORTED, "FP8 linear layers take bf16 or e4m3 activations");
+  if (fp8 && (!(kv->x_scale > 0.f) || !(kv->w_scale > 0.f) || (yq && !(kv->y_scale > 0.f))))
+    return fail(UPR_ERR_INVALID_ARG, "scales must be > 0");
   if (M == 0) return UPR_OK;
   if (!x || !w || !y) return fail(UPR_ERR_INVALID_ARG, "NULL tensor pointer");
   if ((reinterpret_cast<uintptr_t>(x) & 15) || (reinterpret_cast<uintptr_t>(w) & 15) || (reinterpret_cast<uintptr_t>(y) & 15))
@@ -721,10 +726,11 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   {
     const bool f32 = x_dtype == UPR_F32;
     cuuint64_t gdim[2] = {static_cast<cuuint64_t>(K), static_cast<cuuint64_t>(M)};
-    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(K) * (f32 ? 4 : 2)};
-    if (enc(&tx, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(x),
+    cuuint64_t gstride[1] = {static_cast<cuuint64_t>(K) * (f32 ? 4 : xq ? 1 : 2)};
+    if (enc(&tx, f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : xq ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16,
+            2, const_cast<void*>(x),
             gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-            (f32 || fp8) ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+            (f32 || (fp8 && !xq)) ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for x");
   }
@@ -758,6 +764,8 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   a.y_is_f32 = y_dtype == UPR_F32;
   a.out_scale = fp8 ? kv->x_scale * kv->w_scale : 1.0f;
   a.x_mult = fp8 ? 1.0f / kv->x_scale : 1.0f;
+  a.y_is_fp8 = yq ? 1 : 0;
+  a.y_mult = yq ? 1.0f / kv->y_scale : 1.0f;
   int sms = sm_count();
   if (sms <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
   cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -767,7 +775,12 @@ static upr_status linear_impl(const void* x, upr_dtype x_dtype, const void* w, c
   if (fp8 || (N > 128 && tiles2 >= sms / 2)) {
     int pairs = sms / 2;
     if (tiles2 < pairs) pairs = static_cast<int>(tiles2);
-    if (fp8) {
+    if (xq) {
+      using C = upr::lin2::Cfg<upr::lin2::MODE_FP8Q>;
+      UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_FP8Q>,
+                                          cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemTotal));
+      upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_FP8Q><<<2 * pairs, upr::lin2::kThreads, C::kSmemTotal, st>>>(tx, tw, a);
+    } else if (fp8) {
       using C = upr::lin2::Cfg<upr::lin2::MODE_FP8>;
       UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::lin2::upr_linear_pair_kernel<upr::lin2::MODE_FP8>,
                                           cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemTotal));
@@ -825,6 +838,17 @@ upr_status upr_linear_fp8_fwd(const void* x, float x_scale, const void* w_e4m3, 
     return fail(UPR_ERR_INVALID_ARG, "residual must be 16-byte aligned");
   KvScatter kv{nullptr, nullptr, 0, 0, 0, 0, 0, residual, 1, x_scale, w_scale};
   return linear_impl(x, UPR_BF16, w_e4m3, bias, y, y_dtype, M, N, K, act, &kv, stream);
+}
+
+upr_status upr_linear_fp8_ex_fwd(const void* x, upr_dtype x_dtype, float x_scale, const void* w_e4m3, float w_scale,
+                                 const float* bias, const void* residual, void* y, upr_dtype y_dtype, float y_scale,
+                                 int64_t M, int N, int K, upr_activation act, void* stream) {
+  if (residual != nullptr && (reinterpret_cast<uintptr_t>(residual) & 15))
+    return fail(UPR_ERR_INVALID_ARG, "residual must be 16-byte aligned");
+  if (x_dtype != UPR_BF16 && x_dtype != UPR_FP8_E4M3)
+    return fail(UPR_ERR_UNSUPPORTED, "x_dtype %d (bf16 or e4m3)", (int)x_dtype);
+  KvScatter kv{nullptr, nullptr, 0, 0, 0, 0, 0, residual, 1, x_scale, w_scale, y_scale};
+  return linear_impl(x, x_dtype, w_e4m3, bias, y, y_dtype, M, N, K, act, &kv, stream);
 }
 
 upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,

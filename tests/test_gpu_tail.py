@@ -280,6 +280,50 @@ def test_linear_fp8_matches_oracle(P, shape):
     assert err <= 2e-4 * max(1.0, np.abs(want).max())
 
 
+
+def test_fp8_chain_keeps_the_hidden_tensor_in_e4m3(P):
+    """MLP up -> down as an FP8 chain (upr_linear_fp8_ex_fwd): the first layer leaves E4M3 bytes, the second reads
+    them through TMA.  Layer 1's bytes: the quantisation decision is taken on the GPU's own fp32 value, the oracle's
+    on its fp64 value rounded to fp32 -- codes may differ where a value sits on a rounding boundary, by one E4M3 step
+    at most, for a small fraction.  Layer 2 is checked against the oracle fed the GPU's OWN bytes (same operands)."""
+    M, D, F = 1500, 256, 1024
+    dev = "cuda"
+    x = S.normal_bf16(91, "x", (M, D), dev)
+    w1f = S.normal_bf16(92, "w1", (F, D), dev).float() / np.sqrt(D)
+    w2f = S.normal_bf16(93, "w2", (D, F), dev).float() / np.sqrt(F)
+    q8 = lambda wf, sc: (wf * (np.float32(1.0) / np.float32(sc))).to(torch.float8_e4m3fn).view(torch.uint8)
+    x_scale = float(np.float32(4.5) / np.float32(448.0))
+    w1_scale = float(np.float32(w1f.abs().max().item()) / np.float32(448.0))
+    w2_scale = float(np.float32(w2f.abs().max().item()) / np.float32(448.0))
+    h_scale = float(np.float32(6.0) / np.float32(448.0))           # SiLU outputs of unit-variance pre-activations
+    w1, w2 = q8(w1f, w1_scale), q8(w2f, w2_scale)
+    b1 = S.normal_bf16(94, "b1", (F,), dev).float() * 0.2
+    b2 = S.normal_bf16(95, "b2", (D,), dev).float() * 0.2
+    h8 = torch.empty((M, F), dtype=torch.uint8, device=dev)
+    y = torch.empty((M, D), dtype=torch.bfloat16, device=dev)
+    P.upr_linear_fp8_ex_fwd(x, x_scale, w1, w1_scale, b1, None, h8, h_scale, P.UPR_ACT_SILU)
+    assert P.upr_last_launch_count() == 1
+    P.upr_linear_fp8_ex_fwd(h8, h_scale, w2, w2_scale, b2, x, y, 1.0, P.UPR_ACT_NONE)
+    torch.cuda.synchronize()
+    # layer 1
+    h_want = oracle.linear_fp8(x.float().cpu().numpy(), x_scale, w1.cpu().numpy(), w1_scale, f64(b1), act=oracle.ACT_SILU)
+    code_want = oracle.e4m3_encode((h_want.astype(np.float32) * (np.float32(1.0) / np.float32(h_scale))).astype(np.float32))
+    got8 = h8.cpu().numpy()
+    differ = got8 != code_want
+    dec_g, dec_w = oracle.e4m3_decode(got8), oracle.e4m3_decode(code_want)
+    step = np.maximum(np.abs(dec_w), 2.0 ** -6) * 2.0 ** -3        # one E4M3 step at that magnitude (3 mantissa bits)
+    assert differ.mean() < 5e-3, differ.mean()
+    assert (np.abs(dec_g - dec_w) <= step + 1e-12).all()
+    print(f"fp8 chain: {differ.mean():.2e} of layer-1 codes differ (all by <= one step)")
+    # layer 2 on the GPU's bytes
+    y_want = oracle.linear_fp8q(got8, h_scale, w2.cpu().numpy(), w2_scale, f64(b2)) + f64(x)
+    err = np.abs(f64(y) - y_want).max()
+    assert err <= 2.0 ** -8 * max(1.0, np.abs(y_want).max()) + 2e-4, err     # bf16 output rounding
+    # errors are reported, not hidden
+    with pytest.raises(P.UprError):
+        P.upr_linear_fp8_ex_fwd(h8, 0.0, w2, w2_scale, b2, None, y, 1.0)
+
+
 def test_action_heads_and_utility_match_oracle(P):
     """z -> [stacked first layers of the C heads, SiLU] (tcgen05 GEMM) -> logits -> sigmoid -> utility."""
     dev = "cuda"

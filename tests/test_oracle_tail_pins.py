@@ -173,3 +173,26 @@ def test_linear_fp8_against_torch_float8_and_the_exact_case(oracle):
     np.testing.assert_array_equal(oracle.linear_fp8(xi, 1.0, wi8, 1.0), oracle.linear(xi, wi))
     # scales factor out: y(x, 2 x_scale) with x doubled == 2 y
     np.testing.assert_allclose(oracle.linear_fp8(2 * xi, 2.0, wi8, 1.0), 2 * oracle.linear(xi, wi), rtol=0, atol=1e-12)
+
+
+def test_linear_fp8q_is_the_plain_layer_on_decoded_bytes(oracle):
+    """Activations that arrive as E4M3 bytes: pinned to torch's float8 decode + a float64 matmul (library routines), to
+    upro_linear_fp8 on the decoded values (quantising a representable value is the identity), and to the exact
+    integer case."""
+    r = rng(9)
+    M, N, K = 6, 5, 64
+    x8 = r.integers(0, 256, size=(M, K)).astype(np.uint8)
+    w8 = r.integers(0, 256, size=(N, K)).astype(np.uint8)
+    x8[(x8 & 0x7F) == 0x7F] = 0x38          # no NaN codes
+    w8[(w8 & 0x7F) == 0x7F] = 0xB8
+    b = r.standard_normal(N)
+    xs, ws = 0.25, 0.03125
+    got = oracle.linear_fp8q(x8, xs, w8, ws, b, act=oracle.ACT_RELU)
+    xd = torch.from_numpy(x8).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+    wd = torch.from_numpy(w8).view(torch.float8_e4m3fn).to(torch.float64).numpy()
+    np.testing.assert_allclose(got, np.maximum((xd @ wd.T) * xs * ws + b, 0.0), rtol=0, atol=1e-9)
+    # the in-kernel-quantising layer fed the decoded values (scale 1: x * 1.0f is exact, encode(decode(b)) == b)
+    np.testing.assert_array_equal(oracle.linear_fp8q(x8, 1.0, w8, ws, b), oracle.linear_fp8(xd.astype(np.float32), 1.0, w8, ws, b))
+    xi = r.integers(-8, 9, size=(M, K)).astype(np.float32)
+    wi = r.integers(-8, 9, size=(N, K)).astype(np.float32)
+    np.testing.assert_array_equal(oracle.linear_fp8q(oracle.e4m3_encode(xi), 1.0, oracle.e4m3_encode(wi), 1.0), oracle.linear(xi, wi))
