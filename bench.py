@@ -314,13 +314,42 @@ def decode_layer_leg(P, pl, w, k_pool, v_pool, slots, stream, dev, ev, hidden_mu
     up_bf16 = time_it(lambda: P.upr_linear_fwd(layer.h2, prm["w1"], prm["b1"], layer.u, P.UPR_ACT_SILU, stream))
     up_fp8 = time_it(lambda: P.upr_linear_fp8_fwd(layer.h2, 6.0 / 448.0, w1_8, w_scale, prm["b1"], None, layer.u,
                                                   P.UPR_ACT_SILU, stream))
+    # the whole MLP as an FP8 chain: up-projection leaves E4M3 bytes, the down-projection reads them through TMA
+    w2f = prm["w2"].float()
+    w2_scale = float(w2f.abs().max().item()) / 448.0
+    w2_8 = (w2f / w2_scale).to(torch.float8_e4m3fn).view(torch.uint8)
+    u8 = torch.empty((M, hidden), dtype=torch.uint8, device=dev)
+    y8 = torch.empty((M, D), dtype=torch.bfloat16, device=dev)
+
+    def mlp_fp8_chain():
+        P.upr_linear_fp8_ex_fwd(layer.h2, 6.0 / 448.0, w1_8, w_scale, prm["b1"], None, u8, 6.0 / 448.0, P.UPR_ACT_SILU, stream)
+        P.upr_linear_fp8_ex_fwd(u8, 6.0 / 448.0, w2_8, w2_scale, prm["b2"], x, y8, 1.0, P.UPR_ACT_NONE, stream)
+
+    def mlp_bf16():
+        P.upr_linear_fwd(layer.h2, prm["w1"], prm["b1"], layer.u, P.UPR_ACT_SILU, stream)
+        P.upr_linear_residual_fwd(layer.u, prm["w2"], prm["b2"], x, y8, P.UPR_ACT_NONE, stream)
+    mlp_chain_ms = time_it(mlp_fp8_chain)
+    mlp_bf16_ms = time_it(mlp_bf16)
+    down_fp8q = time_it(lambda: P.upr_linear_fp8_ex_fwd(u8, 6.0 / 448.0, w2_8, w2_scale, prm["b2"], x, y8, 1.0,
+                                                        P.UPR_ACT_NONE, stream))
+    # the whole decode layer with the MLP as an FP8 chain (LN2 -> E4M3, up -> E4M3, down -> bf16 + residual),
+    # timed alternately with the bf16 layer so that both see the same clocks
+    layer8 = pl.RankingDecodeLayer(attn1, D, hidden, prm, fp8_mlp={
+        "w1_8": w1_8, "w1_scale": w_scale, "w2_8": w2_8, "w2_scale": w2_scale, "h_scale": 5.0 / 448.0, "u_scale": 6.0 / 448.0})
+    ms8 = min(time_it(lambda: layer8(x, stream=stream)) for _ in range(2))
+    ms16 = time_it(lambda: layer(x, stream=stream))
     fl_up = 2.0 * M * D * hidden
     gemm_flops = 2.0 * M * D * (4 * D + 2 * hidden)
     attn_flops = (w.flops / w.n_layers) + 4.0 * w.d * M * w.H      # one layer's pairs + the self pair
     return {"ms": ms, "candidates_per_s": M / (ms * 1e-3), "launches": layer.launches, "D_model": D, "mlp_hidden": hidden,
             "gemm_flops": gemm_flops, "attn_flops": attn_flops, "tflops": (gemm_flops + attn_flops) / (ms * 1e-3) / 1e12,
             "mlp_up_bf16_ms": up_bf16, "mlp_up_bf16_tflops": fl_up / (up_bf16 * 1e-3) / 1e12,
-            "mlp_up_fp8_ms": up_fp8, "mlp_up_fp8_tflops": fl_up / (up_fp8 * 1e-3) / 1e12}
+            "mlp_up_fp8_ms": up_fp8, "mlp_up_fp8_tflops": fl_up / (up_fp8 * 1e-3) / 1e12,
+            "mlp_down_fp8_e4m3_in_ms": down_fp8q, "mlp_down_fp8_e4m3_in_tflops": fl_up / (down_fp8q * 1e-3) / 1e12,
+            "mlp_bf16_ms": mlp_bf16_ms, "mlp_bf16_tflops": 2 * fl_up / (mlp_bf16_ms * 1e-3) / 1e12,
+            "mlp_fp8_chain_ms": mlp_chain_ms, "mlp_fp8_chain_tflops": 2 * fl_up / (mlp_chain_ms * 1e-3) / 1e12,
+            "fp8_mlp_layer_ms": ms8, "bf16_layer_again_ms": ms16, "fp8_mlp_layer_candidates_per_s": M / (ms8 * 1e-3),
+            "fp8_mlp_layer_tflops": (gemm_flops + attn_flops) / (ms8 * 1e-3) / 1e12}
 
 
 # ----------------------------------------------------------------------------- CUDA arm

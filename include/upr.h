@@ -265,6 +265,10 @@ upr_status upr_linear_fp8_ex_fwd(const void* x, upr_dtype x_dtype, float x_scale
  * hidden dimension; x, y device bf16 [M, D]; gamma, beta device fp32 [D]; D % 8 == 0, D <= 4096. */
 upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,
                              float eps, void* stream);
+/* The same with the output quantised for an FP8 layer: y_e4m3 device E4M3 bytes [M, D],
+ * byte = cvt.rn.satfinite.e4m3( fp32(layer-norm value) * (1.0f / y_scale) ), y_scale > 0. */
+upr_status upr_layernorm_fp8_fwd(const void* x, const float* gamma, const float* beta, void* y_e4m3, float y_scale,
+                                 int64_t M, int D, float eps, void* stream);
 
 /*
  * Prefill into the layout: the K (or V) projection of M history tokens written straight into

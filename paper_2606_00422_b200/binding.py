@@ -15,7 +15,7 @@ UPR_ROW_ALIGN, UPR_TAIL_ROWS = 16, 128
 EXPORTED_SYMBOLS = [
     "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
     "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
-    "upr_last_error", "upr_version", "upr_last_attn_kernel", "upr_linear_fp8_ex_fwd",
+    "upr_last_error", "upr_version", "upr_last_attn_kernel", "upr_linear_fp8_ex_fwd", "upr_layernorm_fp8_fwd",
     "upr_linear_fwd", "upr_linear_residual_fwd", "upr_linear_fp8_fwd", "upr_layernorm_fwd", "upr_kv_project_into_pool", "upr_action_utility", "upr_topk_per_user",
     "upr_pool_export", "upr_pool_open", "upr_pool_close", "upr_slot_ring_init", "upr_slot_ring_acquire",
 ]
@@ -112,6 +112,9 @@ def _load() -> ctypes.CDLL:
         lib.upr_layernorm_fwd.restype = ctypes.c_int
         lib.upr_layernorm_fwd.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64,
                                           ctypes.c_int, ctypes.c_float, ctypes.c_void_p]
+        lib.upr_layernorm_fp8_fwd.restype = ctypes.c_int
+        lib.upr_layernorm_fp8_fwd.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_float,
+                                              ctypes.c_int64, ctypes.c_int, ctypes.c_float, ctypes.c_void_p]
         lib.upr_kv_project_into_pool.restype = ctypes.c_int
         lib.upr_kv_project_into_pool.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p,
                                                  ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64] + \
@@ -282,6 +285,12 @@ def upr_layernorm_fwd(x, gamma, beta, y, eps: float = 1e-5, stream=None) -> None
     """x, y bf16 [M, D]; gamma, beta fp32 [D]."""
     _check(_load().upr_layernorm_fwd(_ptr(x), _ptr(gamma), _ptr(beta), _ptr(y), int(x.shape[0]), int(x.shape[1]), eps,
                                      _stream(stream)))
+
+
+def upr_layernorm_fp8_fwd(x, gamma, beta, y8, y_scale: float, eps: float = 1e-5, stream=None) -> None:
+    """x bf16 [M, D]; y8 uint8 E4M3 bytes [M, D] quantised with y_scale; gamma, beta fp32 [D]."""
+    _check(_load().upr_layernorm_fp8_fwd(_ptr(x), _ptr(gamma), _ptr(beta), _ptr(y8), y_scale, int(x.shape[0]),
+                                         int(x.shape[1]), eps, _stream(stream)))
 
 
 def upr_kv_project_into_pool(x, w, bias, pool, tok_slot, tok_pos, layer: int, stream=None) -> None:

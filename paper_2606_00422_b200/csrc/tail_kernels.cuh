@@ -102,10 +102,13 @@ __global__ void __launch_bounds__(kTopkThreads) upr_topk_kernel(const float* __r
 // statistics, two passes over registers (D <= 4096, D % 8 == 0): one warp per row, 16-byte loads.  HBM-bound.
 constexpr int kLnMaxChunks = 16;   // 16-byte chunks per lane: D <= 32 * 8 * 16 = 4096
 
+// Y_FP8: the output leaves as E4M3 bytes, byte = cvt.rn.satfinite.e4m3(value * y_mult) -- the operand of an FP8
+// linear layer (upr_linear_fp8_ex_fwd with x_dtype = UPR_FP8_E4M3), one byte per element instead of two.
+template <bool Y_FP8>
 __global__ void __launch_bounds__(256) upr_layernorm_kernel(const __nv_bfloat16* __restrict__ x,
                                                             const float* __restrict__ gamma,
                                                             const float* __restrict__ beta, long long M, int D,
-                                                            float eps, __nv_bfloat16* __restrict__ y) {
+                                                            float eps, void* __restrict__ y_out, float y_mult) {
   const int lane = threadIdx.x & 31;
   const long long warp0 = (static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
   const long long n_warps = (static_cast<long long>(gridDim.x) * blockDim.x) >> 5;
@@ -144,7 +147,8 @@ __global__ void __launch_bounds__(256) upr_layernorm_kernel(const __nv_bfloat16*
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
     const float rstd = rsqrtf(sq / static_cast<float>(D) + eps);
-    uint4* dst = reinterpret_cast<uint4*>(y + m * D);
+    uint4* dst = reinterpret_cast<uint4*>(static_cast<__nv_bfloat16*>(y_out) + m * D);
+    uint2* dst8 = reinterpret_cast<uint2*>(static_cast<uint8_t*>(y_out) + m * D);
 #pragma unroll
     for (int i = 0; i < kLnMaxChunks; ++i) {
       const int c = i * 32 + lane;
@@ -160,9 +164,13 @@ __global__ void __launch_bounds__(256) upr_layernorm_kernel(const __nv_bfloat16*
         for (int k = 0; k < 4; ++k) {
           const float lo = fmaf((v[i][2 * k] - mean) * rstd, g[2 * k], b[2 * k]);
           const float hi = fmaf((v[i][2 * k + 1] - mean) * rstd, g[2 * k + 1], b[2 * k + 1]);
-          o[k] = pack_bf16x2(lo, hi);
+          if (Y_FP8)
+            o[k] = __nv_cvt_float2_to_fp8x2(make_float2(lo * y_mult, hi * y_mult), __NV_SATFINITE, __NV_E4M3);
+          else
+            o[k] = pack_bf16x2(lo, hi);
         }
-        dst[c] = make_uint4(o[0], o[1], o[2], o[3]);
+        if (Y_FP8) dst8[c] = make_uint2(o[0] | (o[1] << 16), o[2] | (o[3] << 16));
+        else dst[c] = make_uint4(o[0], o[1], o[2], o[3]);
       }
     }
   }

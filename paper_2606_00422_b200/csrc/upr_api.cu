@@ -851,22 +851,38 @@ upr_status upr_linear_fp8_ex_fwd(const void* x, upr_dtype x_dtype, float x_scale
   return linear_impl(x, x_dtype, w_e4m3, bias, y, y_dtype, M, N, K, act, &kv, stream);
 }
 
-upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,
-                             float eps, void* stream) {
+static upr_status layernorm_impl(const void* x, const float* gamma, const float* beta, void* y, bool y_fp8, float y_scale,
+                                 int64_t M, int D, float eps, void* stream) {
   g_launches = 0;
   if (M < 0 || D <= 0) return fail(UPR_ERR_INVALID_ARG, "bad sizes M=%lld D=%d", (long long)M, D);
   if (D % 8 != 0 || D > 4096) return fail(UPR_ERR_UNSUPPORTED, "D=%d must be a multiple of 8 and <= 4096", D);
+  if (y_fp8 && !(y_scale > 0.f)) return fail(UPR_ERR_INVALID_ARG, "y_scale must be > 0");
   if (M == 0) return UPR_OK;
   if (!x || !gamma || !beta || !y) return fail(UPR_ERR_INVALID_ARG, "NULL tensor pointer");
   upr_status s = check_device();
   if (s != UPR_OK) return s;
   const long long blocks = (M + 7) / 8;
   const int grid = static_cast<int>(blocks < sm_count() * 8LL ? blocks : sm_count() * 8LL);
-  upr::upr_layernorm_kernel<<<grid, 256, 0, static_cast<cudaStream_t>(stream)>>>(
-      static_cast<const __nv_bfloat16*>(x), gamma, beta, M, D, eps, static_cast<__nv_bfloat16*>(y));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (y_fp8)
+    upr::upr_layernorm_kernel<true><<<grid, 256, 0, st>>>(static_cast<const __nv_bfloat16*>(x), gamma, beta, M, D, eps, y,
+                                                          1.0f / y_scale);
+  else
+    upr::upr_layernorm_kernel<false><<<grid, 256, 0, st>>>(static_cast<const __nv_bfloat16*>(x), gamma, beta, M, D, eps, y,
+                                                           1.0f);
   UPR_CUDA_CHECK(cudaGetLastError());
   g_launches = 1;
   return UPR_OK;
+}
+
+upr_status upr_layernorm_fwd(const void* x, const float* gamma, const float* beta, void* y, int64_t M, int D,
+                             float eps, void* stream) {
+  return layernorm_impl(x, gamma, beta, y, false, 1.f, M, D, eps, stream);
+}
+
+upr_status upr_layernorm_fp8_fwd(const void* x, const float* gamma, const float* beta, void* y_e4m3, float y_scale,
+                                 int64_t M, int D, float eps, void* stream) {
+  return layernorm_impl(x, gamma, beta, y_e4m3, true, y_scale, M, D, eps, stream);
 }
 
 upr_status upr_kv_project_into_pool(const void* x, upr_dtype x_dtype, const void* w, const float* bias, void* pool,

@@ -123,9 +123,12 @@ class RankingDecodeLayer:
         h1 = LN1(x);  q, k_self, v_self = h1 Wq^T, h1 Wk^T, h1 Wv^T
         a  = cross-attention(q; cached history K/V of the user; own key/value)        (fp32)
         x2 = x + a Wo^T;  h2 = LN2(x2);  y = x2 + W2 silu(W1 h2 + b1) + b2
-    x: bf16 [total_q, D]; weights bf16 [out, in] (synthetic), LN parameters fp32.  Buffers are allocated once."""
+    x: bf16 [total_q, D]; weights bf16 [out, in] (synthetic), LN parameters fp32.  Buffers are allocated once.
+    With `fp8_mlp` = {"w1_8", "w1_scale", "w2_8", "w2_scale", "h_scale", "u_scale"} (E4M3 weight bytes and per-tensor
+    scales) the MLP runs as an FP8 chain: LN2 writes E4M3 bytes, both GEMMs take both operands as
+    E4M3 through TMA, the hidden tensor stays E4M3 in between."""
 
-    def __init__(self, attn: CrossAttention, D: int, hidden: int, params: dict, device=None):
+    def __init__(self, attn: CrossAttention, D: int, hidden: int, params: dict, device=None, fp8_mlp: dict = None):
         self.attn = attn
         assert attn.n_layers == 1, "one attention object per layer"
         self.D, self.hidden, self.p = D, hidden, params
@@ -140,6 +143,10 @@ class RankingDecodeLayer:
         self.h2 = torch.empty((M, D), **bf)
         self.u = torch.empty((M, hidden), **bf)
         self.y = torch.empty((M, D), **bf)
+        self.fp8 = fp8_mlp
+        if fp8_mlp is not None:
+            self.h2_8 = torch.empty((M, D), dtype=torch.uint8, device=dev)
+            self.u_8 = torch.empty((M, hidden), dtype=torch.uint8, device=dev)
         self.launches = 0
 
     def __call__(self, x: torch.Tensor, stream=None) -> torch.Tensor:
@@ -152,8 +159,16 @@ class RankingDecodeLayer:
         B_.upr_linear_fwd(self.h1, p["wv"], None, self.vs.view(M, Hq * d), stream=stream); n += 1
         out = a(self.q, self.ks, self.vs, stream=stream); n += B_.upr_last_launch_count()
         B_.upr_linear_residual_fwd(out.view(M, Hq * d), p["wo"], None, x, self.x2, stream=stream); n += 1
-        B_.upr_layernorm_fwd(self.x2, p["ln2_g"], p["ln2_b"], self.h2, stream=stream); n += 1
-        B_.upr_linear_fwd(self.h2, p["w1"], p["b1"], self.u, B_.UPR_ACT_SILU, stream=stream); n += 1
-        B_.upr_linear_residual_fwd(self.u, p["w2"], p["b2"], self.x2, self.y, stream=stream); n += 1
+        f8 = self.fp8
+        if f8 is None:
+            B_.upr_layernorm_fwd(self.x2, p["ln2_g"], p["ln2_b"], self.h2, stream=stream); n += 1
+            B_.upr_linear_fwd(self.h2, p["w1"], p["b1"], self.u, B_.UPR_ACT_SILU, stream=stream); n += 1
+            B_.upr_linear_residual_fwd(self.u, p["w2"], p["b2"], self.x2, self.y, stream=stream); n += 1
+        else:
+            B_.upr_layernorm_fp8_fwd(self.x2, p["ln2_g"], p["ln2_b"], self.h2_8, f8["h_scale"], stream=stream); n += 1
+            B_.upr_linear_fp8_ex_fwd(self.h2_8, f8["h_scale"], f8["w1_8"], f8["w1_scale"], p["b1"], None, self.u_8,
+                                     f8["u_scale"], B_.UPR_ACT_SILU, stream=stream); n += 1
+            B_.upr_linear_fp8_ex_fwd(self.u_8, f8["u_scale"], f8["w2_8"], f8["w2_scale"], p["b2"], self.x2, self.y, 1.0,
+                                     B_.UPR_ACT_NONE, stream=stream); n += 1
         self.launches = n
         return self.y

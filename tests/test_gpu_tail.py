@@ -228,6 +228,63 @@ def test_one_ranking_decode_layer_matches_the_oracle_chain(P):
     assert err <= 4 * 2.0 ** -8 * np.abs(want).max()
 
 
+
+def _codes_agree(got8, want_values_f64, scale, max_differ=5e-3):
+    """E4M3 bytes from the GPU against the oracle's quantisation of its own fp64 values: equal except where a value
+    sits on a rounding boundary (the GPU decides on its fp32 value), and then one E4M3 step apart at most."""
+    code_want = oracle.e4m3_encode((want_values_f64.astype(np.float32) * (np.float32(1.0) / np.float32(scale))).astype(np.float32))
+    differ = got8 != code_want
+    dec_g, dec_w = oracle.e4m3_decode(got8), oracle.e4m3_decode(code_want)
+    step = np.maximum(np.abs(dec_w), 2.0 ** -6) * 2.0 ** -3
+    assert differ.mean() < max_differ, differ.mean()
+    assert (np.abs(dec_g - dec_w) <= step + 1e-12).all()
+    return float(differ.mean())
+
+
+def test_decode_layer_with_an_fp8_mlp_chain(P):
+    """PAPER.md:206 (FP8 linear layers) inside the decode layer: LN2 writes E4M3, up-projection (E4M3 x E4M3, SiLU)
+    writes E4M3, down-projection (E4M3 x E4M3) + residual writes bf16.  Each stage is checked against the oracle fed
+    the GPU's OWN input bytes of that stage, so every comparison is between the same operands."""
+    from paper_2606_00422_b200 import pipeline as pl
+    dev = "cuda"
+    H, d, hidden = 2, 128, 1024
+    D = H * d
+    L, C = [300, 64, 0, 129], [700, 17, 5, 600]
+    w = S.custom_workload("layer8", 151, L, C, H, d, 1, self_term=True)
+    M = w.total_q
+    k_pool, v_pool = S.gen_pool(w, "k_pool", dev), S.gen_pool(w, "v_pool", dev)
+    view = pl.PoolView.of(k_pool, v_pool, torch.as_tensor(S.slot_ids(w), device=dev), w.seq_lens)
+    attn = pl.CrossAttention(view, w.cand_offsets, P.UPR_BF16)
+    prm = {"ln1_g": torch.ones(D, device=dev), "ln1_b": torch.zeros(D, device=dev),
+           "ln2_g": 1.0 + 0.1 * S.normal_bf16(154, "g2", (D,), dev).float(), "ln2_b": 0.1 * S.normal_bf16(155, "b2", (D,), dev).float(),
+           "wq": weights(156, "wq", D, D, dev), "wk": weights(157, "wk", D, D, dev), "wv": weights(158, "wv", D, D, dev),
+           "wo": weights(159, "wo", D, D, dev), "w1": weights(160, "w1", hidden, D, dev), "w2": weights(161, "w2", D, hidden, dev),
+           "b1": 0.1 * S.normal_bf16(162, "bb1", (hidden,), dev).float(), "b2": 0.1 * S.normal_bf16(163, "bb2", (D,), dev).float()}
+
+    def q8(wt):
+        wf = wt.float()
+        sc = float(np.float32(wf.abs().max().item()) / np.float32(448.0))
+        return (wf * (np.float32(1.0) / np.float32(sc))).to(torch.float8_e4m3fn).view(torch.uint8), sc
+    w1_8, w1_s = q8(prm["w1"])
+    w2_8, w2_s = q8(prm["w2"])
+    f8 = {"w1_8": w1_8, "w1_scale": w1_s, "w2_8": w2_8, "w2_scale": w2_s,
+          "h_scale": float(np.float32(5.0) / np.float32(448.0)), "u_scale": float(np.float32(6.0) / np.float32(448.0))}
+    x = S.normal_bf16(164, "x", (M, D), dev)
+    layer = pl.RankingDecodeLayer(attn, D, hidden, prm, fp8_mlp=f8)
+    y = layer(x)
+    torch.cuda.synchronize()
+    assert layer.launches == 10
+    x2 = f64(layer.x2)
+    h8, u8 = layer.h2_8.cpu().numpy(), layer.u_8.cpu().numpy()
+    d1 = _codes_agree(h8, oracle.layernorm(x2, f64(prm["ln2_g"]), f64(prm["ln2_b"])), f8["h_scale"])
+    d2 = _codes_agree(u8, oracle.linear_fp8q(h8, f8["h_scale"], w1_8.cpu().numpy(), w1_s, f64(prm["b1"]), act=oracle.ACT_SILU),
+                      f8["u_scale"])
+    want = oracle.linear_fp8q(u8, f8["u_scale"], w2_8.cpu().numpy(), w2_s, f64(prm["b2"])) + x2
+    err = np.abs(f64(y) - want).max()
+    print(f"fp8 mlp: codes differing {d1:.1e} (LN2), {d2:.1e} (up); down-projection max-abs {err:.2e}")
+    assert err <= 2.0 ** -8 * max(1.0, np.abs(want).max()) + 2e-4
+
+
 def test_pair_gemm_residual_and_pool_epilogues(P):
     """The CTA-pair GEMM's residual and pool-addressing epilogues (M large enough for the pair kernel)."""
     dev = "cuda"
