@@ -210,6 +210,25 @@ int upr_cross_attn_num_splits(const upr_attn_params* p);
  */
 upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream);
 
+/*
+ * The same call for callers that must not allocate (CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): identical to upr_cross_attn_fwd_ex -- same params, same kernels, same results -- except that
+ * p->workspace / p->workspace_bytes are IGNORED and the scratch (scheduler counter, work-list tables, split-K
+ * partials) is a static device array inside the library, UPR_NOALLOC_SCRATCH_BYTES long.  The call performs no
+ * cudaMalloc / cudaFree and calls no allocating library routine; the first call on a device looks the array's
+ * address up (cudaGetSymbolAddress) and keeps it.
+ *   - Limit: a call whose upr_cross_attn_workspace_bytes(p) exceeds UPR_NOALLOC_SCRATCH_BYTES is refused with
+ *     UPR_ERR_WORKSPACE and a message that states both numbers (without split-K the need is 256 + ~12 (B + 1)
+ *     bytes; split-K adds n_layers * total_q * H * num_splits * (d + 2) * 4).
+ *   - Cost: every GPU on which the library is loaded holds the array until the process exits.
+ *   - ALL calls on a device share the one array: two calls that overlap on the GPU (different streams, or two
+ *     host threads) race on the scheduler state and corrupt each other's results.  Order them on one stream or
+ *     with events.  The array keeps the last call's contents; each call rewrites what it reads before reading it.
+ */
+#define UPR_NOALLOC_SCRATCH_BYTES (8u << 20)
+size_t upr_cross_attn_noalloc_scratch_bytes(void);
+upr_status upr_cross_attn_fwd_noalloc(const upr_attn_params* p, void* stream);
+
 /* ====================================================================================
  * Around the attention: the rest of one ranking decode layer and the consumer
  * of the ranking pass (8(f)4).  Candidate tokens only; synthetic weights.

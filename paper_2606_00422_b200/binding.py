@@ -13,7 +13,7 @@ UPR_KV_PACKED, UPR_KV_POOL = 0, 1
 UPR_KERNEL_AUTO, UPR_KERNEL_SINGLE, UPR_KERNEL_PAIR = 0, 1, 2
 UPR_ROW_ALIGN, UPR_TAIL_ROWS = 16, 128
 EXPORTED_SYMBOLS = [
-    "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex",
+    "upr_kv_cache_layout", "upr_kv_pack", "upr_cross_attn_fwd", "upr_cross_attn_fwd_ex", "upr_cross_attn_fwd_noalloc", "upr_cross_attn_noalloc_scratch_bytes",
     "upr_cross_attn_workspace_bytes", "upr_cross_attn_num_splits", "upr_last_launch_count",
     "upr_last_error", "upr_version", "upr_last_attn_kernel", "upr_linear_fp8_ex_fwd", "upr_layernorm_fp8_fwd",
     "upr_linear_fwd", "upr_linear_residual_fwd", "upr_linear_fp8_fwd", "upr_layernorm_fwd", "upr_kv_project_into_pool", "upr_action_utility", "upr_topk_per_user",
@@ -90,6 +90,10 @@ def _load() -> ctypes.CDLL:
                                     ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         lib.upr_cross_attn_fwd.restype = ctypes.c_int
         lib.upr_cross_attn_fwd.argtypes = [ctypes.c_void_p] * 6 + [ctypes.c_int] * 4 + [ctypes.c_void_p]
+        lib.upr_cross_attn_fwd_noalloc.restype = ctypes.c_int
+        lib.upr_cross_attn_fwd_noalloc.argtypes = [ctypes.POINTER(_AttnParams), ctypes.c_void_p]
+        lib.upr_cross_attn_noalloc_scratch_bytes.restype = ctypes.c_size_t
+        lib.upr_cross_attn_noalloc_scratch_bytes.argtypes = []
         lib.upr_cross_attn_fwd_ex.restype = ctypes.c_int
         lib.upr_cross_attn_fwd_ex.argtypes = [ctypes.POINTER(_AttnParams), ctypes.c_void_p]
         lib.upr_linear_fwd.restype = ctypes.c_int
@@ -238,6 +242,23 @@ def upr_cross_attn_fwd_ex(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H
                 k_self, v_self, k_scale, v_scale, sm_scale, num_splits, max_seq_len, workspace, kv_source,
                 pool_slots, pool_n_max, H_kv, slot_ids, kv_bytes, kv_rows, kernel, causal)
     _check(_load().upr_cross_attn_fwd_ex(ctypes.byref(p), _stream(stream)))
+
+
+def upr_cross_attn_fwd_noalloc(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers, kv_dtype, q_dtype,
+                               total_q, k_self=None, v_self=None, k_scale=None, v_scale=None, sm_scale=0.0,
+                               num_splits=0, max_seq_len=0, stream=None, kv_source=UPR_KV_PACKED, pool_slots=0,
+                               pool_n_max=0, H_kv=0, slot_ids=None, kv_bytes=0, kv_rows=0,
+                               kernel=UPR_KERNEL_AUTO, causal=0) -> None:
+    """upr_cross_attn_fwd_ex without a workspace argument: the scratch is a static device array in the library
+    (upr_cross_attn_noalloc_scratch_bytes() long); no allocation happens in the call."""
+    p = _params(q, k_cache, v_cache, seq_lens, cand_offsets, out, B, H, d, n_layers, kv_dtype, q_dtype, total_q,
+                k_self, v_self, k_scale, v_scale, sm_scale, num_splits, max_seq_len, None, kv_source,
+                pool_slots, pool_n_max, H_kv, slot_ids, kv_bytes, kv_rows, kernel, causal)
+    _check(_load().upr_cross_attn_fwd_noalloc(ctypes.byref(p), _stream(stream)))
+
+
+def upr_cross_attn_noalloc_scratch_bytes() -> int:
+    return int(_load().upr_cross_attn_noalloc_scratch_bytes())
 
 
 # ---------------------------------------------------------------------------- decode-layer tail, consumer, pool

@@ -687,6 +687,64 @@ upr_status upr_cross_attn_fwd_ex(const upr_attn_params* p, void* stream) {
   return run_attn(p, /*have_workspace=*/true, static_cast<cudaStream_t>(stream));
 }
 
+// ------------------------------------------------------------------ the entry point that allocates nothing
+// Scratch of upr_cross_attn_fwd_noalloc: the workspace of upr_cross_attn_fwd_ex (scheduler counter, work-list
+// tables, split-K partials) as a file-scope device array.  Every GPU that loads the library holds these bytes until
+// the process exits.  In HOST code `g_noalloc_scratch` is only a stand-in for the symbol, not a device address: the
+// address comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[UPR_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+void* g_noalloc_ptr[kMaxDevices] = {};   // device address of g_noalloc_scratch on device i, or nullptr = not asked yet
+
+upr_status noalloc_scratch(void** out) {
+  int dev = 0;
+  UPR_CUDA_CHECK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return fail(UPR_ERR_UNSUPPORTED, "device ordinal %d out of range", dev);
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (g_noalloc_ptr[dev] == nullptr) {
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);   // device `dev` is current
+    if (e != cudaSuccess || ptr == nullptr)
+      return fail(UPR_ERR_CUDA, "cudaGetSymbolAddress(g_noalloc_scratch) on device %d: %s", dev, cudaGetErrorString(e));
+    if ((reinterpret_cast<uintptr_t>(ptr) & 255) != 0)
+      return fail(UPR_ERR_CUDA, "static scratch is not 256-byte aligned");
+    g_noalloc_ptr[dev] = ptr;
+  }
+  *out = g_noalloc_ptr[dev];
+  return UPR_OK;
+}
+}  // namespace
+
+size_t upr_cross_attn_noalloc_scratch_bytes(void) { return UPR_NOALLOC_SCRATCH_BYTES; }
+
+upr_status upr_cross_attn_fwd_noalloc(const upr_attn_params* p, void* stream) {
+  g_launches = 0;
+  if (p == nullptr) return fail(UPR_ERR_INVALID_ARG, "params is NULL");
+  upr_attn_params q = *p;
+  q.workspace = nullptr;
+  q.workspace_bytes = 0;
+  const size_t need = upr_cross_attn_workspace_bytes(&q);
+  if (need == 0) return run_attn(&q, /*have_workspace=*/true, static_cast<cudaStream_t>(stream));   // invalid sizes: validate() names them
+  if (need > static_cast<size_t>(UPR_NOALLOC_SCRATCH_BYTES))
+    return fail(UPR_ERR_WORKSPACE,
+                "upr_cross_attn_fwd_noalloc: this call needs %zu bytes of scratch, the static scratch holds %zu "
+                "(UPR_NOALLOC_SCRATCH_BYTES); lower num_splits / total_q, or use upr_cross_attn_fwd_ex with a workspace",
+                need, static_cast<size_t>(UPR_NOALLOC_SCRATCH_BYTES));
+  if (q.B == 0 || q.total_q == 0) return run_attn(&q, /*have_workspace=*/false, static_cast<cudaStream_t>(stream));
+  void* ws = nullptr;
+  upr_status s = noalloc_scratch(&ws);
+  if (s != UPR_OK) return s;
+  q.workspace = ws;
+  q.workspace_bytes = UPR_NOALLOC_SCRATCH_BYTES;
+  // everything in the scratch that must start from a known state is written by the call itself before it is read:
+  // the scheduler counter and the work-list tables by the schedule kernel / a memset, every split-K partial the
+  // combine kernel reads by the attention kernel.  Nothing of an earlier call's contents is used.
+  return run_attn(&q, /*have_workspace=*/true, static_cast<cudaStream_t>(stream));
+}
+
 // ------------------------------------------------------------------ decode-layer tail, consumer, pool
 namespace {
 struct KvScatter { const int32_t* tok_slot; const int32_t* tok_pos; int layer, S, H, n, d; const void* residual;
