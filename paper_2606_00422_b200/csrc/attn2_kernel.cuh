@@ -4,6 +4,11 @@
 // Same mathematics as attn_kernel.cuh (out = softmax(scale * q K^T) V per candidate over its
 // user's cached history; optional self key/value), different mapping:
 //
+//  * the self term (a6) is ONE MORE KEY TILE per 128-row Q tile: the candidates' own keys / values, loaded by TMA
+//    in the Q tile's row order, under the identity mask of PAPER.md:198 (row r sees key r only).  It goes through
+//    the same S MMA, softmax step and PV MMA as a history tile, so there is no per-item side path (the per-row dot
+//    products and value rows read from global memory cost ~10 000 cycles per item when they were one).
+//
 //  * a cluster of two CTAs (two SMs) owns a work item = (layer, user, KV head, history split,
 //    block of <= 256 query rows); each CTA holds ONE 128-row Q tile and its 128 lanes of TMEM;
 //    tcgen05.mma.cta_group::2 (M = 256) is issued by one thread of the pair's leader and runs on
@@ -28,7 +33,7 @@
 //
 // Roles per CTA (512 threads): warps 0-3 / 4-7 softmax groups, 8 producer (+ scheduler; the
 // leader's fetches the item index and forwards it to the peer), 9 MMA issuer (leader only), 10-11
-// self-logit helpers, 12-15 epilogue.  TMEM: S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512).
+// spare, 12-15 epilogue.  TMEM: S0 [0,128) S1 [128,256) O0 [256,384) O1 [384,512).
 #pragma once
 #include <cuda.h>
 #include <cuda_bf16.h>
@@ -94,6 +99,7 @@ struct Item {
   int cands;     // candidates in the block, 1 .. 2 * cpt
   int kv_row0;   // row of the split's first key in the [rows, d] view of K / V
   int n_keys;    // keys of the split's range (>= 0)
+  int n_self;    // self tiles appended behind the history tiles: 0, or one per 128-row Q tile with candidates
   int lim0;      // causal mode: keys visible to the block's first candidate (row r of the block sees lim0 + r);
                  // otherwise 1 << 30
 };
@@ -108,16 +114,14 @@ struct __align__(16) Ctrl {
   uint64_t p_full[2][2];           // [S buffer][half]: leader's copy collects both CTAs' arrivals
   uint64_t pv_done[4];            // PV half-step hs completes phase hs / 4 of pv_done[hs % 4]
   uint64_t o_full[2], o_empty[2];
-  uint64_t l_ready[kItemSlots], self_full[kItemSlots];
+  uint64_t l_ready[kItemSlots];
   Item items[kItemSlots];
   uint32_t idx_ring[kItemSlots];
   uint32_t tmem_base;
   uint32_t pad_[3];
   int mma_fifo[4][4];                      // MMA thread only: keyed items between its S and PV cursors
-  float s_self[kItemSlots][kRows];         // self logits, log2 units
   float mx_sh[2][2][kRows];                // [S buffer][softmax group][row]: maximum of the group's 64 columns
   float epi_l[kItemSlots][2][kRows];       // the two groups' partial row sums
-  float epi_wself[kItemSlots][kRows];      // weight of the candidate's own value row
 };
 constexpr int kSmemQ = 2 * kQBytes;                          //  65536
 constexpr int kSmemKV = kKvSlots * kHalfBytes;               // 131072
@@ -131,31 +135,16 @@ __host__ __device__ constexpr uint32_t idesc_pair(int N, int b_mn_major) {
   return make_idesc_bf16(256, N, 0, b_mn_major);
 }
 
-// dot(q_row, kself_row), both bf16 rows of 128 in global memory
-__device__ __forceinline__ float row_dot128(const void* a, const void* b, size_t e) {
-  const uint4* pa = reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(a) + e);
-  const uint4* pb = reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(b) + e);
-  float acc = 0.f;
-#pragma unroll 4
-  for (int i = 0; i < kD / 8; ++i) {
-    const uint4 x = __ldg(pa + i), y = __ldg(pb + i);
-    const __nv_bfloat162* xs = reinterpret_cast<const __nv_bfloat162*>(&x);
-    const __nv_bfloat162* ys = reinterpret_cast<const __nv_bfloat162*>(&y);
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const float2 fx = __bfloat1622float2(xs[k]), fy = __bfloat1622float2(ys[k]);
-      acc = fmaf(fx.x, fy.x, acc);
-      acc = fmaf(fx.y, fy.y, acc);
-    }
-  }
-  return acc;
-}
-
+// kSelf: the call has a self term (k_self / v_self).  Two instantiations, so that the code of the self tiles costs the
+// calls without a self term nothing (registers, scheduling of the steady-state loop).
+template <bool kSelf>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 128] bf16, box 64 keys x 64 d
                      const __grid_constant__ CUtensorMap tmap_v,    // [rows, 128] bf16, box 128 keys x 64 d
                      const __grid_constant__ CUtensorMap tmap_q,    // [n_layers*total_q, H_q*128], box cpt x 64
                      const __grid_constant__ CUtensorMap tmap_out,  // fp32 [n_layers*total_q, H_q*128], box 32 x 32
+                     const __grid_constant__ CUtensorMap tmap_ks,   // k_self like q, box min(64, cpt) rows x 64
+                     const __grid_constant__ CUtensorMap tmap_vs,   // v_self like q, box cpt rows x 64
                      const Args args) {
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -171,7 +160,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
   // compiler knows it is warp-uniform: 0 = leader; this CTA owns tile `rank` of every item
   const uint32_t rank = blockIdx.x & 1u;
   const bool leader = rank == 0;
-  const bool has_self = args.k_self != nullptr;
+  constexpr bool has_self = kSelf;
   const bool partial = args.num_splits > 1;
   const int G = args.G, cpt = args.cpt;
 
@@ -185,16 +174,14 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
     diag_c0 = static_cast<unsigned long long>(clock64());
   }
   if (threadIdx.x == 0) {
-    // readers that release an item slot: 8 softmax warps, 4 epilogue warps, 2 helper warps (self
-    // term only), the MMA thread (leader only)
-    const uint32_t readers = 8 + 4 + (has_self ? 2 : 0) + (leader ? 1 : 0);
+    // readers that release an item slot: 8 softmax warps, 4 epilogue warps, the MMA thread (leader only)
+    const uint32_t readers = 8 + 4 + (leader ? 1 : 0);
     for (int i = 0; i < kItemSlots; ++i) {
       mbar_init(smem_u32(&ctrl->item_full[i]), 1);
       mbar_init(smem_u32(&ctrl->item_empty[i]), readers);
       mbar_init(smem_u32(&ctrl->idx_full[i]), 1);
       mbar_init(smem_u32(&ctrl->idx_free[i]), 1);
       mbar_init(smem_u32(&ctrl->l_ready[i]), 8);
-      mbar_init(smem_u32(&ctrl->self_full[i]), 2);
     }
     for (int i = 0; i < kKvSlots; ++i) {
       mbar_init(smem_u32(&ctrl->kv_full[i]), 1);    // leader's arrive.expect_tx; bytes from both CTAs
@@ -216,6 +203,10 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
     tma_prefetch_desc(&tmap_k);
     tma_prefetch_desc(&tmap_v);
     tma_prefetch_desc(&tmap_q);
+    if (has_self) {
+      tma_prefetch_desc(&tmap_ks);
+      tma_prefetch_desc(&tmap_vs);
+    }
   }
   if (warp == kMmaWarp) {
     tmem_alloc_pair(smem_u32(&ctrl->tmem_base), 512);
@@ -324,8 +315,12 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
         it.kv_row0 = kv_row0;
         it.n_keys = n_keys;
         it.lim0 = lim0;
+        // the candidates' own keys (first split only): one tile per 128-row Q tile that holds candidates
+        const int n_self = (has_self && split == 0) ? (it.cands > cpt ? 2 : 1) : 0;
+        it.n_self = n_self;
         mbar_arrive(smem_u32(&ctrl->item_full[islot]));
-        const int nt = (n_keys + kKeys - 1) / kKeys;
+        const int nt_hist = (n_keys + kKeys - 1) / kKeys;
+        const int nt = nt_hist + n_self;
         if (nt > 0) {
           // ---- this CTA's Q tile: G boxes of cpt candidates x 64 columns per 64-column half
           const int qb = n_keyed & 1;
@@ -351,7 +346,23 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
               if (leader) mbar_arrive_expect_tx(smem_u32(&ctrl->kv_full[slot]), 2 * kHalfBytes);
               const uint32_t dst = kv_smem + slot * kHalfBytes;
               const uint32_t bar = lead_kv_full + slot * 8;
-              if (kv == 0) {
+              if (j >= nt_hist) {
+                // self tile t: its 128 keys are the rows of Q tile t (g-major: key g * cpt + cl = candidate cl, head g)
+                const int srow0 = layer * args.total_q + it.c0 + (j - nt_hist) * cpt;
+                if (kv == 0) {
+                  const int kbox = min(64, cpt);      // keys [64 rank, 64 rank + 64) in boxes of kbox rows
+                  for (int r0 = static_cast<int>(rank) * 64; r0 < static_cast<int>(rank) * 64 + 64; r0 += kbox) {
+                    const int g = r0 / cpt, cl0 = r0 - g * cpt;
+                    const uint32_t d2 = dst + (r0 - static_cast<int>(rank) * 64) * 128;
+                    tma_load_2d_pair(d2, &tmap_ks, (hkv * G + g) * kD, srow0 + cl0, bar);
+                    tma_load_2d_pair(d2 + kKBoxBytes, &tmap_ks, (hkv * G + g) * kD + 64, srow0 + cl0, bar);
+                  }
+                } else {
+                  for (int g = 0; g < G; ++g)       // 128 keys x columns [64 rank, 64 rank + 64)
+                    tma_load_2d_pair(dst + g * cpt * 128, &tmap_vs, (hkv * G + g) * kD + static_cast<int>(rank) * 64,
+                                     srow0, bar);
+                }
+              } else if (kv == 0) {
                 const int row = kv_row0 + j * kKeys + static_cast<int>(rank) * 64;
                 tma_load_2d_pair(dst, &tmap_k, 0, row, bar);
                 tma_load_2d_pair(dst + kKBoxBytes, &tmap_k, 64, row, bar);
@@ -393,7 +404,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       // PV cursor: a FIFO (shared memory, private to this thread) of the keyed items between the
       // two cursors; the head entry is cached in registers
       uint32_t f_head = 0, f_tail = 0;   // f_tail - f_head = keyed items entered by S and not finished by PV
-      int p_j = 0, p_nkeys = 0, p_slot = 0;
+      int p_j = 0, p_nkeys = 0, p_slot = 0, p_nt = 0;
       uint32_t p_kv = 0;
       uint32_t gp = 0;            // global tiles PV-issued
       uint32_t p_keyed = 0;       // keyed items the PV cursor has finished
@@ -414,7 +425,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
               s_end = true;
               break;
             }
-            const int nt = (it.n_keys + kKeys - 1) / kKeys;
+            const int nt = (it.n_keys + kKeys - 1) / kKeys + it.n_self;
             ++s_item;
             if (nt == 0) {              // key-less item: nothing for the tensor pipe
               mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
@@ -428,6 +439,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             ctrl->mma_fifo[fi][0] = it.n_keys;
             ctrl->mma_fifo[fi][1] = islot;
             ctrl->mma_fifo[fi][2] = static_cast<int>(s_kv);
+            ctrl->mma_fifo[fi][3] = nt;
             ++f_tail;
             const int qb = s_keyed & 1;
             mbar_wait_cluster(smem_u32(&ctrl->q_full[qb]), (s_keyed >> 1) & 1);
@@ -461,16 +473,19 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             p_nkeys = ctrl->mma_fifo[fi][0];
             p_slot = ctrl->mma_fifo[fi][1];
             p_kv = static_cast<uint32_t>(ctrl->mma_fifo[fi][2]);
+            p_nt = ctrl->mma_fifo[fi][3];
           }
           const int n_keys = p_nkeys;
-          const int nt = (n_keys + kKeys - 1) / kKeys;
+          const int nt = p_nt;                                  // history tiles, then self tiles
           const uint32_t ob = p_keyed & 1;
           if (p_j == 0 && p_keyed >= 2)   // the epilogue must have drained this O buffer (item p_keyed - 2)
             mbar_wait_cluster(smem_u32(&ctrl->o_empty[ob]), ((p_keyed >> 1) - 1) & 1);
           const uint32_t sb = gp & 1;
           const uint32_t vpos = p_kv + 2 * p_j + 1;
           const uint32_t vslot = vpos % kKvSlots;
-          const int ksteps = (min(kKeys, n_keys - p_j * kKeys) + 15) >> 4;
+          // k-steps of 16 keys: the history's last tile may be short; a self tile has all 128 (P is 0 off the diagonal)
+          const int keys_left = n_keys - p_j * kKeys;
+          const int ksteps = keys_left > 0 ? (min(kKeys, keys_left) + 15) >> 4 : kKeys / 16;
           const uint32_t v_lo = kv_lo + kLoMN + ((vslot * kHalfBytes) >> 4);
           const uint32_t tp = tmem_base + sb * kKeys;          // P(g, h): packed bf16 pairs at columns 64 h + [0, 32)
           const uint32_t to = tmem_base + 256 + ob * kD;
@@ -502,37 +517,9 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
     }
     __syncwarp();
   } else if (warp == kHelpWarp0 || warp == kHelpWarp0 + 1) {
-    // ================================================================= self-logit helpers
-    // s_self = scale * <q_c, k_self_c> for the NEXT items' rows while the current one runs
+    // ================================================================= spare warps
+    // (they only hand their registers to the softmax groups)
     setmaxnreg_dec<kOtherRegs>();
-    if (has_self) {
-      const int hw = warp - kHelpWarp0;
-      for (uint32_t n = 0;; ++n) {
-        const int islot = n & (kItemSlots - 1);
-        mbar_wait<6>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
-        const Item it = ctrl->items[islot];
-        if (!it.valid) break;
-        if (it.split == 0) {
-          const int nh = cands_here(it);
-#pragma unroll
-          for (int rr = 0; rr < 2; ++rr) {
-            const int row = hw * 64 + rr * 32 + lane;
-            const int g = row / cpt, cl = row - g * cpt;
-            float s = 0.f;
-            if (cl < nh) {
-              const size_t e = ((static_cast<size_t>(it.layer) * args.total_q + it.c0 + rank * cpt + cl) * args.H_q +
-                                it.hkv * G + g) * kD;
-              s = row_dot128(args.q, args.k_self, e) * args.scale_log2;
-            }
-            ctrl->s_self[islot][row] = s;
-          }
-          __syncwarp();
-          if (lane == 0) mbar_arrive(smem_u32(&ctrl->self_full[islot]));
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(smem_u32(&ctrl->item_empty[islot]));
-      }
-    }
   } else if (warp < 8) {
     // ================================================================= softmax groups
     // Both groups work on EVERY key tile of the CTA's 128 rows, two threads per row: group wg owns
@@ -553,33 +540,61 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
     const uint32_t p_full_addr = mapa_shared(smem_u32(&ctrl->p_full[0][wg]), 0);   // the leader's barriers
     uint32_t g0 = 0;          // global key tiles before the current item
     uint32_t n_keyed = 0;     // keyed items before the current one (O buffer)
-    uint32_t self_par = 0;    // bit s: parity of the next self_full[s] phase to wait for
     for (uint32_t n = 0;; ++n) {
       const int islot = n & (kItemSlots - 1);
       mbar_wait<7>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
       const Item it = ctrl->items[islot];
       if (!it.valid) break;
-      const int nt = (it.n_keys + kKeys - 1) / kKeys;
+      const int nt_hist = (it.n_keys + kKeys - 1) / kKeys;
+      const int nt = nt_hist + (kSelf ? it.n_self : 0);   // history tiles, then one self tile per Q tile with candidates
       const int nh = cands_here(it);
       const int g = row / cpt, cl = row - g * cpt;
       const bool row_valid = cl < nh;
-      const bool self_here = has_self && it.split == 0;
       const uint32_t ob = n_keyed & 1;
       const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD + wg * (kD / 2);   // own half of O's columns
-      float s_self = 0.f;
-      if (self_here) {
-        mbar_wait<8>(smem_u32(&ctrl->self_full[islot]), (self_par >> islot) & 1);
-        self_par ^= 1u << islot;
-        s_self = ctrl->s_self[islot][row];
-      }
-      // running state, log2 units; the self key (first split only) seeds it (its weight 1 is
-      // carried by group 0's partial sum)
-      float m_used = self_here ? s_self : -INFINITY;
-      float l = (self_here && wg == 0) ? 1.f : 0.f;
+      // running state, log2 units
+      float m_used = -INFINITY;
+      float l = 0.f;
       if (nh > 0) {
         // keys this thread's row may see (causal mode; otherwise all of the item's)
         const int lim_row = min(it.n_keys, it.lim0 + static_cast<int>(rank) * cpt + cl);
         const int lim_cta = it.lim0 + static_cast<int>(rank) * cpt;      // ... and the CTA tile's first row
+        // The two threads of a row exchange the maxima of their halves, take the same lazy-rescale decision
+        // (m moves only when the tile's maximum exceeds it by more than kTau) and rescale their halves of O.
+        auto advance_max = [&](const float mx_mine, const int j, const uint32_t gidx, const uint32_t sb) {
+          ctrl->mx_sh[sb][wg][row] = mx_mine;
+          named_bar_sync(kBarMax, 256);
+          const float mx = fmaxf(mx_mine, ctrl->mx_sh[sb][wg ^ 1][row]) * args.scale_log2;
+          const float m_new = fmaxf(m_used, mx);
+          const bool need = m_new > m_used + kTau;
+          if (j == 0) {
+            // nothing accumulated in O yet (the first PV overwrites)
+            if (need) {
+              l *= ex2_approx(m_used - m_new);
+              m_used = m_new;
+            }
+          } else if (__any_sync(0xffffffffu, need)) {
+            // the PV half-steps of the earlier tiles (hs < 2 g) may still be accumulating into O.
+            // Steps <= 2 g - 4 are complete (they were issued before S(g), which has been read); a
+            // ring of four barriers keeps the parity wait on step 2 g - 1 unambiguous even though
+            // this path is taken rarely.
+            const uint32_t hp = 2 * gidx - 1;
+            mbar_wait<10>(smem_u32(&ctrl->pv_done[hp & 3]), (hp >> 2) & 1);
+            tc_fence_after();
+            const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
+#pragma unroll
+            for (int c0 = 0; c0 < kD / 2; c0 += 16) {
+              uint32_t orr[16];
+              tmem_ld16(tm_o + c0, orr);
+              tmem_wait_ld_regs(orr);
+#pragma unroll
+              for (int c = 0; c < 16; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
+              tmem_st16(tm_o + c0, orr);
+            }
+            l *= alpha;
+            if (need) m_used = m_new;
+          }
+        };
         // One 128-key tile.  Tiles that need masking (the item's last tile: history tail; causal mode: the
         // tiles that reach past the diagonal) are a separate instantiation so that the steady-state loop
         // body stays small.
@@ -612,38 +627,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             mxd = fmax3(mxd, __uint_as_float(sr[c + 6]), __uint_as_float(sr[c + 7]));
           }
           const float mx_mine = fmaxf(fmaxf(mxa, mxb), fmaxf(mxc, mxd));
-          ctrl->mx_sh[sb][wg][row] = mx_mine;
-          named_bar_sync(kBarMax, 256);
-          const float mx = fmaxf(mx_mine, ctrl->mx_sh[sb][wg ^ 1][row]) * args.scale_log2;
-          const float m_new = fmaxf(m_used, mx);
-          const bool need = m_new > m_used + kTau;
-          if (j == 0) {
-            // nothing accumulated in O yet (the first PV overwrites); only l may hold the self weight
-            if (need) {
-              l *= ex2_approx(m_used - m_new);
-              m_used = m_new;
-            }
-          } else if (__any_sync(0xffffffffu, need)) {
-            // the PV half-steps of the earlier tiles (hs < 2 g) may still be accumulating into O.
-            // Steps <= 2 g - 4 are complete (they were issued before S(g), which has been read); a
-            // ring of four barriers keeps the parity wait on step 2 g - 1 unambiguous even though
-            // this path is taken rarely.
-            const uint32_t hp = 2 * gidx - 1;
-            mbar_wait<10>(smem_u32(&ctrl->pv_done[hp & 3]), (hp >> 2) & 1);
-            tc_fence_after();
-            const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
-#pragma unroll
-            for (int c0 = 0; c0 < kD / 2; c0 += 16) {
-              uint32_t orr[16];
-              tmem_ld16(tm_o + c0, orr);
-              tmem_wait_ld_regs(orr);
-#pragma unroll
-              for (int c = 0; c < 16; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
-              tmem_st16(tm_o + c0, orr);
-            }
-            l *= alpha;
-            if (need) m_used = m_new;
-          }
+          advance_max(mx_mine, j, gidx, sb);
           float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
           // (a row that has seen no key yet -- causal mode with more candidates than keys -- keeps m = -inf:
           // subtract 0 instead, its logits are all -inf and its weights 0)
@@ -676,15 +660,59 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
           __syncwarp();
           if (lane == 0) mbar_arrive_cluster(p_full_addr + sb * 16);
         };
-        for (int j = 0; j < nt; ++j) {
-          if (j == nt - 1 || (j + 1) * kKeys > lim_cta) step(j, cuda::std::true_type{});
+        // Self tile t = j - nt_hist: its keys are Q tile t's own rows under the identity block of the mask
+        // (PAPER.md:198): row r of CTA t sees key r, every other (row, key) pair of the tile is masked.  One logit,
+        // one exponential and one non-zero P entry per row: the row's thread whose columns hold the diagonal
+        // (group row / 64) picks S[r][r] out of the 32 columns its warp's diagonal lies in; everything else in P is 0.
+        auto self_step = [&](const int j) {
+          const uint32_t gidx = g0 + j;
+          const uint32_t sb = gidx & 1;
+          const uint32_t tm_s = tmem_base + lane_base + sb * kKeys + wg * 64;
+          mbar_wait<9>(smem_u32(&ctrl->s_full[sb]), (gidx >> 1) & 1);
+          tc_fence_after();
+          const bool tile_mine = (j - nt_hist) == static_cast<int>(rank);
+          const bool diag_warp = tile_mine && ((warp >> 1) & 1) == wg;       // warp-uniform: rows [32 (warp & 3), +32)
+          const uint32_t dcol = (warp & 1) * 32;                              // ... have their diagonal at these columns
+          float x = -INFINITY;
+          if (diag_warp) {
+            uint32_t sr[32];
+            tmem_ld32(tm_s + dcol, sr);
+            tmem_wait_ld_regs(sr);
+            uint32_t v = 0;
+#pragma unroll
+            for (int c = 0; c < 32; ++c) v = (c == lane) ? sr[c] : v;
+            if (row_valid) x = __uint_as_float(v);
+          }
+          advance_max(x, j, gidx, sb);
+          const float m_sub = (m_used == -INFINITY) ? 0.f : m_used;
+          const float w = ex2_approx(fmaf(x, args.scale_log2, -m_sub));      // 0 for every thread without a diagonal
+          const uint32_t wb = pack_bf16x2(w, 0.f);                            // bf16(w) in the low half
+          l += __uint_as_float(wb << 16);
+          const uint32_t val = (lane & 1) ? (wb << 16) : wb;                  // key row & 63 = dcol + lane: packed column (dcol + lane) / 2
+#pragma unroll
+          for (int hh = 0; hh < 2; ++hh) {
+            uint32_t z[16];
+            const bool here = diag_warp && hh == (warp & 1);
+#pragma unroll
+            for (int i = 0; i < 16; ++i) z[i] = (here && i == (lane >> 1)) ? val : 0u;
+            tmem_st16(tm_s + hh * 16, z);
+          }
+          tmem_wait_st();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cluster(p_full_addr + sb * 16);
+        };
+        for (int j = 0; j < nt_hist; ++j) {
+          if (j == nt_hist - 1 || (j + 1) * kKeys > lim_cta) step(j, cuda::std::true_type{});
           else step(j, cuda::std::false_type{});
+        }
+        if constexpr (kSelf) {
+          for (int j = nt_hist; j < nt; ++j) self_step(j);
         }
         // hand the row's final state to the epilogue: the two partial sums (added there), and from
         // group 0 the weight of the candidate's own value row; split-K partial state by group 0
         // once both sums are in shared memory
         ctrl->epi_l[islot][wg][row] = l;
-        if (wg == 0) ctrl->epi_wself[islot][row] = self_here ? ex2_approx(s_self - m_used) : 0.f;
         if (partial) {
           named_bar_sync(kBarMax, 256);
           if (wg == 0 && row_valid) {
@@ -728,9 +756,8 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       mbar_wait<11>(smem_u32(&ctrl->item_full[islot]), (n / kItemSlots) & 1);
       const Item it = ctrl->items[islot];
       if (!it.valid) break;
-      const int nt = (it.n_keys + kKeys - 1) / kKeys;
+      const int nt = (it.n_keys + kKeys - 1) / kKeys + it.n_self;
       const int nh = cands_here(it);
-      const bool self_here = has_self && it.split == 0;
       const uint32_t ob = n_keyed & 1;
       if (nh > 0) {
         mbar_wait<12>(smem_u32(&ctrl->l_ready[islot]), (lr_par >> islot) & 1);
@@ -742,15 +769,11 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       }
       if (nh > 0) {
         const int row = ew * 32 + lane;                  // row of this thread within the tile
-        const int g_own = row / cpt, cl_own = row - g_own * cpt;
         const float lsum = ctrl->epi_l[islot][0][row] + ctrl->epi_l[islot][1][row];
         const float inv = partial ? 1.0f : (lsum > 0.f ? 1.0f / lsum : 0.f);
-        const float ws = ctrl->epi_wself[islot][row] * inv;
         const float2 sc2 = make_float2(inv, inv);
         const int cand0 = it.c0 + static_cast<int>(rank) * cpt;       // first candidate of this CTA's tile
         const size_t lrow0 = static_cast<size_t>(it.layer) * args.total_q;
-        const size_t se0 = ((lrow0 + cand0 + cl_own) * args.H_q + it.hkv * G + g_own) * kD;   // own row, candidate side
-        const bool add_self = self_here && cl_own < nh;
         const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD;
         // the warp's 32 rows are 32 consecutive candidates of one query head when cpt >= 32
         const int g_w = (ew * 32) / cpt, cl_w = (ew * 32) - g_w * cpt;
@@ -772,31 +795,12 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             }
             if (lane == 0) bulk_wait_read_all();
             __syncwarp();
-            if (!self_here) {
 #pragma unroll
-              for (int c = 0; c < 32; c += 4) {
-                const float2 a = fmul2(make_float2(__uint_as_float(orr[c]), __uint_as_float(orr[c + 1])), sc2);
-                const float2 b2 = fmul2(make_float2(__uint_as_float(orr[c + 2]), __uint_as_float(orr[c + 3])), sc2);
-                sts128(sw_row + (((c >> 2) ^ (lane & 7)) << 4), __float_as_uint(a.x), __float_as_uint(a.y),
-                       __float_as_uint(b2.x), __float_as_uint(b2.y));
-              }
-            } else {
-#pragma unroll
-              for (int c = 0; c < 32; c += 8) {
-                const uint4 x = __ldg(reinterpret_cast<const uint4*>(
-                    static_cast<const __nv_bfloat16*>(args.v_self) + se0 + c0 + c));
-                const uint32_t w[4] = {x.x, x.y, x.z, x.w};
-                float o[8];
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                  o[2 * k + 0] = fmaf(ws, __uint_as_float(w[k] << 16), __uint_as_float(orr[c + 2 * k]) * inv);
-                  o[2 * k + 1] = fmaf(ws, __uint_as_float(w[k] & 0xffff0000u), __uint_as_float(orr[c + 2 * k + 1]) * inv);
-                }
-                sts128(sw_row + (((c >> 2) ^ (lane & 7)) << 4), __float_as_uint(o[0]), __float_as_uint(o[1]),
-                       __float_as_uint(o[2]), __float_as_uint(o[3]));
-                sts128(sw_row + ((((c >> 2) + 1) ^ (lane & 7)) << 4), __float_as_uint(o[4]), __float_as_uint(o[5]),
-                       __float_as_uint(o[6]), __float_as_uint(o[7]));
-              }
+            for (int c = 0; c < 32; c += 4) {
+              const float2 a = fmul2(make_float2(__uint_as_float(orr[c]), __uint_as_float(orr[c + 1])), sc2);
+              const float2 b2 = fmul2(make_float2(__uint_as_float(orr[c + 2]), __uint_as_float(orr[c + 3])), sc2);
+              sts128(sw_row + (((c >> 2) ^ (lane & 7)) << 4), __float_as_uint(a.x), __float_as_uint(a.y),
+                     __float_as_uint(b2.x), __float_as_uint(b2.y));
             }
             if (c0 + 32 < kD) tmem_ld32(tm_o + c0 + 32, orr);   // next block: overlaps the store hand-off
             fence_proxy_async_smem();
@@ -831,22 +835,9 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             }
 #pragma unroll
             for (int c = 0; c < 32; c += 8) {
-              float sv[8];
-#pragma unroll
-              for (int k = 0; k < 8; ++k) sv[k] = 0.f;
-              if (add_self) {
-                const uint4 x = __ldg(reinterpret_cast<const uint4*>(
-                    static_cast<const __nv_bfloat16*>(args.v_self) + se0 + c0 + c));
-                const uint32_t w[4] = {x.x, x.y, x.z, x.w};
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {
-                  sv[2 * k + 0] = __uint_as_float(w[k] << 16);
-                  sv[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
-                }
-              }
               float o[8];
 #pragma unroll
-              for (int k = 0; k < 8; ++k) o[k] = fmaf(ws, sv[k], __uint_as_float(orr[c + k]) * inv);
+              for (int k = 0; k < 8; ++k) o[k] = __uint_as_float(orr[c + k]) * inv;
               sts128(st_w + c * 4, __float_as_uint(o[0]), __float_as_uint(o[1]), __float_as_uint(o[2]),
                      __float_as_uint(o[3]));
               sts128(st_w + c * 4 + 16, __float_as_uint(o[4]), __float_as_uint(o[5]), __float_as_uint(o[6]),

@@ -315,7 +315,7 @@ upr_status run_attn_pair(const upr_attn_params* p, int ns, cudaStream_t st) {
     a.part_ml = a.part_o + static_cast<size_t>(out_rows) * ns * p->d;
   }
 
-  CUtensorMap tk, tv, tq, to;
+  CUtensorMap tk, tv, tq, to, tks, tvs;
   memset(&to, 0, sizeof(to));
   const long long rows = kv_view_rows(p);
   upr_status s = make_kv_tmap(&tk, p->k_cache, p->d, rows, /*box_rows=*/64);    // K half: 64 keys x 64 d boxes
@@ -327,6 +327,18 @@ upr_status run_attn_pair(const upr_attn_params* p, int ns, cudaStream_t st) {
   if (!make_cand_tmap(&tq, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p->q, cand_rows, cand_cols, 64, a.cpt,
                       CU_TENSOR_MAP_L2_PROMOTION_L2_256B))
     return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for q");
+  // the candidates' own keys / values enter as one more key tile per Q tile, in the Q tile's row order
+  tks = tq;
+  tvs = tq;
+  if (p->k_self != nullptr) {
+    if ((reinterpret_cast<uintptr_t>(p->k_self) & 15) || (reinterpret_cast<uintptr_t>(p->v_self) & 15))
+      return fail(UPR_ERR_INVALID_ARG, "k_self / v_self must be 16-byte aligned");
+    if (!make_cand_tmap(&tks, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p->k_self, cand_rows, cand_cols, 64,
+                        a.cpt < 64 ? a.cpt : 64, CU_TENSOR_MAP_L2_PROMOTION_L2_256B) ||
+        !make_cand_tmap(&tvs, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, p->v_self, cand_rows, cand_cols, 64, a.cpt,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B))
+      return fail(UPR_ERR_CUDA, "cuTensorMapEncodeTiled failed for k_self / v_self");
+  }
   if (ns == 1 && make_cand_tmap(&to, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, p->out, cand_rows, cand_cols, 32, 32,
                                 CU_TENSOR_MAP_L2_PROMOTION_NONE))
     a.out_tma = 1;
@@ -337,9 +349,15 @@ upr_status run_attn_pair(const upr_attn_params* p, int ns, cudaStream_t st) {
   int pairs = sm_count() / 2;
   if (pairs <= 0) return fail(UPR_ERR_CUDA, "could not query the SM count");
   if (max_items < pairs) pairs = static_cast<int>(max_items < 1 ? 1 : max_items);
-  UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::pair::upr_attn_pair_kernel,
-                                      cudaFuncAttributeMaxDynamicSharedMemorySize, upr::pair::kSmemTotal));
-  upr::pair::upr_attn_pair_kernel<<<2 * pairs, upr::pair::kThreads, upr::pair::kSmemTotal, st>>>(tk, tv, tq, to, a);
+  if (p->k_self != nullptr) {
+    UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::pair::upr_attn_pair_kernel<true>,
+                                        cudaFuncAttributeMaxDynamicSharedMemorySize, upr::pair::kSmemTotal));
+    upr::pair::upr_attn_pair_kernel<true><<<2 * pairs, upr::pair::kThreads, upr::pair::kSmemTotal, st>>>(tk, tv, tq, to, tks, tvs, a);
+  } else {
+    UPR_CUDA_CHECK(cudaFuncSetAttribute(upr::pair::upr_attn_pair_kernel<false>,
+                                        cudaFuncAttributeMaxDynamicSharedMemorySize, upr::pair::kSmemTotal));
+    upr::pair::upr_attn_pair_kernel<false><<<2 * pairs, upr::pair::kThreads, upr::pair::kSmemTotal, st>>>(tk, tv, tq, to, tks, tvs, a);
+  }
   UPR_CUDA_CHECK(cudaGetLastError());
   g_launches = 2;
   g_kernel = "upr_attn_pair_kernel";
