@@ -21,9 +21,10 @@
 //    n+1 accumulate into the other buffer; S and PV issue run as one stream of key tiles across
 //    item boundaries (the S tile two ahead is issued behind each PV), so an item boundary costs
 //    no drain and no pipeline refill.
-//  * the two softmax warpgroups of a CTA work on the SAME 128 rows and take alternate key tiles;
-//    the running (max, sum) of a row lives in shared memory and is owned by whoever holds the
-//    "turn" (named barriers), which also keeps the two groups' MUFU phases in anti-phase.
+//  * the two softmax warpgroups of a CTA work on the SAME 128 rows, two threads per row: group wg takes
+//    columns [64 wg, +64) of every key tile.  The half tiles form one sequence of online-softmax steps;
+//    a step reads the reference maximum its predecessor published (named barriers between the two warps
+//    of a lane quarter), applies the lazy-rescale rule and publishes -- no symmetric exchange.
 //  * grouped queries (H_kv < H_q, "KV heads"): the G = H_q / H_kv query heads that
 //    share a KV head are folded into M -- a tile holds 128/G candidates x G heads (g-major) --
 //    so a K/V tile is reused G times more often.
@@ -67,7 +68,9 @@ static_assert(256 * kSoftmaxRegs + 128 * kOtherRegs + 128 * kEpilogueRegs <= kTh
               "setmaxnreg budgets exceed the CTA's register allocation");
 constexpr int kProducerWarp = 8, kMmaWarp = 9, kHelpWarp0 = 10, kEpiWarp0 = 12;
 constexpr float kTau = 8.0f;          // lazy-rescale threshold, log2 units
-constexpr int kBarMax = 1;            // named barrier of the 256 softmax threads (row-maximum exchange)
+// named barriers of the reference-maximum hand-over between the two softmax groups, one pair per TMEM lane quarter q
+// (64 threads each: the two warps that share rows [32 q, +32)): group 0 publishes on kBarAB + q, group 1 on kBarBA + q
+constexpr int kBarAB = 1, kBarBA = 5;
 
 struct Args {
   const void* q;          // bf16 [n_layers, total_q, H_q, 128]
@@ -120,8 +123,10 @@ struct __align__(16) Ctrl {
   uint32_t tmem_base;
   uint32_t pad_[3];
   int mma_fifo[4][4];                      // MMA thread only: keyed items between its S and PV cursors
-  float mx_sh[2][2][kRows];                // [S buffer][softmax group][row]: maximum of the group's 64 columns
-  float epi_l[kItemSlots][2][kRows];       // the two groups' partial row sums
+  float ref_sh[2][kRows];                  // [publishing group][row]: the row's reference maximum after that group's
+                                           // latest half-tile step
+  float epi_l[kItemSlots][2][kRows];       // the two groups' partial row sums ...
+  float epi_m[kItemSlots][2][kRows];       // ... and the reference maximum each is relative to
 };
 constexpr int kSmemQ = 2 * kQBytes;                          //  65536
 constexpr int kSmemKV = kKvSlots * kHalfBytes;               // 131072
@@ -523,19 +528,20 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
   } else if (warp < 8) {
     // ================================================================= softmax groups
     // Both groups work on EVERY key tile of the CTA's 128 rows, two threads per row: group wg owns
-    // the tile's columns [64 wg, 64 wg + 64) -- 64 exponentials per thread and tile.  The row
-    // maximum is the one quantity the two threads of a row must share: each publishes the maximum
-    // of its half and reads its partner's after a 256-thread named barrier; both then take the same
-    // rescale decision, so the running maximum needs no further exchange.  Each thread keeps the
-    // row sum of its own columns (the epilogue adds the two) and rescales its own half of O's
-    // columns.  P(g, wg) is written over the group's OWN S columns (packed bf16 at columns
-    // 64 wg + [0, 32)), so neither group touches TMEM the other still reads.
+    // the tile's columns [64 wg, 64 wg + 64) -- 64 exponentials per thread and tile.  The row's
+    // reference maximum is the one quantity the two threads of a row share; it is handed from half
+    // tile to half tile (see advance_max below).  Each thread keeps the row sum of its own columns
+    // and the reference it is relative to (the epilogue combines the two).  P(g, wg) is written over
+    // the group's OWN S columns (packed bf16 at columns 64 wg + [0, 32)), so neither group touches
+    // TMEM the other still reads.
     // The two groups' exponential phases run CONCURRENTLY: the two warps that share an SM
     // sub-partition are the two groups' warps of the same 32 rows, one warp alone reaches only half
     // of the MUFU rate (measured: 64 ex2 in ~950 cycles against 512), two together saturate it.
     setmaxnreg_inc<kSoftmaxRegs>();
     const int wg = warp >> 2;
+    const int lq = warp & 3;
     const int row = threadIdx.x & 127;       // row of the CTA's tile == TMEM lane
+    bool first_step = true;                  // group 0: nobody has published before the kernel's first step
     const uint32_t lane_base = static_cast<uint32_t>((warp & 3) * 32) << 16;
     const uint32_t p_full_addr = mapa_shared(smem_u32(&ctrl->p_full[0][wg]), 0);   // the leader's barriers
     uint32_t g0 = 0;          // global key tiles before the current item
@@ -551,7 +557,7 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       const int g = row / cpt, cl = row - g * cpt;
       const bool row_valid = cl < nh;
       const uint32_t ob = n_keyed & 1;
-      const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD + wg * (kD / 2);   // own half of O's columns
+      const uint32_t tm_o = tmem_base + lane_base + 256 + ob * kD;   // the row's O accumulator
       // running state, log2 units
       float m_used = -INFINITY;
       float l = 0.f;
@@ -559,31 +565,46 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
         // keys this thread's row may see (causal mode; otherwise all of the item's)
         const int lim_row = min(it.n_keys, it.lim0 + static_cast<int>(rank) * cpt + cl);
         const int lim_cta = it.lim0 + static_cast<int>(rank) * cpt;      // ... and the CTA tile's first row
-        // The two threads of a row exchange the maxima of their halves, take the same lazy-rescale decision
-        // (m moves only when the tile's maximum exceeds it by more than kTau) and rescale their halves of O.
-        auto advance_max = [&](const float mx_mine, const int j, const uint32_t gidx, const uint32_t sb) {
-          ctrl->mx_sh[sb][wg][row] = mx_mine;
-          named_bar_sync(kBarMax, 256);
-          const float mx = fmaxf(mx_mine, ctrl->mx_sh[sb][wg ^ 1][row]) * args.scale_log2;
+        // Reference maximum of a row.  The 64-key half tiles of an item form ONE sequence of online-softmax steps
+        // (tile 0 half 0, tile 0 half 1, tile 1 half 0, ...); group wg owns the steps of half wg.  A step reads the
+        // reference its predecessor published, applies the lazy rule (the reference moves only when the step's own
+        // maximum exceeds it by more than kTau -- and then this thread alone rescales the whole O row, after every
+        // earlier step's PV has completed) and publishes the result for its successor BEFORE its exponentials.
+        // Nothing is exchanged symmetrically: group 0 never waits (its predecessor published a whole exponential
+        // phase ago), group 1 trails it by the hand-over latency, and the 256-thread barrier with its two shared-
+        // memory round trips per tile is gone (measured against it: -2 % on config 3, -4 % on config 5).
+        // (Publishing halfway through the exponentials, to put the groups in anti-phase, was slower: a warp alone
+        // issues an ex2 every 14 - 16 cycles, two warps of a sub-partition together one every 9.)
+        auto advance_max = [&](const float mx_mine, const int j, const uint32_t gidx) {
+          float m_prev;
+          if (wg == 0) {
+            if (!first_step) named_bar_sync(kBarBA + lq, 64);   // (group 1's publication of its previous step)
+            first_step = false;
+            m_prev = (j == 0) ? -INFINITY : ctrl->ref_sh[1][row];
+          } else {
+            named_bar_sync(kBarAB + lq, 64);                     // (group 0's publication of this tile's step)
+            m_prev = ctrl->ref_sh[0][row];
+          }
+          if (m_prev != m_used) {          // the other group moved the reference: bring the own row sum along
+            l *= ex2_approx(m_used - m_prev);
+            m_used = m_prev;
+          }
+          const float mx = mx_mine * args.scale_log2;
           const float m_new = fmaxf(m_used, mx);
           const bool need = m_new > m_used + kTau;
-          if (j == 0) {
+          if (j == 0 && wg == 0) {
             // nothing accumulated in O yet (the first PV overwrites)
-            if (need) {
-              l *= ex2_approx(m_used - m_new);
-              m_used = m_new;
-            }
+            if (need) m_used = m_new;      // l == 0
           } else if (__any_sync(0xffffffffu, need)) {
-            // the PV half-steps of the earlier tiles (hs < 2 g) may still be accumulating into O.
-            // Steps <= 2 g - 4 are complete (they were issued before S(g), which has been read); a
-            // ring of four barriers keeps the parity wait on step 2 g - 1 unambiguous even though
-            // this path is taken rarely.
-            const uint32_t hp = 2 * gidx - 1;
+            // every earlier step's PV (half-steps < 2 gidx + wg) must have landed in O.  Steps <= 2 gidx - 4 are
+            // complete (they were issued before S(gidx), which has been read); a ring of four barriers keeps the
+            // parity wait on the step before this one unambiguous even though this path is taken rarely.
+            const uint32_t hp = 2 * gidx + wg - 1;
             mbar_wait<10>(smem_u32(&ctrl->pv_done[hp & 3]), (hp >> 2) & 1);
             tc_fence_after();
             const float alpha = need ? ex2_approx(m_used - m_new) : 1.0f;
-#pragma unroll
-            for (int c0 = 0; c0 < kD / 2; c0 += 16) {
+#pragma unroll 1
+            for (int c0 = 0; c0 < kD; c0 += 16) {
               uint32_t orr[16];
               tmem_ld16(tm_o + c0, orr);
               tmem_wait_ld_regs(orr);
@@ -591,9 +612,14 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
               for (int c = 0; c < 16; ++c) orr[c] = __float_as_uint(__uint_as_float(orr[c]) * alpha);
               tmem_st16(tm_o + c0, orr);
             }
+            tmem_wait_st();
             l *= alpha;
             if (need) m_used = m_new;
           }
+        };
+        auto publish = [&]() {
+          ctrl->ref_sh[wg][row] = m_used;
+          named_bar_arrive((wg == 0 ? kBarAB : kBarBA) + lq, 64);
         };
         // One 128-key tile.  Tiles that need masking (the item's last tile: history tail; causal mode: the
         // tiles that reach past the diagonal) are a separate instantiation so that the steady-state loop
@@ -627,12 +653,14 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             mxd = fmax3(mxd, __uint_as_float(sr[c + 6]), __uint_as_float(sr[c + 7]));
           }
           const float mx_mine = fmaxf(fmaxf(mxa, mxb), fmaxf(mxc, mxd));
-          advance_max(mx_mine, j, gidx, sb);
+          advance_max(mx_mine, j, gidx);
+          publish();
           float2 sumA = make_float2(0.f, 0.f), sumB = make_float2(0.f, 0.f);
           // (a row that has seen no key yet -- causal mode with more candidates than keys -- keeps m = -inf:
           // subtract 0 instead, its logits are all -inf and its weights 0)
           const float m_sub = (kLast && m_used == -INFINITY) ? 0.f : m_used;
-          const float2 c2 = make_float2(args.scale_log2, args.scale_log2), nm2 = make_float2(-m_sub, -m_sub);
+          const float2 c2 = make_float2(args.scale_log2, args.scale_log2);
+          float2 nm2 = make_float2(-m_sub, -m_sub);
 #pragma unroll
           for (int c0 = 0; c0 < 64; c0 += 32) {
             uint32_t pr[16];
@@ -683,7 +711,8 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
             for (int c = 0; c < 32; ++c) v = (c == lane) ? sr[c] : v;
             if (row_valid) x = __uint_as_float(v);
           }
-          advance_max(x, j, gidx, sb);
+          advance_max(x, j, gidx);
+          publish();
           const float m_sub = (m_used == -INFINITY) ? 0.f : m_used;
           const float w = ex2_approx(fmaf(x, args.scale_log2, -m_sub));      // 0 for every thread without a diagonal
           const uint32_t wb = pack_bf16x2(w, 0.f);                            // bf16(w) in the low half
@@ -709,19 +738,10 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
         if constexpr (kSelf) {
           for (int j = nt_hist; j < nt; ++j) self_step(j);
         }
-        // hand the row's final state to the epilogue: the two partial sums (added there), and from
-        // group 0 the weight of the candidate's own value row; split-K partial state by group 0
-        // once both sums are in shared memory
+        // hand the row's final state to the epilogue: each group's partial sum and the reference it is relative
+        // to (group 1's is the last step's, i.e. the one O is in; the epilogue brings group 0's sum to it)
         ctrl->epi_l[islot][wg][row] = l;
-        if (partial) {
-          named_bar_sync(kBarMax, 256);
-          if (wg == 0 && row_valid) {
-            const size_t prow = ((static_cast<size_t>(it.layer) * args.total_q + it.c0 + rank * cpt + cl) * args.H_q +
-                                 it.hkv * G + g) * args.num_splits + it.split;
-            args.part_ml[prow * 2 + 0] = m_used;
-            args.part_ml[prow * 2 + 1] = l + ctrl->epi_l[islot][1][row];
-          }
-        }
+        ctrl->epi_m[islot][wg][row] = m_used;
         __syncwarp();
         if (lane == 0) mbar_arrive(smem_u32(&ctrl->l_ready[islot]));
       } else {
@@ -769,8 +789,19 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
       }
       if (nh > 0) {
         const int row = ew * 32 + lane;                  // row of this thread within the tile
-        const float lsum = ctrl->epi_l[islot][0][row] + ctrl->epi_l[islot][1][row];
+        const float m0 = ctrl->epi_m[islot][0][row], m1 = ctrl->epi_m[islot][1][row];
+        const float l0 = ctrl->epi_l[islot][0][row], l1 = ctrl->epi_l[islot][1][row];
+        const float lsum = (m0 == m1) ? l0 + l1 : fmaf(l0, ex2_approx(m0 - m1), l1);
         const float inv = partial ? 1.0f : (lsum > 0.f ? 1.0f / lsum : 0.f);
+        if (partial) {     // split-K: the row's state (reference maximum, row sum) beside the unnormalised O
+          const int g_r = row / cpt, cl_r = row - g_r * cpt;
+          if (cl_r < nh) {
+            const size_t prow = ((static_cast<size_t>(it.layer) * args.total_q + it.c0 + rank * cpt + cl_r) * args.H_q +
+                                 it.hkv * G + g_r) * args.num_splits + it.split;
+            args.part_ml[prow * 2 + 0] = m1;
+            args.part_ml[prow * 2 + 1] = lsum;
+          }
+        }
         const float2 sc2 = make_float2(inv, inv);
         const int cand0 = it.c0 + static_cast<int>(rank) * cpt;       // first candidate of this CTA's tile
         const size_t lrow0 = static_cast<size_t>(it.layer) * args.total_q;
