@@ -676,8 +676,8 @@ upr_attn_pair_kernel(const __grid_constant__ CUtensorMap tmap_k,    // [rows, 12
               pr[(c >> 1) + 0] = w01;
               pr[(c >> 1) + 1] = w23;
               // the row sum adds the bf16-ROUNDED weights: out stays a convex combination of V rows
-              sumA = fadd2(sumA, make_float2(__uint_as_float(w01 << 16), __uint_as_float(w01 & 0xffff0000u)));
-              sumB = fadd2(sumB, make_float2(__uint_as_float(w23 << 16), __uint_as_float(w23 & 0xffff0000u)));
+              add_bf16x2_f32(sumA.x, sumA.y, w01);
+              add_bf16x2_f32(sumB.x, sumB.y, w23);
             }
             // P(g, wg): packed bf16 pairs over the group's own S columns
             tmem_st16(tm_s + (c0 >> 1), pr);

@@ -892,10 +892,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
               const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
               pr[(c >> 1) + 0] = w01;
               pr[(c >> 1) + 1] = w23;
-              sumA = fadd2(sumA, make_float2(__uint_as_float(w01 << 16),
-                                             __uint_as_float(w01 & 0xffff0000u)));
-              sumB = fadd2(sumB, make_float2(__uint_as_float(w23 << 16),
-                                             __uint_as_float(w23 & 0xffff0000u)));
+              add_bf16x2_f32(sumA.x, sumA.y, w01);
+              add_bf16x2_f32(sumB.x, sumB.y, w23);
             }
             tmem_st16(tm_sb + (c0 >> 1), pr);
           }
