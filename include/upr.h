@@ -201,9 +201,11 @@ int upr_cross_attn_num_splits(const upr_attn_params* p);
  * a2-a8 -- extended forward. As upr_cross_attn_fwd, per layer, plus:
  *  - self term (k_self/v_self non-NULL): logit scale*<q_c, k_self_c> joins candidate c's
  *    softmax and v_self_c its weighted sum; with L_b == 0 the output is v_self_c.
- *  - FP8: K = e4m3(byte) * k_scale[l*H+h], V likewise; dequantised in registers (exactly), MMA
- *    in bf16.  The cache must hold finite codes (upr_kv_pack's satfinite conversion guarantees
- *    it): the NaN code S.1111.111 is not special-cased and decodes to +-480.
+ *  - FP8: K = e4m3(byte) * k_scale[l*H+h], V likewise; dequantised in registers (exactly: one
+ *    cvt to fp16 per two bytes), MMA in fp16 -- q is converted to fp16 on its way into shared
+ *    memory (exact for 2^-14 <= |q| < 65504, saturating above, rounded below), the softmax
+ *    weights are packed as fp16.  The cache must hold finite codes (upr_kv_pack's satfinite
+ *    conversion guarantees it): the NaN code S.1111.111 is not special-cased and stays a NaN.
  *  - split-K: the history is cut into num_splits ranges of whole 128-key tiles, each CTA
  *    writes its partial (m, l, O~) to the workspace and a combine kernel merges them.
  * Errors: WORKSPACE if workspace is NULL/too small; others as above.

@@ -122,8 +122,12 @@ struct AttnCfg {
   static constexpr int kSmemCtrl = 6144;
   static constexpr int kSmemTotal =
       kSmemQ + kSmemKV + kSmemRaw + kSmemEpi + kSmemCtrl + 1024;  // + alignment slack
-  static constexpr uint32_t kIdescQK = make_idesc_bf16(kTileM, kSubN, 0, 0);
-  static constexpr uint32_t kIdescPV = make_idesc_bf16(kTileM, D, 0, 1);
+  // FP8 caches multiply in fp16 (Q converted on the way into shared memory, K / V from E4M3 by one cvt per two
+  // bytes, P packed as fp16): every E4M3 value and every weight <= 2^8 is representable, and the converter warps
+  // need a quarter of the instructions of the bf16 route.  bf16 / fp32 caches multiply in bf16.
+  static constexpr bool kF16 = (KV == KV_FP8);
+  static constexpr uint32_t kIdescQK = kF16 ? make_idesc_f16(kTileM, kSubN, 0, 0) : make_idesc_bf16(kTileM, kSubN, 0, 0);
+  static constexpr uint32_t kIdescPV = kF16 ? make_idesc_f16(kTileM, D, 0, 1) : make_idesc_bf16(kTileM, D, 0, 1);
   static_assert(kSmemTotal <= 232448, "exceeds the 227 KB shared memory of an sm_100 CTA");
 };
 
@@ -186,7 +190,7 @@ __device__ __forceinline__ void user_sizes(const AttnArgs& a, int u, int& w, int
 // Q tile: global [rows, H*D] (bf16 or fp32) -> bf16 smem in the 128B-swizzled K-major layout
 // the UMMA descriptor expects (identical to what a SWIZZLE_128B TMA box would write).
 // ---------------------------------------------------------------------------------------
-template <int D>
+template <int D, bool kToF16 = false>
 __device__ __forceinline__ void load_q_tile(uint32_t tile_smem, const void* q, bool q_is_f32,
                                             size_t elem_base, size_t row_stride, int rows_valid,
                                             int tid128) {
@@ -200,13 +204,19 @@ __device__ __forceinline__ void load_q_tile(uint32_t tile_smem, const void* q, b
       size_t e = elem_base + static_cast<size_t>(row) * row_stride + static_cast<size_t>(c) * 8;
       if (!q_is_f32) {
         v = __ldg(reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(q) + e));
+        if (kToF16) {   // bf16 -> fp16 (exact for |x| in fp16's normal range; saturating beyond it)
+          v.x = pack_f16x2(__uint_as_float(v.x << 16), __uint_as_float(v.x & 0xffff0000u));
+          v.y = pack_f16x2(__uint_as_float(v.y << 16), __uint_as_float(v.y & 0xffff0000u));
+          v.z = pack_f16x2(__uint_as_float(v.z << 16), __uint_as_float(v.z & 0xffff0000u));
+          v.w = pack_f16x2(__uint_as_float(v.w << 16), __uint_as_float(v.w & 0xffff0000u));
+        }
       } else {
         const float4* p = reinterpret_cast<const float4*>(static_cast<const float*>(q) + e);
         float4 a = __ldg(p), b = __ldg(p + 1);
-        v.x = pack_bf16x2(a.x, a.y);
-        v.y = pack_bf16x2(a.z, a.w);
-        v.z = pack_bf16x2(b.x, b.y);
-        v.w = pack_bf16x2(b.z, b.w);
+        v.x = kToF16 ? pack_f16x2(a.x, a.y) : pack_bf16x2(a.x, a.y);
+        v.y = kToF16 ? pack_f16x2(a.z, a.w) : pack_bf16x2(a.z, a.w);
+        v.z = kToF16 ? pack_f16x2(b.x, b.y) : pack_bf16x2(b.x, b.y);
+        v.w = kToF16 ? pack_f16x2(b.z, b.w) : pack_bf16x2(b.z, b.w);
       }
     }
     int box = c >> 3, cc = c & 7;
@@ -271,24 +281,6 @@ __device__ __forceinline__ float row_dot(const void* a, const void* b, bool is_f
     }
   }
   return acc;
-}
-
-// Four E4M3 bytes -> two bf16x2 words, exactly.  The 7 magnitude bits are placed so that the
-// E4M3 exponent sits in the low bits of the bf16 exponent field (value scaled by 2^-120,
-// E4M3 subnormals become bf16 subnormals of the same mantissa), then a packed bf16 multiply
-// by 2^120 restores the value; every E4M3 value is representable in bf16, so the product is
-// exact.  (S.1111.111, E4M3's NaN, decodes to +-480: caches must hold finite codes, as
-// upr_kv_pack's satfinite conversion guarantees.)
-__device__ __forceinline__ void e4m3x4_to_bf16x4(uint32_t w, uint32_t& lo, uint32_t& hi) {
-  const __nv_bfloat162 k = __halves2bfloat162(__ushort_as_bfloat16(0x7B80), __ushort_as_bfloat16(0x7B80));
-  uint32_t a = __byte_perm(w, 0u, 0x1404);  // halves: b0 << 8, b1 << 8
-  uint32_t b = __byte_perm(w, 0u, 0x3424);  //         b2 << 8, b3 << 8
-  a = (a & 0x80008000u) | ((a >> 4) & 0x07f007f0u);
-  b = (b & 0x80008000u) | ((b >> 4) & 0x07f007f0u);
-  __nv_bfloat162 ra = __hmul2(*reinterpret_cast<__nv_bfloat162*>(&a), k);
-  __nv_bfloat162 rb = __hmul2(*reinterpret_cast<__nv_bfloat162*>(&b), k);
-  lo = *reinterpret_cast<uint32_t*>(&ra);
-  hi = *reinterpret_cast<uint32_t*>(&rb);
 }
 
 // ---------------------------------------------------------------------------------------
@@ -681,10 +673,10 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
                 const int row = p / PPR, c16 = p % PPR;
                 const uint4 v = lds128(raw + p * 16);
                 uint32_t o[8];
-                e4m3x4_to_bf16x4(v.x, o[0], o[1]);
-                e4m3x4_to_bf16x4(v.y, o[2], o[3]);
-                e4m3x4_to_bf16x4(v.z, o[4], o[5]);
-                e4m3x4_to_bf16x4(v.w, o[6], o[7]);
+                e4m3x4_to_f16x4(v.x, o[0], o[1]);
+                e4m3x4_to_f16x4(v.y, o[2], o[3]);
+                e4m3x4_to_f16x4(v.z, o[4], o[5]);
+                e4m3x4_to_f16x4(v.w, o[6], o[7]);
                 const int ca = 2 * c16, cb = 2 * c16 + 1;
                 const uint32_t rbase = tile + row * 128;
                 sts128(rbase + (ca >> 3) * Cfg::kBoxBytes + (((ca & 7) ^ (row & 7)) << 4), o[0], o[1],
@@ -730,8 +722,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     uint32_t sf_it[2] = {0, 0};              // s_full phase counters per S buffer
     uint32_t pv_cnt = 0;                     // PV sub-tile MMAs of this tile issued so far (all items)
     // share of exponentials on the FMA pipe: -1 none, 1 -> 25 %, 0 -> 50 %.  Measured (A/B in one
-    // run): d = 64 bf16 cache +7.5 % at 25 %, +3.6 % at 50 %; d = 128 -2.5 %; FP8 cache -7 % (the
-    // converter warps already load the FMA / ALU pipes) -- so only d = 64 with a bf16 cache uses it.
+    // run): d = 64 bf16 cache +7.5 % at 25 %, +3.6 % at 50 %; d = 128 -2.5 %; FP8 cache -7 % with the bf16
+    // converters, -0.6 % / -3.7 % at 25 % / 50 % with the fp16 route -- so only d = 64 with a bf16 cache uses it.
     constexpr int kPolyMask = (D == 64 && KV == KV_BF16) ? 1 : -1;
     const bool has_self = (args.k_self != nullptr);
     const bool q32 = args.q_is_f32 != 0;
@@ -744,8 +736,8 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
     };
     auto issue_q = [&](const WorkItem& w) {
       const int rows = min(kTileM, w.n_rows - t * kTileM);
-      if (q32)
-        load_q_tile<D>(q_tile_smem, args.q, true, tile_elem0_of(w), row_stride, rows, tid128);
+      if (q32 || Cfg::kF16)
+        load_q_tile<D, Cfg::kF16>(q_tile_smem, args.q, q32, tile_elem0_of(w), row_stride, rows, tid128);
       else
         load_q_tile_async<D>(q_tile_smem, args.q, tile_elem0_of(w), row_stride, rows, tid128);
     };
@@ -889,11 +881,17 @@ upr_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_k,
                 p2 = ex2_approx(x23.x);
                 p3 = ex2_approx(x23.y);
               }
-              const uint32_t w01 = pack_bf16x2(p0, p1), w23 = pack_bf16x2(p2, p3);
+              const uint32_t w01 = Cfg::kF16 ? pack_f16x2(p0, p1) : pack_bf16x2(p0, p1);
+              const uint32_t w23 = Cfg::kF16 ? pack_f16x2(p2, p3) : pack_bf16x2(p2, p3);
               pr[(c >> 1) + 0] = w01;
               pr[(c >> 1) + 1] = w23;
-              add_bf16x2_f32(sumA.x, sumA.y, w01);
-              add_bf16x2_f32(sumB.x, sumB.y, w23);
+              if (Cfg::kF16) {
+                add_f16x2_f32(sumA.x, sumA.y, w01);
+                add_f16x2_f32(sumB.x, sumB.y, w23);
+              } else {
+                add_bf16x2_f32(sumA.x, sumA.y, w01);
+                add_bf16x2_f32(sumB.x, sumB.y, w23);
+              }
             }
             tmem_st16(tm_sb + (c0 >> 1), pr);
           }
