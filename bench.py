@@ -546,10 +546,10 @@ def run_ours(args):
     t_mem = w.kv_bytes / (peaks["hbm_gbs"] * 1e9)
     roof_ms = 1e3 * max(t_flop, t_mem)
     # ncu counters cannot be read from inside an unprofiled run: the DRAM bytes of the ncu capture of this kernel on
-    # this workload are recorded in profiles/r2m_traffic.json (None when there is no capture for it)
+    # this workload are recorded in profiles/r2n_traffic.json (None when there is no capture for it)
     traffic, traffic_source = None, "no ncu capture recorded for this workload"
     try:
-        rec = json.load(open(os.path.join(ROOT, "profiles", "r2m_traffic.json"))).get(w.name)
+        rec = json.load(open(os.path.join(ROOT, "profiles", "r2n_traffic.json"))).get(w.name)
         if rec and rec["kernel"] == attn_kernel_name:
             traffic, traffic_source = rec["dram_read"] + rec["dram_write"], rec["source"] + " (ncu dram__bytes_read.sum + dram__bytes_write.sum, one launch)"
     except OSError:
