@@ -90,6 +90,16 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
 
   int cur_lh = -1;        // amax pass: (layer, head) of the running maximum
   float run_max = 0.f;
+  // The warp walks its blocks in order, so (layer * H + head, row block, user) are carried along instead of being
+  // recomputed per block (a 64-bit division, a modulo and a binary search over the users cost more than moving the
+  // block's 2 - 4 KB: the d = 64 passes ran at 4.3 - 4.8 TB/s with the ALU pipe at 35 - 43 %).
+  int w_lh = 0, w_rb = 0, w_b = 0;
+  if (blk0 < blk1) {
+    w_lh = static_cast<int>(blk0 / blocks_per_head);
+    w_rb = static_cast<int>(blk0 - static_cast<long long>(w_lh) * blocks_per_head);
+    w_b = find_user(row_off, a.B, w_rb * kPackRowBlock);
+  }
+  int w_l = w_lh / a.H, w_h = w_lh - w_l * a.H;
   for (long long blk = blk0; blk < blk1; blk += U) {
     uint4 v[U][NI];
     size_t dst_elem[U];
@@ -104,11 +114,19 @@ __global__ void __launch_bounds__(kPackThreads) upr_pack_kernel(const PackArgs a
 #pragma unroll
       for (int i = 0; i < NI; ++i) v[u][i] = make_uint4(0u, 0u, 0u, 0u);
       if (bk < blk1) {
-        const int rb = static_cast<int>(bk % blocks_per_head);
-        const int lh = static_cast<int>(bk / blocks_per_head);
-        const int h = lh % a.H, l = lh / a.H;
-        const int row = rb * kPackRowBlock;
-        const int b = find_user(row_off, a.B, row);
+        const int lh = w_lh, h = w_h, l = w_l;
+        const int row = w_rb * kPackRowBlock;
+        while (row >= row_off[w_b + 1]) ++w_b;               // (users without rows are skipped)
+        const int b = w_b;
+        if (++w_rb == blocks_per_head) {                     // next block: first rows of the next (layer, head)
+          w_rb = 0;
+          w_b = 0;
+          ++w_lh;
+          if (++w_h == a.H) {
+            w_h = 0;
+            ++w_l;
+          }
+        }
         const int j0 = row - row_off[b];                     // first key index of this block
         const int valid_rows = max(0, min(kPackRowBlock, __ldg(a.seq_lens + b) - j0));
         const int slot = __ldg(a.slot_ids + b);
