@@ -2,6 +2,8 @@
 same seeded inputs.  Tolerances are BASELINE.json's: max-abs 1e-2 for bf16 K/V (5e-2 for FP8),
 unit-variance inputs; the stricter self-imposed gates of SURVEY.md 8(c) are asserted too.
 Integer / byte outputs (layout tables, packed caches) must match bit for bit."""
+import math
+
 import numpy as np
 import pytest
 import torch
@@ -526,6 +528,51 @@ def test_peaked_queries_and_custom_scale(P):
     got2, _, _ = run_cuda(P, inp, sm_scale=0.05)
     mx2, _ = error_stats(got2, oracle_all(inp, sm_scale=0.05))
     assert mx2 <= TOL_BF16, mx2
+
+
+# Positions (key index) of planted dominant keys, per case: each later one out-weighs everything before it by far more
+# than the lazy-rescale threshold 2^8, so the reference maximum MOVES at exactly these half tiles.  The CTA-pair kernel
+# hands the reference from half tile to half tile (columns [0,64) of a 128-key tile belong to softmax group 0,
+# [64,128) to group 1; the group that moves it rescales the whole O row): the cases put the moves in group 0's
+# columns, in group 1's, in consecutive half tiles, in the first tile, and in the last (partial) tile, where group 1's
+# step is the item's last and the epilogue has to bring group 0's row sum to group 1's reference.
+PLANTED_CASES = [
+    ("half0_then_half1", [130, 330]),          # tile 1 half 0, tile 2 half 1
+    ("half1_then_half0", [200, 390]),          # tile 1 half 1, tile 3 half 0
+    ("same_tile_both_halves", [260, 330]),     # tile 2 half 0 then tile 2 half 1
+    ("first_tile_only", [5, 70]),              # both halves of tile 0, nothing later
+    ("last_key_of_partial_tile", [100, 699]),  # ..., the very last key (tile 5 of a 700-key history, half 0)
+    ("last_tile_half1", [64, 620]),            # tile 4 half 1 = last full-width half tile before the tail
+    ("every_half_tile", [10, 75, 140, 200, 270, 330, 400, 460, 520, 590, 650]),
+]
+
+
+@pytest.mark.parametrize("case", PLANTED_CASES, ids=[c[0] for c in PLANTED_CASES])
+@pytest.mark.parametrize("num_splits", [1, 2])
+def test_pair_kernel_reference_handover_with_planted_maxima(P, case, num_splits):
+    name, positions = case
+    w = S.custom_workload("planted_" + name, 97, [700, 257, 64], [300, 129, 140], H=2, d=128, n_layers=1)
+    inp = Inputs(w, "cuda")
+    d = w.d
+    u = torch.zeros(d, dtype=torch.float32, device="cuda")
+    u[::2] = 1.0
+    u /= u.norm()
+    # every query gets a common component along u, every planted key points along u with a growing amplitude:
+    # planted logits are (4 + N(0,1)) * amp / sqrt(d) -- 10, 20, 30, ... natural-log units apart
+    inp.q.copy_((inp.q.float() + 4.0 * u * math.sqrt(d) / 2.0).to(torch.bfloat16))
+    for b in range(w.B):
+        Lb, s = int(w.seq_lens[b]), int(inp.slot_ids_host[b])
+        for i, pos in enumerate(p for p in positions if p < Lb):
+            inp.k_pool[0, s, :, pos, :] = ((i + 1) * 5.0 * u).to(torch.bfloat16)
+    want = oracle_all(inp)
+    for runner in (run_cuda, run_cuda_pool):
+        res = runner(P, inp, num_splits=num_splits, kernel=P.UPR_KERNEL_PAIR)
+        assert P.upr_last_attn_kernel() == "upr_attn_pair_kernel"
+        got = res[0]
+        assert np.all(np.isfinite(got))
+        mx, rel = error_stats(got, want)
+        # rows are dominated by one or two keys: bf16 rounding of P (2^-9) x max|v| <= 4.3, DESIGN.md section 6
+        assert mx <= 2e-2 and rel <= 1e-2, (name, num_splits, runner.__name__, mx, rel)
 
 
 def test_basic_entry_point_and_candidate_permutation(P):
