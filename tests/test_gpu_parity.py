@@ -544,16 +544,20 @@ PLANTED_CASES = [
     ("last_key_of_partial_tile", [100, 699]),  # ..., the very last key (tile 5 of a 700-key history, half 0)
     ("last_tile_half1", [64, 620]),            # tile 4 half 1 = last full-width half tile before the tail
     ("every_half_tile", [10, 75, 140, 200, 270, 330, 400, 460, 520, 590, 650]),
+    # the 768-key user's very last key, in group 1's columns of its last tile: the item ends with the two groups'
+    # row sums relative to DIFFERENT references (group 0 never sees the move), which the epilogue must reconcile
+    ("last_step_of_item", [300, 767]),
 ]
 
 
 @pytest.mark.parametrize("case", PLANTED_CASES, ids=[c[0] for c in PLANTED_CASES])
 @pytest.mark.parametrize("num_splits", [1, 2])
-def test_pair_kernel_reference_handover_with_planted_maxima(P, case, num_splits):
+@pytest.mark.parametrize("kern,d", [("pair", 128), ("single", 128), ("single", 64)])
+def test_lazy_rescale_with_planted_maxima(P, case, num_splits, kern, d):
+    """(the 1-CTA kernel takes the same cases: one thread per row there, 64-key steps, the thread rescales its O row)"""
     name, positions = case
-    w = S.custom_workload("planted_" + name, 97, [700, 257, 64], [300, 129, 140], H=2, d=128, n_layers=1)
+    w = S.custom_workload("planted_" + name, 97, [700, 257, 64, 768], [300, 129, 140, 150], H=2, d=d, n_layers=1)
     inp = Inputs(w, "cuda")
-    d = w.d
     u = torch.zeros(d, dtype=torch.float32, device="cuda")
     u[::2] = 1.0
     u /= u.norm()
@@ -566,13 +570,14 @@ def test_pair_kernel_reference_handover_with_planted_maxima(P, case, num_splits)
             inp.k_pool[0, s, :, pos, :] = ((i + 1) * 5.0 * u).to(torch.bfloat16)
     want = oracle_all(inp)
     for runner in (run_cuda, run_cuda_pool):
-        res = runner(P, inp, num_splits=num_splits, kernel=P.UPR_KERNEL_PAIR)
-        assert P.upr_last_attn_kernel() == "upr_attn_pair_kernel"
+        res = runner(P, inp, num_splits=num_splits,
+                     kernel=P.UPR_KERNEL_PAIR if kern == "pair" else P.UPR_KERNEL_SINGLE)
+        assert P.upr_last_attn_kernel() == ("upr_attn_pair_kernel" if kern == "pair" else "upr_attn_fwd_kernel")
         got = res[0]
         assert np.all(np.isfinite(got))
         mx, rel = error_stats(got, want)
         # rows are dominated by one or two keys: bf16 rounding of P (2^-9) x max|v| <= 4.3, DESIGN.md section 6
-        assert mx <= 2e-2 and rel <= 1e-2, (name, num_splits, runner.__name__, mx, rel)
+        assert mx <= 2e-2 and rel <= 1e-2, (name, num_splits, kern, d, runner.__name__, mx, rel)
 
 
 def test_basic_entry_point_and_candidate_permutation(P):
