@@ -550,13 +550,24 @@ PLANTED_CASES = [
 ]
 
 
-@pytest.mark.parametrize("case", PLANTED_CASES, ids=[c[0] for c in PLANTED_CASES])
+# (case, amplitude planted on the candidates' own keys or None for no self term): the self-term variants run on three
+# of the cases
+PLANTED_PARAMS = [(c, None) for c in PLANTED_CASES] + [
+    (c, amp) for c in PLANTED_CASES if c[0] in ("half1_then_half0", "last_step_of_item", "first_tile_only")
+    for amp in (0.0, 2.0, 60.0)]
+
+
+@pytest.mark.parametrize("case,self_amp", PLANTED_PARAMS,
+                         ids=[c[0] + ("" if a is None else f"-self{a:g}") for c, a in PLANTED_PARAMS])
 @pytest.mark.parametrize("num_splits", [1, 2])
 @pytest.mark.parametrize("kern,d", [("pair", 128), ("single", 128), ("single", 64)])
-def test_lazy_rescale_with_planted_maxima(P, case, num_splits, kern, d):
-    """(the 1-CTA kernel takes the same cases: one thread per row there, 64-key steps, the thread rescales its O row)"""
+def test_lazy_rescale_with_planted_maxima(P, case, num_splits, kern, d, self_amp):
+    """(the 1-CTA kernel takes the same cases: one thread per row there, 64-key steps, the thread rescales its O row.
+    With a self term the candidate's own key is planted too: negligible, comparable to the history's dominant keys,
+    or dominant itself -- in the pair kernel it is the LAST key tile of the item and then moves the reference there.)"""
     name, positions = case
-    w = S.custom_workload("planted_" + name, 97, [700, 257, 64, 768], [300, 129, 140, 150], H=2, d=d, n_layers=1)
+    w = S.custom_workload("planted_" + name, 97, [700, 257, 64, 768], [300, 129, 140, 150], H=2, d=d, n_layers=1,
+                          self_term=self_amp is not None)
     inp = Inputs(w, "cuda")
     u = torch.zeros(d, dtype=torch.float32, device="cuda")
     u[::2] = 1.0
@@ -568,6 +579,8 @@ def test_lazy_rescale_with_planted_maxima(P, case, num_splits, kern, d):
         Lb, s = int(w.seq_lens[b]), int(inp.slot_ids_host[b])
         for i, pos in enumerate(p for p in positions if p < Lb):
             inp.k_pool[0, s, :, pos, :] = ((i + 1) * 5.0 * u).to(torch.bfloat16)
+    if self_amp:
+        inp.k_self.copy_((inp.k_self.float() + self_amp * u).to(torch.bfloat16))
     want = oracle_all(inp)
     for runner in (run_cuda, run_cuda_pool):
         res = runner(P, inp, num_splits=num_splits,
