@@ -593,6 +593,50 @@ def test_lazy_rescale_with_planted_maxima(P, case, num_splits, kern, d, self_amp
         assert mx <= 2e-2 and rel <= 1e-2, (name, num_splits, kern, d, runner.__name__, mx, rel)
 
 
+def _plant(inp, positions, q_shift=4.0):
+    """Common component along u on every query, dominant keys along u at `positions` (growing amplitude)."""
+    w, d = inp.w, inp.w.d
+    u = torch.zeros(d, dtype=torch.float32, device="cuda")
+    u[::2] = 1.0
+    u /= u.norm()
+    inp.q.copy_((inp.q.float() + q_shift * u * math.sqrt(d) / 2.0).to(torch.bfloat16))
+    for b in range(w.B):
+        Lb, s = int(w.seq_lens[b]), int(inp.slot_ids_host[b])
+        for i, pos in enumerate(p for p in positions if p < Lb):
+            inp.k_pool[:, s, :, pos, :] = ((i + 1) * 5.0 * u).to(torch.bfloat16)
+
+
+@pytest.mark.parametrize("Hkv", [2, 1])
+@pytest.mark.parametrize("num_splits", [1, 2])
+def test_lazy_rescale_planted_maxima_grouped_queries(P, Hkv, num_splits):
+    """The same with the query group folded into M (rows of a tile are g-major: 128 / G candidates x G heads)."""
+    w = S.custom_workload("planted_gqa", 98, [700, 257, 768], [150, 70, 33], 4, 128, 1, n_max=800)
+    inp = Inputs(w, "cuda", H_kv=Hkv)
+    _plant(inp, [70, 200, 330, 390, 620, 767])
+    want = oracle_all(inp)
+    for runner in (run_cuda, run_cuda_pool):
+        got = runner(P, inp, num_splits=num_splits, kernel=P.UPR_KERNEL_PAIR)[0]
+        assert P.upr_last_attn_kernel() == "upr_attn_pair_kernel"
+        mx, rel = error_stats(got, want)
+        assert np.all(np.isfinite(got)) and mx <= 2e-2 and rel <= 1e-2, (Hkv, num_splits, runner.__name__, mx, rel)
+
+
+def test_lazy_rescale_planted_maxima_causal(P):
+    """Causal mode (history prefill): row cl sees keys j <= cl + (L_b - C_b), so rows of one tile see DIFFERENT numbers
+    of the planted keys -- the reference moves for some rows of a warp and not for others."""
+    from paper_2606_00422_b200 import pipeline as pl
+    w = S.custom_workload("planted_causal", 99, [700, 300, 513], [700, 120, 513], 2, 128, 1, n_max=800)
+    inp = Inputs(w, "cuda")
+    _plant(inp, [5, 70, 130, 200, 330, 390, 500, 620, 699])
+    src = pl.PoolView.of(inp.k_pool, inp.v_pool, inp.slot_ids, w.seq_lens)
+    attn = pl.CrossAttention(src, w.cand_offsets, P.UPR_BF16, H_q=2, causal=True)
+    got = attn(inp.q).cpu().numpy()
+    torch.cuda.synchronize()
+    assert P.upr_last_attn_kernel() == "upr_attn_pair_kernel"
+    mx, rel = error_stats(got, _causal_oracle(inp))
+    assert np.all(np.isfinite(got)) and mx <= 2e-2 and rel <= 1e-2, (mx, rel)
+
+
 def test_basic_entry_point_and_candidate_permutation(P):
     """upr_cross_attn_fwd (the named entry point: the library reads the row count from the device and supplies the
     workspace); permuting a user's candidates permutes its outputs."""
