@@ -352,6 +352,61 @@ def decode_layer_leg(P, pl, w, k_pool, v_pool, slots, stream, dev, ev, hidden_mu
             "fp8_mlp_layer_tflops": (gemm_flops + attn_flops) / (ms8 * 1e-3) / 1e12}
 
 
+def prefill_leg(P, pl, w, pool_shape, slots_host, stream, dev, ev, iters=5):
+    """SURVEY 8(f)2, second half, timed: the history prefill of ONE layer over the workload's histories (PAPER.md:138,
+    198, 202) -- K / V projections of the history tokens written straight into the pool layout [1,S,H,n,D] by the GEMM's
+    epilogue, the Q projection, and the causal O(n^2) self-attention reading those slots in place (pair kernel,
+    causal = 1).  Own pools (the workload's are not touched); synthetic weights; C-ABI calls only."""
+    import math
+    _, S_slots, H, n_max, d = pool_shape
+    D = H * d
+    L = w.seq_lens.astype(np.int64)
+    M = int(L.sum())
+    x = S.normal_bf16(w.seed, "pf_x", (M, D), dev)
+
+    def wgt(tag):
+        return (S.normal_bf16(w.seed, tag, (D, D), dev).float() / math.sqrt(D)).to(torch.bfloat16)
+    wq, wk, wv = wgt("pf_wq"), wgt("pf_wk"), wgt("pf_wv")
+    tok_slot = torch.from_numpy(np.repeat(np.asarray(slots_host, dtype=np.int32), L)).to(dev)
+    tok_pos = torch.from_numpy(np.concatenate([np.arange(n, dtype=np.int32) for n in L])).to(dev)
+    kp = torch.zeros((1, S_slots, H, n_max, d), dtype=torch.bfloat16, device=dev)
+    vp = torch.zeros_like(kp)
+    qh = torch.empty((M, D), dtype=torch.bfloat16, device=dev)
+    co = np.concatenate([[0], np.cumsum(L)]).astype(np.int32)
+    view = pl.PoolView.of(kp, vp, torch.as_tensor(np.asarray(slots_host, dtype=np.int32), device=dev), w.seq_lens)
+    attn = pl.CrossAttention(view, co, P.UPR_BF16, causal=True)
+    e = [ev() for _ in range(3)]
+
+    def once(record=False):
+        if record:
+            e[0].record(stream)
+        P.upr_kv_project_into_pool(x, wk, None, kp, tok_slot, tok_pos, 0, stream)
+        P.upr_kv_project_into_pool(x, wv, None, vp, tok_slot, tok_pos, 0, stream)
+        P.upr_linear_fwd(x, wq, None, qh, P.UPR_ACT_NONE, stream)
+        if record:
+            e[1].record(stream)
+        attn(qh.view(1, M, H, d), stream=stream)
+        if record:
+            e[2].record(stream)
+    once(); once()
+    torch.cuda.synchronize()
+    proj_ms, attn_ms = [], []
+    for _ in range(iters):
+        once(record=True)
+        torch.cuda.synchronize()
+        proj_ms.append(e[0].elapsed_time(e[1]))
+        attn_ms.append(e[1].elapsed_time(e[2]))
+    pm, am = float(np.mean(proj_ms)), float(np.mean(attn_ms))
+    pairs = float((L * (L + 1) // 2).sum())
+    attn_flops = 4.0 * d * H * pairs                 # the visible (query, key) pairs only: QK^T and PV
+    proj_flops = 3 * 2.0 * M * D * D
+    return {"layers": 1, "history_tokens": M, "D_model": D, "proj_ms": pm, "attn_ms": am, "ms": pm + am,
+            "history_tokens_per_s": M / ((pm + am) * 1e-3), "visible_pairs": pairs,
+            "attn_flops_visible": attn_flops, "attn_tflops_visible": attn_flops / (am * 1e-3) / 1e12,
+            "proj_tflops": proj_flops / (pm * 1e-3) / 1e12, "kernel": P.upr_last_attn_kernel(),
+            "note": "causal tiles on the diagonal are half masked: issued MMA flops exceed the visible-pair count"}
+
+
 # ----------------------------------------------------------------------------- CUDA arm
 def run_ours(args):
     import paper_2606_00422_b200 as P
@@ -532,6 +587,8 @@ def run_ours(args):
         tail = ranking_tail(P, w, attn, q, k_self, v_self, q_host, stream, dev, ev)
         if w.kv_dtype == "bf16" and w.d == 128:
             tail["decode_layer"] = decode_layer_leg(P, pl, w, k_pool, v_pool, slots, stream, dev, ev)
+            if int(w.seq_lens.sum()) * w.H * w.d <= (1 << 29):      # bounded: <= 1 GiB of bf16 activations
+                tail["prefill"] = prefill_leg(P, pl, w, tuple(k_pool.shape), S.slot_ids(w), stream, dev, ev)
 
     if rank != 0:
         if dist is not None:
